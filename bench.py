@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py -- overrelaxation site-updates/s at 32^4 on B200 (BASELINE.json metric, configs[2]).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variant f64-18]
+
+One STEP = the whole hot path over one 32^4 lattice: ITERS overrelaxation iterations (omega = 1.7;
+each = half-sweep of parity 0 then parity 1) with an F/theta reduction every
+CHECK iterations (rows a7-a9), driven through the C ABI (gf_sweep / gf_measure).  ``value`` is
+site-updates/s with the field resident in HBM; ``e2e`` adds, every step, the host->device copy of
+the canonical field from pinned memory (gf_load_host) and the device->host copy of the fixed field
+(gf_store_host).  The field (604 MB in fp64) is larger than the 126 MB L2, so no flush is needed.
+N > 1: one independent lattice per GPU (replicas only, no data-path collective), weak scaling.
+
+--impl reference times the CPU oracle (oracle/, fp64, OpenMP over all host cores) on the same
+workload, one iteration per step; rank 0 only.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+DIMS = (32, 32, 32, 32)
+V = DIMS[0] * DIMS[1] * DIMS[2] * DIMS[3]
+OMEGA = 1.7
+EPS = 0.6
+SEED = 1
+FLOP_PER_SITE_UPDATE = 2136          # nominal count, SURVEY.md 8(d) / DESIGN.md
+METRIC = "overrelaxation site-updates/s at 32^4"
+VARIANTS = {            # name: (precision key, recon, bytes per real)
+    "f64-18": ("f64", 18, 8), "f64-12": ("f64", 12, 8),
+    "f32-18": ("f32", 18, 4), "f32-12": ("f32", 12, 4),
+}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import gf_inputs as gi
+    import paper_1305_3440_b200 as gf
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    peak, peak_src = measured_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # same recipe on every rank, rank-dependent seed: one independent configuration per GPU
+    U64 = gi.torch_smooth_random_gauge(DIMS, EPS, SEED + rank, device=dev)
+
+    def bench_variant(name, steps, warmup, with_e2e):
+        pkey, recon, B = VARIANTS[name]
+        prec = gf.GF_F64 if pkey == "f64" else gf.GF_F32
+        cdtype = torch.complex128 if pkey == "f64" else torch.complex64
+        fld = gf.GaugeField(DIMS, recon=recon, precisions=(pkey,), device=dev, staging=with_e2e)
+        Uc = U64.to(cdtype).contiguous()
+        fld.pack(Uc, prec)
+        n_blocks = args.iters // args.check
+        sweep_ms = []
+
+        def step(record):
+            for _ in range(n_blocks):
+                if record:
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                fld.iterate(args.check, gf.GF_OVERRELAX, OMEGA, 0.0, prec)
+                if record:
+                    b.record()
+                    sweep_ms.append((a, b))
+                fld.measure(prec)
+
+        for _ in range(warmup):
+            step(False)
+        launches0 = gf.gf_launch_count(fld.ctx)
+        sampler = ClockSampler(local_rank)
+        barrier()
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            step(True)
+        e1.record()
+        barrier()
+        clocks = sampler.stop()
+        ms_total = max_over_ranks(e0.elapsed_time(e1))
+        launches = gf.gf_launch_count(fld.ctx) - launches0
+        F, th = fld.measure(prec)
+        kern_ms = sum(a.elapsed_time(b) for a, b in sweep_ms) / (len(sweep_ms) * 2 * args.check)
+        bytes_per_launch = (V // 2) * 16 * recon * B
+        achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
+        out = {
+            "value": world * V * args.iters * steps / (ms_total * 1e-3),
+            "ms_per_step": ms_total / steps,
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
+                         "bytes_per_launch": bytes_per_launch, "avg_launch_ms": kern_ms, "peak_source": peak_src,
+                         "frac_of_8TBs_nominal": achieved / 8000.0},
+            "final_F": F[0], "final_theta": th[0],
+        }
+        if with_e2e:
+            host = torch.empty(fld.shape, dtype=cdtype).pin_memory()
+            host.copy_(Uc)
+            for _ in range(max(1, warmup // 2)):
+                fld.load_host(host, prec); step(False); fld.store_host(host, prec)
+            host.copy_(Uc)
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(steps):
+                fld.load_host(host, prec)
+                step(False)
+                fld.store_host(host, prec)          # synchronises: the fixed field is on the host
+            torch.cuda.synchronize()
+            dt = max_over_ranks(time.perf_counter() - t0)
+            nbytes = host.numel() * host.element_size()
+            out["e2e"] = {"value": world * V * args.iters * steps / dt, "unit": "site-updates/s",
+                          "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 16 * n_blocks,
+                          "ms_per_step": 1e3 * dt / steps}
+            del host
+        fld.close()
+        del fld, Uc
+        torch.cuda.empty_cache()
+        return out
+
+    main = bench_variant(args.variant, args.steps, args.warmup, True)
+    variants = {}
+    if not args.no_variants:
+        for name in VARIANTS:
+            if name == args.variant:
+                continue
+            r = bench_variant(name, max(1, args.steps // 3), 3, False)
+            variants[name] = {"site_updates_per_s": r["value"], "gflops_nominal": r["value"] * FLOP_PER_SITE_UPDATE / 1e9,
+                              "roofline_GBs": r["roofline"]["achieved"], "roofline_frac": r["roofline"]["frac"]}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(U64.cpu().numpy(), budget_s=12.0)
+
+    if rank == 0:
+        pkey, recon, _ = VARIANTS[args.variant]
+        line = {
+            "metric": METRIC, "value": main["value"], "unit": "site-updates/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": pkey, "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[2]: SU(3) Landau 32^4, overrelaxation omega=1.7, %s links "
+                                   "stored as %d reals, eps=0.6 smooth field + Haar gauge transform" % (pkey, recon),
+                       "lattice": list(DIMS), "iterations_per_step": args.iters, "theta_F_every": args.check,
+                       "l2": "field (%d MB) larger than L2, no flush" % (V * 4 * recon * VARIANTS[args.variant][2] // 2**20),
+                       "parallelism": "replicas only (one lattice per GPU)" if world > 1 else "single GPU"},
+            "gflops_nominal": main["value"] * FLOP_PER_SITE_UPDATE / 1e9,
+            "gpu_launches": main["gpu_launches"], "clocks": main["clocks"], "e2e": main["e2e"],
+            "roofline": main["roofline"], "cpu_baseline": cpu, "variants": variants,
+            "final_F": main["final_F"], "final_theta": main["final_theta"],
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(U, budget_s):
+    """The oracle as it stands, all host cores, full iterations of the same 32^4 workload until
+    `budget_s` seconds of wall time have passed (at least one iteration)."""
+    import oracle
+    cores = oracle.set_threads(0)
+    n, t0 = 0, time.perf_counter()
+    while True:
+        oracle.sweep(U, DIMS, 0, oracle.LANDAU, oracle.OVERRELAX, OMEGA)
+        oracle.sweep(U, DIMS, 1, oracle.LANDAU, oracle.OVERRELAX, OMEGA)
+        n += 1
+        dt = time.perf_counter() - t0
+        if dt >= budget_s:
+            break
+    oracle.set_threads(1)
+    return {"value": n * V / dt, "unit": "site-updates/s", "cores": cores, "kind": "oracle",
+            "sample": "%d full overrelaxation iteration(s) of the same 32^4 field, fp64, %.1f s" % (n, dt)}
+
+
+def run_reference(args):
+    """The reference arm of this tier = the CPU oracle, timed as it stands on the host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import gf_inputs as gi
+    import oracle
+    dims = DIMS
+    t_gen = time.perf_counter()
+    # a step is a bounded sample of the workload: ONE full iteration of the 32^4 lattice (about a
+    # second on a few cores), where a step of the CUDA arm is `--iters` iterations
+    U = gi.smooth_random_gauge(dims, EPS, SEED)
+    t_gen = time.perf_counter() - t_gen
+    cores = oracle.set_threads(0)
+
+    def step():
+        oracle.sweep(U, dims, 0, oracle.LANDAU, oracle.OVERRELAX, OMEGA)
+        oracle.sweep(U, dims, 1, oracle.LANDAU, oracle.OVERRELAX, OMEGA)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    val = args.steps * V / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "site-updates/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[2]: SU(3) Landau 32^4, overrelaxation omega=1.7, CPU oracle fp64",
+                   "lattice": list(dims), "iterations_per_step": 1},
+        "cpu_baseline": {"value": val, "unit": "site-updates/s", "cores": cores, "kind": "oracle",
+                         "sample": "each step = 1 full overrelaxation iteration of the 32^4 field (input generated in %.0f s)" % t_gen},
+        "e2e": {"value": val, "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gflops_nominal": val * FLOP_PER_SITE_UPDATE / 1e9,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variant", default="f64-18", choices=sorted(VARIANTS))
+    ap.add_argument("--iters", type=int, default=100, help="iterations per step")
+    ap.add_argument("--check", type=int, default=10, help="F/theta reduction every CHECK iterations")
+    ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

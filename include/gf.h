@@ -1,0 +1,167 @@
+/*
+ * gf.h -- C ABI of libgf_b200: SU(3) lattice gauge fixing by checkerboard relaxation on one
+ * NVIDIA B200 (sm_100a).
+ *
+ * The problem the calls follow (Schroeck & Vogt, arXiv:1305.3440; PAPER.md = its text):
+ * given links U_mu(x) in SU(3) on a periodic N_t x N_x x N_y x N_z lattice, find the gauge
+ * transformation g(x) that makes the functional F^g[U] (eq. 2) stationary, by
+ * sweeping over the two parity sublattices and replacing, at every site, the links
+ * by  g(x) U_mu(x)  and  U_mu(x-mu) g(x)^dagger  (eq. 3) with g(x) the local
+ * maximiser of Re tr[g(x) K(x)] (eq. 7-9), until the precision theta
+ * (eq. 4-5) falls below a target.
+ *
+ * Conventions
+ *   dims[4] = {N_t, N_x, N_y, N_z}, every extent even and >= 2, N_t <= 4096.
+ *   mu = 0 is time, mu = 1,2,3 = x,y,z.  parity(x) = (t+x+y+z) mod 2.
+ *   Canonical link layout (what callers hold): contiguous complex array of shape
+ *   (N_t, N_z, N_y, N_x, 4, 3, 3): site s = x + N_x (y + N_y (z + N_z t)), then mu, then the
+ *   3x3 matrix row-major, (re, im) interleaved; complex128 or complex64.
+ *   The internal device layout (parity-split, 16-byte-chunk structure of arrays, 18 or 12 reals
+ *   per link) is private; gf_pack / gf_unpack convert.
+ *
+ * Memory and streams
+ *   Every DEVICE buffer (link storage, workspace, canonical staging) is allocated by the caller
+ *   (e.g. a torch tensor's data_ptr()), must be 16-byte aligned, and is only borrowed by the
+ *   context until gf_destroy.  The library allocates no device memory (only a few KB of pinned
+ *   host memory for scalar results), launches work only on the stream given to gf_init_lattice,
+ *   and never synchronises the device except where stated.  Pointers named dev_* are device
+ *   pointers, host_* are host pointers.
+ *
+ * Errors
+ *   Every int-returning call returns GF_OK (0), a positive informational code with valid
+ *   outputs, or a negative error; nothing throws, aborts or prints.  gf_last_error gives the
+ *   text of the last error of a context.  Argument errors are detected before any launch, so a
+ *   call that fails with GF_EINVAL / GF_ESTATE leaves the link field unchanged.
+ */
+#ifndef GF_B200_H
+#define GF_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gf_ctx gf_ctx; /* opaque; owned by the library; freed by gf_destroy */
+
+enum { GF_OK = 0, GF_NOT_CONVERGED = 1, GF_EINVAL = -1, GF_ENOMEM = -2, GF_ECUDA = -3, GF_ESTATE = -4 };
+enum { GF_LANDAU = 0, GF_COULOMB = 1 };                   /* gauge */
+enum { GF_F32 = 0, GF_F64 = 1, GF_MIXED = 2 };            /* precision */
+enum { GF_RELAX = 0, GF_OVERRELAX = 1, GF_STOCHASTIC = 2 }; /* algo: PAPER.md:73, :80, :84 */
+enum { GF_RECON18 = 18, GF_RECON12 = 12 };                /* reals stored per link */
+
+/* Bytes of device memory one internal link field needs: 8 * (V/2) * recon * sizeof(real).
+ * precision is GF_F32 or GF_F64.  Returns 0 for invalid arguments. */
+size_t gf_storage_bytes(const int dims[4], int precision, int recon);
+
+/* Bytes of device scratch the reductions need (per-block partial sums).  0 if dims invalid. */
+size_t gf_workspace_bytes(const int dims[4]);
+
+/* Creates a context.  gauge: GF_LANDAU (K, F, theta over mu = 0..3) or
+ * GF_COULOMB (over the spatial mu = 1..3, F and theta per time slice; the transformation still
+ * acts on all eight links of a site).  recon: GF_RECON18 stores all 9 complex entries,
+ * GF_RECON12 stores rows 0 and 1 and rebuilds row 2 = conj(row0 x row1) on load.
+ * dev_links_f64 / dev_links_f32: storage of gf_storage_bytes() each, either may be NULL if that
+ * precision is never used (GF_MIXED needs both).  dev_workspace: gf_workspace_bytes().
+ * cuda_stream: a cudaStream_t (NULL = the legacy default stream).  seed: key of the Philox
+ * generator used by GF_STOCHASTIC; the half-sweep counter starts at 0.
+ * Errors: GF_EINVAL (bad dims / enum / alignment / both link pointers NULL), GF_ENOMEM,
+ * GF_ECUDA (no sm_100 device, ...; *out is then NULL). */
+int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
+                    void* dev_links_f32, void* dev_workspace, void* cuda_stream, uint64_t seed);
+
+/* canonical (device) -> internal field of `precision` (GF_F32 | GF_F64); converts the real type
+ * if canonical_is_f64 differs.  Asynchronous on the context's stream. */
+int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision);
+
+/* internal field of `precision` -> canonical (device); GF_RECON12 rebuilds row 2.  Asynchronous. */
+int gf_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision);
+
+/* Host-buffer variants: copy a canonical field between HOST memory (pinned for a truly
+ * asynchronous copy) and the internal field, staging through dev_staging (a caller-owned device
+ * buffer of V*4*9*2*sizeof(real of the canonical type) bytes).  gf_load_host is asynchronous;
+ * gf_store_host synchronises the stream before returning, so host_canonical is complete. */
+int gf_load_host(gf_ctx* ctx, const void* host_canonical, int canonical_is_f64, int precision,
+                 void* dev_staging);
+int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is_f64, int precision,
+                  void* dev_staging);
+
+/* One half-sweep: every site x of `parity` (0|1) forms
+ * K(x) = sum_mu [U_mu(x) + U_mu(x-mu)^dagger] (eq. 8, neighbours' g = 1), runs the three SU(2)
+ * subgroup maximisations (0,1), (0,2), (1,2) (eq. 9 on the SU(2) projection of each 2x2 block,
+ * K refreshed in between), modified per `algo`: GF_RELAX as is; GF_OVERRELAX a -> normalise(1 +
+ * omega (a - 1)), omega in [1,2); GF_STOCHASTIC a -> a^2 if u < p, p in [0,1], u the
+ * Philox4x32-10 draw of (seed; site, half-sweep counter; subgroup); then writes
+ * g U_mu(x) and U_mu(x-mu) g^dagger in place (eq. 3).  precision: GF_F32 | GF_F64 selects the
+ * field and the arithmetic.  Enqueues one kernel and returns without synchronising; increments
+ * the context's half-sweep counter.  Errors: GF_EINVAL (parity, algo, omega, p, precision),
+ * GF_ESTATE (no storage for that precision), GF_ECUDA. */
+int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision);
+
+/* F (eq. 2) and theta (eq. 4-5, with A_mu the traceless
+ * anti-Hermitian part of U_mu) of the field of `precision`, accumulated in fp64 with a fixed
+ * reduction order.  host_out receives 1 double (Landau) or N_t doubles (Coulomb: per time slice,
+ * spatial directions, normalised by N_s^3).  These calls synchronise the stream.
+ * gf_measure computes both in one pass over the field; either pointer may be NULL. */
+int gf_functional(gf_ctx* ctx, int precision, double* host_out);
+int gf_theta(gf_ctx* ctx, int precision, double* host_out);
+int gf_measure(gf_ctx* ctx, int precision, double* host_functional, double* host_theta);
+
+/* Iterates {gf_sweep(parity 0); gf_sweep(parity 1)} (= 1 iteration); after every
+ * iteration that is a multiple of check_every (and after the last) evaluates theta (Coulomb:
+ * max over slices) and stops when it is below theta_target.  precision GF_MIXED: fp32
+ * iterations until theta < max(theta_target, 1e-6), then gf_cast fp32->fp64 (with SU(3)
+ * re-projection) and fp64 iterations; the fp32 field must hold the input and the result is in
+ * the fp64 field.  *iters_out = iterations done (both phases), *theta_out = last theta.
+ * Returns GF_OK, or GF_NOT_CONVERGED (valid outputs) when max_iter was reached.  Synchronises. */
+int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int precision, double theta_target,
+                 int max_iter, int check_every, int* iters_out, double* theta_out);
+
+/* Sets the Philox key and the half-sweep counter (checkpoint/resume: the RNG state is just these). */
+int gf_set_rng(gf_ctx* ctx, uint64_t seed, uint32_t half_sweep_counter);
+int gf_get_counter(const gf_ctx* ctx, uint32_t* half_sweep_counter_out);
+
+/* Re-projects every link of the field onto SU(3) (Gram-Schmidt on rows 0,1; row 2 = conj cross). */
+int gf_reunitarize(gf_ctx* ctx, int precision);
+
+/* Copies the internal field of one precision into the other; fp32 -> fp64 also re-projects. */
+int gf_cast(gf_ctx* ctx, int from_precision, int to_precision);
+
+/* Diagnostics (synchronise).  gf_plaquette: mean plaquette 1/(6 N_c V) sum Re tr[U_mu(x)
+ * U_nu(x+mu) U_mu(x+nu)^dagger U_nu(x)^dagger], gauge invariant.  gf_unitarity: host_out[0] =
+ * max |U U^dagger - 1| entry, host_out[1] = max |det U - 1| over all links. */
+int gf_plaquette(gf_ctx* ctx, int precision, double* host_out);
+int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2);
+
+/* Kernel configuration of gf_sweep for `precision`: lanes_per_site in {1,2,4} threads cooperate
+ * on one site (each owns 8/lanes links; K is combined with warp shuffles); block_threads in
+ * {64,128,256,512}.  0 = keep the built-in default.  Results do not depend on it beyond the
+ * summation order inside K. */
+int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_threads);
+
+/* Arithmetic of the per-site solver when the STORAGE is fp32 (gf_sweep with GF_F32): K(x) is
+ * accumulated and the three SU(2) solves run in solver_precision: GF_F32 (everything in fp32),
+ * GF_F64 (fp64 registers: no extra memory traffic, ~15 % more time, removes the amplification of
+ * fp32 rounding at sites whose SU(2) projection |v| is small), or GF_SOLVER_AUTO (the default:
+ * GF_F64 for GF_STOCHASTIC, whose g -> g^2 step doubles that amplification, GF_F32 otherwise).
+ * The 3x3 products g U and U g^dagger are always formed in the storage precision.  No effect on
+ * GF_F64 sweeps. */
+enum { GF_SOLVER_AUTO = -1 };
+int gf_set_solver_precision(gf_ctx* ctx, int solver_precision);
+
+/* Runs the device Philox4x32-10 on n (counter, key) pairs: dev_counters n*4, dev_keys n*2,
+ * dev_out n*4 uint32 words (device pointers).  For known-answer tests.  Asynchronous. */
+int gf_debug_philox(gf_ctx* ctx, int n, const uint32_t* dev_counters, const uint32_t* dev_keys,
+                    uint32_t* dev_out);
+
+/* Number of kernels this context has launched so far (for launch accounting in benchmarks). */
+int gf_launch_count(const gf_ctx* ctx, uint64_t* count_out);
+
+const char* gf_last_error(const gf_ctx* ctx);
+void gf_destroy(gf_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GF_B200_H */

@@ -1,0 +1,18 @@
+"""paper_1305_3440_b200 -- B200-native SU(3) lattice gauge fixing (arXiv:1305.3440).
+
+Thin Python binding of ``libgf_b200.so`` (C ABI: ``include/gf.h``).  The functions below have the
+same names as the C entry points and only marshal arguments; every step of the method runs in
+the library's CUDA kernels.  PyTorch is used for device memory and streams only.  There is no CPU
+fallback: importing the binding without the built library raises.
+"""
+from .binding import (  # noqa: F401
+    GF_OK, GF_NOT_CONVERGED, GF_EINVAL, GF_ENOMEM, GF_ECUDA, GF_ESTATE,
+    GF_LANDAU, GF_COULOMB, GF_F32, GF_F64, GF_MIXED,
+    GF_RELAX, GF_OVERRELAX, GF_STOCHASTIC, GF_RECON18, GF_RECON12, GF_SOLVER_AUTO,
+    GFError, lib, lib_path,
+    gf_storage_bytes, gf_workspace_bytes, gf_init_lattice, gf_destroy, gf_last_error,
+    gf_pack, gf_unpack, gf_load_host, gf_store_host, gf_sweep, gf_functional, gf_theta,
+    gf_measure, gf_fix_until, gf_set_rng, gf_get_counter, gf_reunitarize, gf_cast,
+    gf_plaquette, gf_unitarity, gf_set_tuning, gf_set_solver_precision, gf_debug_philox, gf_launch_count,
+)
+from .field import GaugeField  # noqa: F401

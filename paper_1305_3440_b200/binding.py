@@ -1,0 +1,214 @@
+"""ctypes marshalling for libgf_b200.so -- one Python function per C entry point of include/gf.h.
+
+Device pointers are plain integers (``tensor.data_ptr()``), the stream is
+``torch.cuda.current_stream().cuda_stream``.  Calls return the C return code; negative codes
+raise ``GFError`` carrying ``gf_last_error``'s text unless ``check=False`` is passed.
+"""
+import ctypes as C
+import os
+
+GF_OK, GF_NOT_CONVERGED = 0, 1
+GF_EINVAL, GF_ENOMEM, GF_ECUDA, GF_ESTATE = -1, -2, -3, -4
+GF_LANDAU, GF_COULOMB = 0, 1
+GF_F32, GF_F64, GF_MIXED = 0, 1, 2
+GF_RELAX, GF_OVERRELAX, GF_STOCHASTIC = 0, 1, 2
+GF_RECON18, GF_RECON12 = 18, 12
+GF_SOLVER_AUTO = -1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+lib_path = os.path.join(_HERE, "libgf_b200.so")
+
+
+class GFError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("libgf_b200 error %d: %s" % (code, text))
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(lib_path):
+        raise ImportError(
+            "%s is missing: build it with `python paper_1305_3440_b200/build.py` "
+            "(there is no CPU or PyTorch fallback)" % lib_path)
+    L = C.CDLL(lib_path)
+    vp, i32, u32, u64, dbl = C.c_void_p, C.c_int, C.c_uint32, C.c_uint64, C.c_double
+    ip, dp = C.POINTER(C.c_int), C.POINTER(C.c_double)
+    sig = {
+        "gf_storage_bytes": (C.c_size_t, [ip, i32, i32]),
+        "gf_workspace_bytes": (C.c_size_t, [ip]),
+        "gf_init_lattice": (i32, [C.POINTER(vp), ip, i32, i32, vp, vp, vp, vp, u64]),
+        "gf_pack": (i32, [vp, vp, i32, i32]),
+        "gf_unpack": (i32, [vp, vp, i32, i32]),
+        "gf_load_host": (i32, [vp, vp, i32, i32, vp]),
+        "gf_store_host": (i32, [vp, vp, i32, i32, vp]),
+        "gf_sweep": (i32, [vp, i32, i32, dbl, dbl, i32]),
+        "gf_functional": (i32, [vp, i32, dp]),
+        "gf_theta": (i32, [vp, i32, dp]),
+        "gf_measure": (i32, [vp, i32, dp, dp]),
+        "gf_fix_until": (i32, [vp, i32, dbl, dbl, i32, dbl, i32, i32, ip, dp]),
+        "gf_set_rng": (i32, [vp, u64, u32]),
+        "gf_get_counter": (i32, [vp, C.POINTER(u32)]),
+        "gf_reunitarize": (i32, [vp, i32]),
+        "gf_cast": (i32, [vp, i32, i32]),
+        "gf_plaquette": (i32, [vp, i32, dp]),
+        "gf_unitarity": (i32, [vp, i32, dp]),
+        "gf_set_tuning": (i32, [vp, i32, i32, i32]),
+        "gf_set_solver_precision": (i32, [vp, i32]),
+        "gf_debug_philox": (i32, [vp, i32, vp, vp, vp]),
+        "gf_launch_count": (i32, [vp, C.POINTER(u64)]),
+        "gf_last_error": (C.c_char_p, [vp]),
+        "gf_destroy": (None, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(L, name)
+        f.restype, f.argtypes = res, args
+    return L
+
+
+lib = _load()
+EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
+           "gf_sweep gf_functional gf_theta gf_measure gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
+           "gf_cast gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_debug_philox gf_launch_count gf_last_error "
+           "gf_destroy").split()
+
+
+def _dims(dims):
+    return (C.c_int * 4)(*[int(d) for d in dims])
+
+
+def _rc(ctx, rc, check=True):
+    if rc < 0 and check:
+        raise GFError(rc, gf_last_error(ctx))
+    return rc
+
+
+def gf_storage_bytes(dims, precision, recon):
+    return lib.gf_storage_bytes(_dims(dims), precision, recon)
+
+
+def gf_workspace_bytes(dims):
+    return lib.gf_workspace_bytes(_dims(dims))
+
+
+def gf_init_lattice(dims, gauge, recon, dev_links_f64, dev_links_f32, dev_workspace, cuda_stream, seed,
+                    check=True):
+    """Returns the opaque context handle (an int), or the negative code if check=False."""
+    ctx = C.c_void_p()
+    rc = lib.gf_init_lattice(C.byref(ctx), _dims(dims), gauge, recon, dev_links_f64 or None,
+                             dev_links_f32 or None, dev_workspace or None, cuda_stream or None, int(seed))
+    if rc < 0:
+        if check:
+            raise GFError(rc, "gf_init_lattice failed")
+        return rc
+    return ctx.value
+
+
+def gf_destroy(ctx):
+    lib.gf_destroy(ctx)
+
+
+def gf_last_error(ctx):
+    s = lib.gf_last_error(ctx)
+    return s.decode() if s else ""
+
+
+def gf_pack(ctx, dev_canonical, canonical_is_f64, precision, check=True):
+    return _rc(ctx, lib.gf_pack(ctx, dev_canonical, int(canonical_is_f64), precision), check)
+
+
+def gf_unpack(ctx, dev_canonical, canonical_is_f64, precision, check=True):
+    return _rc(ctx, lib.gf_unpack(ctx, dev_canonical, int(canonical_is_f64), precision), check)
+
+
+def gf_load_host(ctx, host_canonical, canonical_is_f64, precision, dev_staging, check=True):
+    return _rc(ctx, lib.gf_load_host(ctx, host_canonical, int(canonical_is_f64), precision, dev_staging), check)
+
+
+def gf_store_host(ctx, host_canonical, canonical_is_f64, precision, dev_staging, check=True):
+    return _rc(ctx, lib.gf_store_host(ctx, host_canonical, int(canonical_is_f64), precision, dev_staging), check)
+
+
+def gf_sweep(ctx, parity, algo, omega, p, precision, check=True):
+    return _rc(ctx, lib.gf_sweep(ctx, parity, algo, omega, p, precision), check)
+
+
+def _nout(ctx_dims, gauge):
+    return ctx_dims[0] if gauge == GF_COULOMB else 1
+
+
+def gf_functional(ctx, precision, n_out=1, check=True):
+    """n_out: 1 (Landau) or Nt (Coulomb).  Returns a list of floats."""
+    out = (C.c_double * n_out)()
+    _rc(ctx, lib.gf_functional(ctx, precision, out), check)
+    return list(out)
+
+
+def gf_theta(ctx, precision, n_out=1, check=True):
+    out = (C.c_double * n_out)()
+    _rc(ctx, lib.gf_theta(ctx, precision, out), check)
+    return list(out)
+
+
+def gf_measure(ctx, precision, n_out=1, check=True):
+    """Returns (F list, theta list) from one pass over the field."""
+    f = (C.c_double * n_out)()
+    t = (C.c_double * n_out)()
+    _rc(ctx, lib.gf_measure(ctx, precision, f, t), check)
+    return list(f), list(t)
+
+
+def gf_fix_until(ctx, algo, omega, p, precision, theta_target, max_iter, check_every, check=True):
+    """Returns (return code, iterations, theta)."""
+    it = C.c_int(0)
+    th = C.c_double(0.0)
+    rc = _rc(ctx, lib.gf_fix_until(ctx, algo, omega, p, precision, theta_target, max_iter, check_every,
+                                   C.byref(it), C.byref(th)), check)
+    return rc, it.value, th.value
+
+
+def gf_set_rng(ctx, seed, half_sweep_counter, check=True):
+    return _rc(ctx, lib.gf_set_rng(ctx, int(seed), int(half_sweep_counter)), check)
+
+
+def gf_get_counter(ctx):
+    c = C.c_uint32(0)
+    _rc(ctx, lib.gf_get_counter(ctx, C.byref(c)))
+    return c.value
+
+
+def gf_reunitarize(ctx, precision, check=True):
+    return _rc(ctx, lib.gf_reunitarize(ctx, precision), check)
+
+
+def gf_cast(ctx, from_precision, to_precision, check=True):
+    return _rc(ctx, lib.gf_cast(ctx, from_precision, to_precision), check)
+
+
+def gf_plaquette(ctx, precision, check=True):
+    out = C.c_double(0.0)
+    _rc(ctx, lib.gf_plaquette(ctx, precision, C.byref(out)), check)
+    return out.value
+
+
+def gf_unitarity(ctx, precision, check=True):
+    out = (C.c_double * 2)()
+    _rc(ctx, lib.gf_unitarity(ctx, precision, out), check)
+    return out[0], out[1]
+
+
+def gf_set_tuning(ctx, precision, lanes_per_site, block_threads, check=True):
+    return _rc(ctx, lib.gf_set_tuning(ctx, precision, lanes_per_site, block_threads), check)
+
+
+def gf_set_solver_precision(ctx, solver_precision, check=True):
+    return _rc(ctx, lib.gf_set_solver_precision(ctx, solver_precision), check)
+
+
+def gf_debug_philox(ctx, n, dev_counters, dev_keys, dev_out, check=True):
+    return _rc(ctx, lib.gf_debug_philox(ctx, n, dev_counters, dev_keys, dev_out), check)
+
+
+def gf_launch_count(ctx):
+    c = C.c_uint64(0)
+    _rc(ctx, lib.gf_launch_count(ctx, C.byref(c)))
+    return c.value

@@ -1,0 +1,504 @@
+// gf_api.cu -- the C ABI of include/gf.h: argument checks, the context, the host-side fix loop
+// and the mixed-precision hand-off.  No arithmetic of the method runs on the
+// host: every step is one of the kernels in gf_sweep.cu / gf_aux.cu.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/gf.h"
+#include "gf_internal.h"
+
+using namespace gf;
+
+namespace {
+constexpr int kMeasureBlock = 128;
+constexpr int kMaxNt = 4096;
+}
+
+struct gf_ctx {
+    int dims[4];
+    int gauge, recon;
+    void* links[2];             // [PREC_F32], [PREC_F64]
+    double* workspace;
+    double* partials;           // workspace: per-block partial sums
+    double* slice_out;          // workspace: 2 doubles per time slice
+    double* host_pinned;        // 2 * Nt doubles
+    cudaStream_t stream;
+    uint64_t seed;
+    uint32_t counter;
+    Geom G;
+    MeasureGrid mg;
+    size_t V;
+    int lanes[2], block[2];
+    int solver_mode;            // fp32 storage: K and the SU(2) solves in GF_F32, GF_F64 or GF_SOLVER_AUTO
+    uint64_t launches;
+    char err[256];
+};
+
+static int fail(gf_ctx* ctx, int code, const char* fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+static int cuda_fail(gf_ctx* ctx, cudaError_t e, const char* what)
+{
+    return fail(ctx, GF_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+static bool dims_ok(const int dims[4])
+{
+    if (!dims) return false;
+    uint64_t V = 1;
+    for (int i = 0; i < 4; ++i) {
+        if (dims[i] < 2 || (dims[i] & 1)) return false;
+        V *= (uint64_t)dims[i];
+    }
+    return dims[0] <= kMaxNt && V < (uint64_t(1) << 32);
+}
+
+static MeasureGrid measure_grid(const int dims[4])
+{
+    MeasureGrid mg;
+    mg.Sh = (uint32_t)((uint64_t)dims[1] * dims[2] * dims[3] / 2);
+    mg.block = kMeasureBlock;
+    mg.bpp = (mg.Sh + mg.block - 1) / mg.block;
+    return mg;
+}
+
+extern "C" size_t gf_storage_bytes(const int dims[4], int precision, int recon)
+{
+    if (!dims_ok(dims) || (precision != GF_F32 && precision != GF_F64) || (recon != 18 && recon != 12)) return 0;
+    const size_t V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
+    return V * 4 * (size_t)recon * (precision == GF_F64 ? 8 : 4);
+}
+
+extern "C" size_t gf_workspace_bytes(const int dims[4])
+{
+    if (!dims_ok(dims)) return 0;
+    const MeasureGrid mg = measure_grid(dims);
+    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double);
+}
+
+extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
+                               void* dev_links_f32, void* dev_workspace, void* cuda_stream, uint64_t seed)
+{
+    if (!out) return GF_EINVAL;
+    *out = nullptr;
+    if (!dims_ok(dims)) return GF_EINVAL;
+    if (gauge != GF_LANDAU && gauge != GF_COULOMB) return GF_EINVAL;
+    if (recon != GF_RECON18 && recon != GF_RECON12) return GF_EINVAL;
+    if (!dev_links_f64 && !dev_links_f32) return GF_EINVAL;
+    if (!dev_workspace) return GF_EINVAL;
+    if (((uintptr_t)dev_links_f64 | (uintptr_t)dev_links_f32 | (uintptr_t)dev_workspace) & 15u) return GF_EINVAL;
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return GF_ECUDA;
+    if (prop.major != 10) return GF_ECUDA;              // built for sm_100a only; no fallback
+
+    gf_ctx* c = new (std::nothrow) gf_ctx;
+    if (!c) return GF_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    memcpy(c->dims, dims, sizeof(c->dims));
+    c->gauge = gauge;
+    c->recon = recon;
+    c->links[PREC_F32] = dev_links_f32;
+    c->links[PREC_F64] = dev_links_f64;
+    c->workspace = static_cast<double*>(dev_workspace);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->seed = seed;
+    c->counter = 0;
+    c->V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
+    c->mg = measure_grid(dims);
+    c->partials = c->workspace;
+    c->slice_out = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
+
+    Geom& G = c->G;
+    G.nt = dims[0];
+    G.nxh = dims[1] / 2;
+    G.ny = dims[2];
+    G.nz = dims[3];
+    G.Vh = (uint32_t)(c->V / 2);
+    G.extent[0] = dims[0]; G.extent[1] = dims[1]; G.extent[2] = dims[2]; G.extent[3] = dims[3];
+    G.stride[1] = 1;
+    G.stride[2] = G.nxh;
+    G.stride[3] = G.nxh * G.ny;
+    G.stride[0] = G.nxh * G.ny * G.nz;
+    G.div_nxh = make_fastdiv(G.nxh);
+    G.div_ny = make_fastdiv(G.ny);
+    G.div_nz = make_fastdiv(G.nz);
+
+    // defaults chosen by measurement on B200 at 32^4 ("Kernels"); gf_set_tuning overrides
+    c->lanes[PREC_F32] = 2;  c->block[PREC_F32] = 128;
+    c->lanes[PREC_F64] = 2;  c->block[PREC_F64] = 128;
+    c->solver_mode = GF_SOLVER_AUTO;
+
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return GF_ENOMEM;
+    }
+    *out = c;
+    return GF_OK;
+}
+
+extern "C" void gf_destroy(gf_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
+    delete ctx;
+}
+
+extern "C" const char* gf_last_error(const gf_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+static int check_prec(gf_ctx* ctx, int precision)
+{
+    if (!ctx) return GF_EINVAL;
+    if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
+    if (!ctx->links[precision]) return fail(ctx, GF_ESTATE, "no link storage for precision %d", precision);
+    return GF_OK;
+}
+
+extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    cudaError_t e = launch_pack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_pack");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    cudaError_t e = launch_unpack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_unpack");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+static size_t canonical_bytes(const gf_ctx* ctx, int is_f64) { return ctx->V * 4 * 18 * (is_f64 ? 8 : 4); }
+
+extern "C" int gf_load_host(gf_ctx* ctx, const void* host_canonical, int canonical_is_f64, int precision, void* dev_staging)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (!host_canonical || !dev_staging) return fail(ctx, GF_EINVAL, "null host or staging pointer");
+    cudaError_t e = cudaMemcpyAsync(dev_staging, host_canonical, canonical_bytes(ctx, canonical_is_f64), cudaMemcpyHostToDevice, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_load_host copy");
+    return gf_pack(ctx, dev_staging, canonical_is_f64, precision);
+}
+
+extern "C" int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is_f64, int precision, void* dev_staging)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (!host_canonical || !dev_staging) return fail(ctx, GF_EINVAL, "null host or staging pointer");
+    rc = gf_unpack(ctx, dev_staging, canonical_is_f64, precision);
+    if (rc) return rc;
+    cudaError_t e = cudaMemcpyAsync(host_canonical, dev_staging, canonical_bytes(ctx, canonical_is_f64), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_store_host copy");
+    return GF_OK;
+}
+
+static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
+{
+    if (algo != GF_RELAX && algo != GF_OVERRELAX && algo != GF_STOCHASTIC) return fail(ctx, GF_EINVAL, "unknown algo %d", algo);
+    if (algo == GF_OVERRELAX && !(omega >= 1.0 && omega < 2.0)) return fail(ctx, GF_EINVAL, "omega must be in [1,2)");
+    if (algo == GF_STOCHASTIC && !(p >= 0.0 && p <= 1.0)) return fail(ctx, GF_EINVAL, "p must be in [0,1]");
+    return GF_OK;
+}
+
+static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
+{
+    SweepArgs a;
+    a.links = ctx->links[precision];
+    a.G = ctx->G;
+    a.parity = (uint32_t)parity;
+    a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
+    a.algo = algo;
+    a.omega = omega;
+    a.p = p;
+    a.key0 = (uint32_t)ctx->seed;
+    a.key1 = (uint32_t)(ctx->seed >> 32);
+    a.counter = ctx->counter;
+    const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
+    cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, ctx->lanes[precision], ctx->block[precision], a, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_sweep launch");
+    ctx->counter += 1;
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (parity != 0 && parity != 1) return fail(ctx, GF_EINVAL, "parity must be 0 or 1");
+    rc = check_algo(ctx, algo, omega, p);
+    if (rc) return rc;
+    return enqueue_sweep(ctx, parity, algo, omega, p, precision);
+}
+
+// Runs the measurement kernels and leaves per-slice sums (F, theta) in ctx->host_pinned.
+static int measure_to_host(gf_ctx* ctx, int precision)
+{
+    const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
+    cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->G, mu0, ctx->mg, ctx->partials,
+                                   ctx->slice_out, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
+    ctx->launches += 2;
+    e = cudaMemcpyAsync(ctx->host_pinned, ctx->slice_out, sizeof(double) * 2 * ctx->dims[0], cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "measure copy");
+    return GF_OK;
+}
+
+// Normalises the slice sums: Landau 1/(Nc Nd V) and 1/(Nc V); Coulomb per slice
+// 1/(Nc 3 Ns^3) and 1/(Nc Ns^3).  Returns max_t theta_t (Landau: theta).
+static double finish_measure(const gf_ctx* ctx, double* host_F, double* host_theta)
+{
+    const int nt = ctx->dims[0];
+    const double* s = ctx->host_pinned;
+    if (ctx->gauge == GF_COULOMB) {
+        const double Vs = (double)(ctx->V / nt);
+        double worst = 0.0;
+        for (int t = 0; t < nt; ++t) {
+            const double F = s[2 * t] / (3.0 * 3.0 * Vs), th = s[2 * t + 1] / (3.0 * Vs);
+            if (host_F) host_F[t] = F;
+            if (host_theta) host_theta[t] = th;
+            if (th > worst || t == 0) worst = th;
+        }
+        return worst;
+    }
+    double F = 0.0, th = 0.0;
+    for (int t = 0; t < nt; ++t) {
+        F += s[2 * t];
+        th += s[2 * t + 1];
+    }
+    F /= 3.0 * 4.0 * (double)ctx->V;
+    th /= 3.0 * (double)ctx->V;
+    if (host_F) host_F[0] = F;
+    if (host_theta) host_theta[0] = th;
+    return th;
+}
+
+extern "C" int gf_measure(gf_ctx* ctx, int precision, double* host_functional, double* host_theta)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    rc = measure_to_host(ctx, precision);
+    if (rc) return rc;
+    finish_measure(ctx, host_functional, host_theta);
+    return GF_OK;
+}
+
+extern "C" int gf_functional(gf_ctx* ctx, int precision, double* host_out)
+{
+    if (ctx && !host_out) return fail(ctx, GF_EINVAL, "null output");
+    return gf_measure(ctx, precision, host_out, nullptr);
+}
+
+extern "C" int gf_theta(gf_ctx* ctx, int precision, double* host_out)
+{
+    if (ctx && !host_out) return fail(ctx, GF_EINVAL, "null output");
+    return gf_measure(ctx, precision, nullptr, host_out);
+}
+
+// One phase of the fix loop in one precision.  Returns GF_OK when theta < target was seen.
+static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
+                     int check_every, int* it_io, double* theta_out)
+{
+    int it = *it_io;
+    int rc = GF_NOT_CONVERGED;
+    while (it < max_iter) {
+        int n = check_every - (it % check_every);
+        if (n > max_iter - it) n = max_iter - it;
+        for (int k = 0; k < n; ++k) {
+            int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
+            if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
+            if (e != GF_OK) { *it_io = it; return e; }
+        }
+        it += n;
+        int e = measure_to_host(ctx, precision);
+        if (e != GF_OK) { *it_io = it; return e; }
+        *theta_out = finish_measure(ctx, nullptr, nullptr);
+        if (*theta_out < target) { rc = GF_OK; break; }
+    }
+    *it_io = it;
+    return rc;
+}
+
+extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int precision, double theta_target,
+                            int max_iter, int check_every, int* iters_out, double* theta_out)
+{
+    if (!ctx) return GF_EINVAL;
+    if (precision != GF_F32 && precision != GF_F64 && precision != GF_MIXED) return fail(ctx, GF_EINVAL, "bad precision");
+    if (precision == GF_MIXED && (!ctx->links[PREC_F32] || !ctx->links[PREC_F64]))
+        return fail(ctx, GF_ESTATE, "GF_MIXED needs both fp32 and fp64 storage");
+    if (precision != GF_MIXED && !ctx->links[precision]) return fail(ctx, GF_ESTATE, "no link storage for precision %d", precision);
+    int rc = check_algo(ctx, algo, omega, p);
+    if (rc) return rc;
+    if (max_iter < 0 || check_every < 1 || !(theta_target >= 0.0)) return fail(ctx, GF_EINVAL, "bad max_iter / check_every / theta_target");
+
+    int it = 0;
+    double theta = -1.0;
+    if (precision == GF_MIXED) {
+        const double t32 = theta_target > 1e-6 ? theta_target : 1e-6;
+        rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta);
+        if (rc < 0) return rc;
+        int e = gf_cast(ctx, GF_F32, GF_F64);
+        if (e != GF_OK) return e;
+        if (rc == GF_OK && !(theta < theta_target)) rc = fix_phase(ctx, algo, omega, p, GF_F64, theta_target, max_iter, check_every, &it, &theta);
+        else if (rc == GF_NOT_CONVERGED) {
+            e = measure_to_host(ctx, GF_F64);
+            if (e != GF_OK) return e;
+            theta = finish_measure(ctx, nullptr, nullptr);
+        }
+    } else {
+        if (max_iter == 0) {
+            rc = measure_to_host(ctx, precision);
+            if (rc) return rc;
+            theta = finish_measure(ctx, nullptr, nullptr);
+            rc = theta < theta_target ? GF_OK : GF_NOT_CONVERGED;
+        } else {
+            rc = fix_phase(ctx, algo, omega, p, precision, theta_target, max_iter, check_every, &it, &theta);
+        }
+    }
+    if (rc < 0) return rc;
+    if (iters_out) *iters_out = it;
+    if (theta_out) *theta_out = theta;
+    return rc;
+}
+
+extern "C" int gf_set_rng(gf_ctx* ctx, uint64_t seed, uint32_t half_sweep_counter)
+{
+    if (!ctx) return GF_EINVAL;
+    ctx->seed = seed;
+    ctx->counter = half_sweep_counter;
+    return GF_OK;
+}
+
+extern "C" int gf_get_counter(const gf_ctx* ctx, uint32_t* half_sweep_counter_out)
+{
+    if (!ctx || !half_sweep_counter_out) return GF_EINVAL;
+    *half_sweep_counter_out = ctx->counter;
+    return GF_OK;
+}
+
+extern "C" int gf_reunitarize(gf_ctx* ctx, int precision)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    cudaError_t e = launch_cast(precision, precision, ctx->recon, ctx->links[precision], ctx->links[precision], ctx->G, 1, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_reunitarize");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_cast(gf_ctx* ctx, int from_precision, int to_precision)
+{
+    int rc = check_prec(ctx, from_precision);
+    if (rc) return rc;
+    rc = check_prec(ctx, to_precision);
+    if (rc) return rc;
+    if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_cast needs two different precisions");
+    const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
+    cudaError_t e = launch_cast(from_precision, to_precision, ctx->recon, ctx->links[from_precision], ctx->links[to_precision],
+                                ctx->G, reproject, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_cast");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+static int slices_to_host(gf_ctx* ctx, const char* what)
+{
+    ctx->launches += 2;
+    cudaError_t e = cudaMemcpyAsync(ctx->host_pinned, ctx->slice_out, sizeof(double) * 2 * ctx->dims[0], cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, what);
+    return GF_OK;
+}
+
+extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (!host_out) return fail(ctx, GF_EINVAL, "null output");
+    cudaError_t e = launch_plaquette(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_plaquette launch");
+    rc = slices_to_host(ctx, "gf_plaquette copy");
+    if (rc) return rc;
+    double sum = 0.0;
+    for (int t = 0; t < ctx->dims[0]; ++t) sum += ctx->host_pinned[2 * t];
+    *host_out = sum / (6.0 * 3.0 * (double)ctx->V);
+    return GF_OK;
+}
+
+extern "C" int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (!host_out2) return fail(ctx, GF_EINVAL, "null output");
+    cudaError_t e = launch_unitarity(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_unitarity launch");
+    rc = slices_to_host(ctx, "gf_unitarity copy");
+    if (rc) return rc;
+    host_out2[0] = host_out2[1] = 0.0;
+    for (int t = 0; t < ctx->dims[0]; ++t) {
+        if (ctx->host_pinned[2 * t] > host_out2[0]) host_out2[0] = ctx->host_pinned[2 * t];
+        if (ctx->host_pinned[2 * t + 1] > host_out2[1]) host_out2[1] = ctx->host_pinned[2 * t + 1];
+    }
+    return GF_OK;
+}
+
+extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_threads)
+{
+    if (!ctx) return GF_EINVAL;
+    if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
+    const int lanes = lanes_per_site ? lanes_per_site : ctx->lanes[precision];
+    const int block = block_threads ? block_threads : ctx->block[precision];
+    if (!sweep_config_valid(lanes, block)) return fail(ctx, GF_EINVAL, "lanes must be 1,2,4 and block 64..512 (power of two)");
+    ctx->lanes[precision] = lanes;
+    ctx->block[precision] = block;
+    return GF_OK;
+}
+
+extern "C" int gf_set_solver_precision(gf_ctx* ctx, int solver_precision)
+{
+    if (!ctx) return GF_EINVAL;
+    if (solver_precision != GF_F32 && solver_precision != GF_F64 && solver_precision != GF_SOLVER_AUTO)
+        return fail(ctx, GF_EINVAL, "solver precision must be GF_F32, GF_F64 or GF_SOLVER_AUTO");
+    ctx->solver_mode = solver_precision;
+    return GF_OK;
+}
+
+extern "C" int gf_debug_philox(gf_ctx* ctx, int n, const uint32_t* dev_counters, const uint32_t* dev_keys, uint32_t* dev_out)
+{
+    if (!ctx) return GF_EINVAL;
+    if (n < 0 || !dev_counters || !dev_keys || !dev_out) return fail(ctx, GF_EINVAL, "bad arguments");
+    if (n == 0) return GF_OK;
+    cudaError_t e = launch_philox(n, dev_counters, dev_keys, dev_out, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_debug_philox");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_launch_count(const gf_ctx* ctx, uint64_t* count_out)
+{
+    if (!ctx || !count_out) return GF_EINVAL;
+    *count_out = ctx->launches;
+    return GF_OK;
+}

@@ -1,0 +1,447 @@
+// gf_aux.cu -- everything around the sweep: the F / theta reduction,
+// diagnostics (plaquette, unitarity), layout conversion (pack / unpack / cast) and the Philox
+// known-answer kernel.  All of it is HBM bound and off the inner loop; the reductions use a
+// fixed order (warp shuffle -> shared memory -> per-block partials -> one block per time slice),
+// no floating-point atomics.
+#include "gf_internal.h"
+
+namespace gf {
+
+// ------------------------------------------------------------------------------ reductions
+struct OpSum {
+    __device__ static double apply(double a, double b) { return a + b; }
+};
+struct OpMax {   // of non-negative values, so 0 is neutral for both
+    __device__ static double apply(double a, double b) { return fmax(a, b); }
+};
+
+template <typename Op>
+__device__ __forceinline__ double warp_reduce(double v)
+{
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v = Op::apply(v, __shfl_xor_sync(0xffffffffu, v, off));
+    return v;
+}
+
+// Reduces two values per thread over the block; thread 0 writes them to out[0], out[1].
+template <typename Op>
+__device__ __forceinline__ void block_reduce2(double a, double b, double* out)
+{
+    __shared__ double sh[2][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    a = warp_reduce<Op>(a);
+    b = warp_reduce<Op>(b);
+    if (lane == 0) {
+        sh[0][w] = a;
+        sh[1][w] = b;
+    }
+    __syncthreads();
+    if (w == 0) {
+        a = lane < nw ? sh[0][lane] : 0.0;
+        b = lane < nw ? sh[1][lane] : 0.0;
+        a = warp_reduce<Op>(a);
+        b = warp_reduce<Op>(b);
+        if (lane == 0) {
+            out[0] = a;
+            out[1] = b;
+        }
+    }
+}
+
+// One block per time slice: combines that slice's per-block partials in a fixed order.
+template <typename Op>
+__global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32_t per_slice, double* __restrict__ out)
+{
+    const double* p = partials + (size_t)blockIdx.x * per_slice * 2;
+    double a = 0.0, b = 0.0;
+    for (uint32_t i = threadIdx.x; i < per_slice; i += blockDim.x) {
+        a = Op::apply(a, p[2 * i]);
+        b = Op::apply(b, p[2 * i + 1]);
+    }
+    block_reduce2<Op>(a, b, out + 2 * blockIdx.x);
+}
+
+// thread -> (slice t, parity, site) of the measurement grids: blockIdx.y = t, blockIdx.x = 2*chunk + parity
+__device__ __forceinline__ bool measure_site(const Geom& G, const MeasureGrid& mg, uint32_t& parity, Site& s)
+{
+    parity = blockIdx.x & 1u;
+    const uint32_t i = (blockIdx.x >> 1) * blockDim.x + threadIdx.x;
+    const bool live = i < mg.Sh;
+    const uint32_t h = blockIdx.y * mg.Sh + (live ? i : mg.Sh - 1u);
+    s = decode_site(G, h, parity);
+    return live;
+}
+
+__device__ __forceinline__ size_t partial_slot(const MeasureGrid& mg)
+{
+    return ((size_t)blockIdx.y * (2u * mg.bpp) + blockIdx.x) * 2;
+}
+
+// a7 + a8: per-block partial sums of  sum_mu Re tr U_mu(x)  and  tr[Delta(x) Delta(x)^dagger].
+// Delta(x) = sum_mu (A_mu(x) - A_mu(x-mu)) with A the traceless anti-Hermitian part of U
+// (eq. 4); as A is linear in U, Delta = traceless[(M - M^dagger)/(2i)] with
+// M = sum_mu (U_mu(x) - U_mu(x-mu)).  Accumulation in fp64 whatever the storage precision.
+template <typename T, int RECON>
+__global__ void measure_kernel(const T* __restrict__ links, const Geom G, const int mu0, const MeasureGrid mg,
+                               double* __restrict__ partials)
+{
+    uint32_t parity;
+    Site s;
+    const bool live = measure_site(G, mg, parity, s);
+    double M[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) M[k] = 0.0;
+    double F = 0.0;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        if (mu < mu0) continue;
+        T Uf[18], Ub[18];
+        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, s.h, Uf);
+        load_link<RECON>(links + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, backward_index(G, s, mu), Ub);
+        if (RECON == 12) {
+            reconstruct_row2(Uf);
+            reconstruct_row2(Ub);
+        }
+        F += (double)Uf[0] + (double)Uf[8] + (double)Uf[16];
+#pragma unroll
+        for (int k = 0; k < 18; ++k) M[k] += (double)Uf[k] - (double)Ub[k];
+    }
+    // diagonal of (M - M^dagger)/(2i) is Im M_aa; off-diagonal |.|^2 = |M_ab - conj(M_ba)|^2 / 4
+    const double tr3 = (GF_IM(M, 0, 0) + GF_IM(M, 1, 1) + GF_IM(M, 2, 2)) * (1.0 / 3.0);
+    double th = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double d = GF_IM(M, a, a) - tr3;
+        th += d * d;
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = a + 1; b < 3; ++b) {
+            const double dr = GF_RE(M, a, b) - GF_RE(M, b, a), di = GF_IM(M, a, b) + GF_IM(M, b, a);
+            th += 0.5 * (dr * dr + di * di);
+        }
+    if (!live) {
+        F = 0.0;
+        th = 0.0;
+    }
+    block_reduce2<OpSum>(F, th, partials + partial_slot(mg));
+}
+
+template <typename T, int RECON>
+__device__ __forceinline__ void load_full_d(const T* links, const Geom& G, uint32_t parity, int mu, uint32_t h, double (&m)[18])
+{
+    T u[18];
+    load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, u);
+    if (RECON == 12) reconstruct_row2(u);
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m[k] = (double)u[k];
+}
+
+__device__ __forceinline__ void mul_full(const double (&A)[18], const double (&B)[18], double (&C)[18], bool dagger_b)
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            double re = 0.0, im = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double br = dagger_b ? GF_RE(B, b, k) : GF_RE(B, k, b);
+                const double bi = dagger_b ? -GF_IM(B, b, k) : GF_IM(B, k, b);
+                re += GF_RE(A, a, k) * br - GF_IM(A, a, k) * bi;
+                im += GF_RE(A, a, k) * bi + GF_IM(A, a, k) * br;
+            }
+            GF_RE(C, a, b) = re;
+            GF_IM(C, a, b) = im;
+        }
+}
+
+// sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu) U_mu(x+nu)^dagger U_nu(x)^dagger]   (diagnostic)
+template <typename T, int RECON>
+__global__ void plaquette_kernel(const T* __restrict__ links, const Geom G, const MeasureGrid mg,
+                                 double* __restrict__ partials)
+{
+    uint32_t parity;
+    Site s;
+    const bool live = measure_site(G, mg, parity, s);
+    double sum = 0.0;
+    for (int mu = 0; mu < 4; ++mu)
+        for (int nu = mu + 1; nu < 4; ++nu) {
+            double A[18], B[18], C[18], D[18];
+            load_full_d<T, RECON>(links, G, parity, mu, s.h, A);
+            load_full_d<T, RECON>(links, G, parity ^ 1u, nu, forward_index(G, s, mu), B);
+            mul_full(A, B, C, false);
+            load_full_d<T, RECON>(links, G, parity ^ 1u, mu, forward_index(G, s, nu), A);
+            mul_full(C, A, D, true);
+            load_full_d<T, RECON>(links, G, parity, nu, s.h, B);
+            // Re tr[D B^dagger] = sum_ab Re(D_ab conj(B_ab))
+#pragma unroll
+            for (int k = 0; k < 18; ++k) sum += D[k] * B[k];
+        }
+    if (!live) sum = 0.0;
+    block_reduce2<OpSum>(sum, 0.0, partials + partial_slot(mg));
+}
+
+// max |U U^dagger - 1| entry and max |det U - 1| over the four links stored at each site
+template <typename T, int RECON>
+__global__ void unitarity_kernel(const T* __restrict__ links, const Geom G, const MeasureGrid mg,
+                                 double* __restrict__ partials)
+{
+    uint32_t parity;
+    Site s;
+    measure_site(G, mg, parity, s);    // a clamped duplicate site does not change a maximum
+    double dmax = 0.0, detmax = 0.0;
+    for (int mu = 0; mu < 4; ++mu) {
+        double U[18], P[18];
+        load_full_d<T, RECON>(links, G, parity, mu, s.h, U);
+        mul_full(U, U, P, true);
+        P[0] -= 1.0;
+        P[8] -= 1.0;
+        P[16] -= 1.0;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) dmax = fmax(dmax, sqrt(P[2 * k] * P[2 * k] + P[2 * k + 1] * P[2 * k + 1]));
+        // det U = row0 . (row1 x row2)
+        double dr = 0.0, di = 0.0;
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const int b1 = (b + 1) % 3, b2 = (b + 2) % 3;
+            const double cr = GF_RE(U, 1, b1) * GF_RE(U, 2, b2) - GF_IM(U, 1, b1) * GF_IM(U, 2, b2)
+                            - GF_RE(U, 1, b2) * GF_RE(U, 2, b1) + GF_IM(U, 1, b2) * GF_IM(U, 2, b1);
+            const double ci = GF_RE(U, 1, b1) * GF_IM(U, 2, b2) + GF_IM(U, 1, b1) * GF_RE(U, 2, b2)
+                            - GF_RE(U, 1, b2) * GF_IM(U, 2, b1) - GF_IM(U, 1, b2) * GF_RE(U, 2, b1);
+            dr += GF_RE(U, 0, b) * cr - GF_IM(U, 0, b) * ci;
+            di += GF_RE(U, 0, b) * ci + GF_IM(U, 0, b) * cr;
+        }
+        detmax = fmax(detmax, sqrt((dr - 1.0) * (dr - 1.0) + di * di));
+    }
+    block_reduce2<OpMax>(dmax, detmax, partials + partial_slot(mg));
+}
+
+template <template <typename, int> class Launcher, typename... Args>
+static cudaError_t dispatch(int precision, int recon, Args... args)
+{
+    if (precision == PREC_F64)
+        return recon == 12 ? Launcher<double, 12>::run(args...) : Launcher<double, 18>::run(args...);
+    return recon == 12 ? Launcher<float, 12>::run(args...) : Launcher<float, 18>::run(args...);
+}
+
+static dim3 measure_dims(const Geom& G, const MeasureGrid& mg) { return dim3(2u * mg.bpp, G.nt, 1); }
+
+template <typename T, int RECON> struct MeasureLauncher {
+    static cudaError_t run(const void* links, const Geom& G, int mu0, const MeasureGrid& mg, double* partials,
+                           double* slice_out, cudaStream_t st)
+    {
+        measure_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mu0, mg, partials);
+        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
+        return cudaGetLastError();
+    }
+};
+
+template <typename T, int RECON> struct PlaquetteLauncher {
+    static cudaError_t run(const void* links, const Geom& G, const MeasureGrid& mg, double* partials,
+                           double* slice_out, cudaStream_t st)
+    {
+        plaquette_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mg, partials);
+        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
+        return cudaGetLastError();
+    }
+};
+
+template <typename T, int RECON> struct UnitarityLauncher {
+    static cudaError_t run(const void* links, const Geom& G, const MeasureGrid& mg, double* partials,
+                           double* slice_out, cudaStream_t st)
+    {
+        unitarity_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mg, partials);
+        reduce_slices_kernel<OpMax><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
+        return cudaGetLastError();
+    }
+};
+
+cudaError_t launch_measure(int precision, int recon, const void* links, const Geom& G, int mu0,
+                           const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
+{
+    return dispatch<MeasureLauncher>(precision, recon, links, G, mu0, mg, partials, slice_out, st);
+}
+
+cudaError_t launch_plaquette(int precision, int recon, const void* links, const Geom& G,
+                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
+{
+    return dispatch<PlaquetteLauncher>(precision, recon, links, G, mg, partials, slice_out, st);
+}
+
+cudaError_t launch_unitarity(int precision, int recon, const void* links, const Geom& G,
+                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
+{
+    return dispatch<UnitarityLauncher>(precision, recon, links, G, mg, partials, slice_out, st);
+}
+
+// ---------------------------------------------------------------------- pack / unpack / cast
+// a11: canonical AoS (site s, mu, 3x3 row-major complex) <-> the private chunked layout.
+template <typename T, int RECON, typename TC>
+__global__ void pack_kernel(T* __restrict__ links, const Geom G, const TC* __restrict__ canonical)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    const Site s = decode_site(G, h, parity);
+    const size_t site = 2u * (size_t)h + s.xodd;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const TC* src = canonical + (site * 4 + mu) * 18;
+        T m[18];
+#pragma unroll
+        for (int k = 0; k < 18; ++k) m[k] = (T)src[k];
+        store_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, m);
+    }
+}
+
+template <typename T, int RECON, typename TC>
+__global__ void unpack_kernel(const T* __restrict__ links, const Geom G, TC* __restrict__ canonical)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    const Site s = decode_site(G, h, parity);
+    const size_t site = 2u * (size_t)h + s.xodd;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        T m[18];
+        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, m);
+        if (RECON == 12) reconstruct_row2(m);
+        TC* dst = canonical + (site * 4 + mu) * 18;
+#pragma unroll
+        for (int k = 0; k < 18; ++k) dst[k] = (TC)m[k];
+    }
+}
+
+// Gram-Schmidt on rows 0 and 1, row 2 = conj(row 0 x row 1)
+__device__ __forceinline__ void project_su3(double (&m)[18])
+{
+    double n0 = 0.0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) n0 += m[k] * m[k];
+    n0 = 1.0 / sqrt(n0);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) m[k] *= n0;
+    double pr = 0.0, pi = 0.0;                       // conj(row0) . row1
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        pr += GF_RE(m, 0, b) * GF_RE(m, 1, b) + GF_IM(m, 0, b) * GF_IM(m, 1, b);
+        pi += GF_RE(m, 0, b) * GF_IM(m, 1, b) - GF_IM(m, 0, b) * GF_RE(m, 1, b);
+    }
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        GF_RE(m, 1, b) -= pr * GF_RE(m, 0, b) - pi * GF_IM(m, 0, b);
+        GF_IM(m, 1, b) -= pr * GF_IM(m, 0, b) + pi * GF_RE(m, 0, b);
+    }
+    double n1 = 0.0;
+#pragma unroll
+    for (int k = 6; k < 12; ++k) n1 += m[k] * m[k];
+    n1 = 1.0 / sqrt(n1);
+#pragma unroll
+    for (int k = 6; k < 12; ++k) m[k] *= n1;
+    reconstruct_row2(m);
+}
+
+// every (parity, mu, h) link: load as TS, optionally re-project in fp64, store as TD
+template <typename TS, typename TD, int RECON>
+__global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int reproject)   // src may alias dst
+{
+    const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= G.Vh) return;
+    const uint32_t pm = blockIdx.y;                  // parity*4 + mu
+    TS u[18];
+    load_link<RECON>(src + (size_t)pm * RECON * G.Vh, G.Vh, h, u);
+    double m[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m[k] = (double)u[k];
+    if (reproject) project_su3(m);
+    TD o[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) o[k] = (TD)m[k];
+    store_link<RECON>(dst + (size_t)pm * RECON * G.Vh, G.Vh, h, o);
+}
+
+template <typename T, int RECON>
+static cudaError_t pack_run(void* links, const Geom& G, const void* canonical, int canonical_is_f64, cudaStream_t st)
+{
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    if (canonical_is_f64)
+        pack_kernel<T, RECON, double><<<grid, block, 0, st>>>(static_cast<T*>(links), G, static_cast<const double*>(canonical));
+    else
+        pack_kernel<T, RECON, float><<<grid, block, 0, st>>>(static_cast<T*>(links), G, static_cast<const float*>(canonical));
+    return cudaGetLastError();
+}
+
+template <typename T, int RECON>
+static cudaError_t unpack_run(const void* links, const Geom& G, void* canonical, int canonical_is_f64, cudaStream_t st)
+{
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    if (canonical_is_f64)
+        unpack_kernel<T, RECON, double><<<grid, block, 0, st>>>(static_cast<const T*>(links), G, static_cast<double*>(canonical));
+    else
+        unpack_kernel<T, RECON, float><<<grid, block, 0, st>>>(static_cast<const T*>(links), G, static_cast<float*>(canonical));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack(int precision, int recon, void* links, const Geom& G, const void* canonical,
+                        int canonical_is_f64, cudaStream_t st)
+{
+    if (precision == PREC_F64)
+        return recon == 12 ? pack_run<double, 12>(links, G, canonical, canonical_is_f64, st)
+                           : pack_run<double, 18>(links, G, canonical, canonical_is_f64, st);
+    return recon == 12 ? pack_run<float, 12>(links, G, canonical, canonical_is_f64, st)
+                       : pack_run<float, 18>(links, G, canonical, canonical_is_f64, st);
+}
+
+cudaError_t launch_unpack(int precision, int recon, const void* links, const Geom& G, void* canonical,
+                          int canonical_is_f64, cudaStream_t st)
+{
+    if (precision == PREC_F64)
+        return recon == 12 ? unpack_run<double, 12>(links, G, canonical, canonical_is_f64, st)
+                           : unpack_run<double, 18>(links, G, canonical, canonical_is_f64, st);
+    return recon == 12 ? unpack_run<float, 12>(links, G, canonical, canonical_is_f64, st)
+                       : unpack_run<float, 18>(links, G, canonical, canonical_is_f64, st);
+}
+
+template <typename TS, typename TD>
+static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G, int reproject, cudaStream_t st)
+{
+    const uint32_t block = 128;
+    const dim3 grid((G.Vh + block - 1) / block, 8, 1);
+    if (recon == 12)
+        cast_kernel<TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
+    else
+        cast_kernel<TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cast(int from_precision, int to_precision, int recon, const void* src, void* dst,
+                        const Geom& G, int reproject, cudaStream_t st)
+{
+    if (from_precision == PREC_F32 && to_precision == PREC_F64) return cast_run<float, double>(recon, src, dst, G, reproject, st);
+    if (from_precision == PREC_F64 && to_precision == PREC_F32) return cast_run<double, float>(recon, src, dst, G, reproject, st);
+    if (from_precision == PREC_F64) return cast_run<double, double>(recon, src, dst, G, reproject, st);
+    return cast_run<float, float>(recon, src, dst, G, reproject, st);
+}
+
+// ------------------------------------------------------------------------------- Philox KAT
+__global__ void philox_kernel(int n, const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key,
+                              uint32_t* __restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t w[4];
+    philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1], w);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) out[4 * i + k] = w[k];
+}
+
+cudaError_t launch_philox(int n, const uint32_t* ctr, const uint32_t* key, uint32_t* out, cudaStream_t st)
+{
+    philox_kernel<<<(n + 127) / 128, 128, 0, st>>>(n, ctr, key, out);
+    return cudaGetLastError();
+}
+
+}  // namespace gf

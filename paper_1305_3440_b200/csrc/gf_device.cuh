@@ -1,0 +1,304 @@
+// gf_device.cuh -- device-side building blocks of libgf_b200: lattice geometry, the private
+// link layout, 3x3 complex algebra in registers, the SU(2) subgroup step and Philox4x32-10.
+// Written for sm_100a only.  Citations "PAPER.md:<line>" refer to arXiv:1305.3440.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gf {
+
+// ------------------------------------------------------------------------------ fast division
+// Unsigned division by a run-time constant (Granlund-Montgomery): q = (t + ((n - t) >> s1)) >> s2
+// with t = mulhi(n, m).  Exact for every 32-bit n.
+struct FastDiv {
+    uint32_t d, m, s1, s2;
+};
+
+inline FastDiv make_fastdiv(uint32_t d)
+{
+    FastDiv f;
+    f.d = d;
+    uint32_t l = 0;
+    while ((uint64_t(1) << l) < d) ++l;
+    f.m = uint32_t(((uint64_t(1) << 32) * ((uint64_t(1) << l) - d)) / d + 1);
+    f.s1 = l < 1 ? l : 1;
+    f.s2 = l > 0 ? l - 1 : 0;
+    return f;
+}
+
+__device__ __forceinline__ uint32_t fdiv(uint32_t n, const FastDiv& f)
+{
+    const uint32_t t = __umulhi(n, f.m);
+    return (t + ((n - t) >> f.s1)) >> f.s2;
+}
+
+// ---------------------------------------------------------------------------------- geometry
+// Sites of one parity are numbered by the half-index h = s >> 1, s = x + Nx (y + Ny (z + Nz t)),
+// so h = xh + nxh (y + Ny (z + Nz t)) with xh = x >> 1, nxh = Nx/2, and
+// x = 2 xh + ((y + z + t + parity) & 1).  Time slices are contiguous in h.
+struct Geom {
+    uint32_t nxh, ny, nz, nt;   // Nx/2, Ny, Nz, Nt
+    uint32_t Vh;                // sites per parity
+    uint32_t stride[4];         // distance in h of one step in mu (mu=1: unused)
+    uint32_t extent[4];         // N_mu
+    FastDiv div_nxh, div_ny, div_nz;
+};
+
+struct Site {
+    uint32_t h, xh, c[4];       // c[mu]: c[0]=t, c[1]=x, c[2]=y, c[3]=z
+    uint32_t xodd;              // x & 1
+};
+
+__device__ __forceinline__ Site decode_site(const Geom& G, uint32_t h, uint32_t parity)
+{
+    Site s;
+    s.h = h;
+    const uint32_t r0 = fdiv(h, G.div_nxh);
+    s.xh = h - r0 * G.nxh;
+    const uint32_t r1 = fdiv(r0, G.div_ny);
+    s.c[2] = r0 - r1 * G.ny;
+    s.c[0] = fdiv(r1, G.div_nz);
+    s.c[3] = r1 - s.c[0] * G.nz;
+    s.xodd = (s.c[2] + s.c[3] + s.c[0] + parity) & 1u;
+    s.c[1] = 2u * s.xh + s.xodd;
+    return s;
+}
+
+// c[mu] for a run-time mu without indexing the register array dynamically
+__device__ __forceinline__ uint32_t coord(const Site& s, int mu)
+{
+    return mu == 0 ? s.c[0] : mu == 2 ? s.c[2] : mu == 3 ? s.c[3] : s.c[1];
+}
+
+// half-index of x - mu_hat (which has the opposite parity), periodic
+__device__ __forceinline__ uint32_t backward_index(const Geom& G, const Site& s, int mu)
+{
+    if (mu == 1) {
+        if (s.xodd) return s.h;                                   // x-1 = 2 xh: same xh
+        return s.xh > 0 ? s.h - 1u : s.h + G.nxh - 1u;            // x-1 = 2 (xh-1) + 1, wraps
+    }
+    return coord(s, mu) > 0 ? s.h - G.stride[mu] : s.h + G.stride[mu] * (G.extent[mu] - 1u);
+}
+
+// half-index of x + mu_hat
+__device__ __forceinline__ uint32_t forward_index(const Geom& G, const Site& s, int mu)
+{
+    if (mu == 1) {
+        if (!s.xodd) return s.h;                                  // x+1 = 2 xh + 1: same xh
+        return s.xh + 1u < G.nxh ? s.h + 1u : s.h + 1u - G.nxh;
+    }
+    return coord(s, mu) + 1u < G.extent[mu] ? s.h + G.stride[mu] : s.h - G.stride[mu] * (G.extent[mu] - 1u);
+}
+
+// --------------------------------------------------------------------------------- link layout
+// field[parity][mu] is a block of RECON*Vh reals; inside a block the link of half-index h is
+// split into 16-byte chunks, chunk c of all sites contiguous:  block[c][h].
+//   fp64: chunk = double2 = one complex entry (9 or 6 chunks).
+//   fp32: chunk = float4 = two complex entries (RECON18: 4 chunks + one float2 tail array;
+//         RECON12: 3 chunks).
+// A warp reading chunk c of 32 consecutive sites moves 512 contiguous bytes with one 128-bit
+// load per lane; a neighbour shifted by one site stays 16-byte aligned.
+// Registers hold a link as m[18] = row-major (re, im) pairs.
+
+template <typename T> struct Vec16;
+template <> struct Vec16<double> { using type = double2; };
+template <> struct Vec16<float> { using type = float4; };
+
+template <typename T>
+__host__ __device__ __forceinline__ size_t block_offset(uint32_t parity, int mu, int recon, uint32_t Vh)
+{
+    return (size_t)(parity * 4u + (uint32_t)mu) * (size_t)recon * (size_t)Vh;   // in reals
+}
+
+template <int RECON>
+__device__ __forceinline__ void load_link(const double* __restrict__ blk, uint32_t Vh, uint32_t h, double (&m)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + h;
+#pragma unroll
+    for (int c = 0; c < RECON / 2; ++c) {
+        const double2 v = p[(size_t)c * Vh];
+        m[2 * c] = v.x;
+        m[2 * c + 1] = v.y;
+    }
+}
+
+template <int RECON>
+__device__ __forceinline__ void load_link(const float* __restrict__ blk, uint32_t Vh, uint32_t h, float (&m)[18])
+{
+    const float4* p = reinterpret_cast<const float4*>(blk) + h;
+#pragma unroll
+    for (int c = 0; c < RECON / 4; ++c) {
+        const float4 v = p[(size_t)c * Vh];
+        m[4 * c] = v.x;
+        m[4 * c + 1] = v.y;
+        m[4 * c + 2] = v.z;
+        m[4 * c + 3] = v.w;
+    }
+    if (RECON == 18) {
+        const float2 v = reinterpret_cast<const float2*>(blk + (size_t)16 * Vh)[h];
+        m[16] = v.x;
+        m[17] = v.y;
+    }
+}
+
+template <int RECON>
+__device__ __forceinline__ void store_link(double* __restrict__ blk, uint32_t Vh, uint32_t h, const double (&m)[18])
+{
+    double2* p = reinterpret_cast<double2*>(blk) + h;
+#pragma unroll
+    for (int c = 0; c < RECON / 2; ++c) p[(size_t)c * Vh] = make_double2(m[2 * c], m[2 * c + 1]);
+}
+
+template <int RECON>
+__device__ __forceinline__ void store_link(float* __restrict__ blk, uint32_t Vh, uint32_t h, const float (&m)[18])
+{
+    float4* p = reinterpret_cast<float4*>(blk) + h;
+#pragma unroll
+    for (int c = 0; c < RECON / 4; ++c)
+        p[(size_t)c * Vh] = make_float4(m[4 * c], m[4 * c + 1], m[4 * c + 2], m[4 * c + 3]);
+    if (RECON == 18) reinterpret_cast<float2*>(blk + (size_t)16 * Vh)[h] = make_float2(m[16], m[17]);
+}
+
+// ------------------------------------------------------------------------- 3x3 complex algebra
+#define GF_RE(m, a, b) (m)[2 * (3 * (a) + (b))]
+#define GF_IM(m, a, b) (m)[2 * (3 * (a) + (b)) + 1]
+
+// row 2 = conj(row 0 x row 1): the third row of an SU(3) matrix (GF_RECON12)
+template <typename T>
+__device__ __forceinline__ void reconstruct_row2(T (&m)[18])
+{
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const int b1 = (b + 1) % 3, b2 = (b + 2) % 3;
+        // (row0 x row1)_b = u0[b1] u1[b2] - u0[b2] u1[b1]
+        const T re = GF_RE(m, 0, b1) * GF_RE(m, 1, b2) - GF_IM(m, 0, b1) * GF_IM(m, 1, b2)
+                   - GF_RE(m, 0, b2) * GF_RE(m, 1, b1) + GF_IM(m, 0, b2) * GF_IM(m, 1, b1);
+        const T im = GF_RE(m, 0, b1) * GF_IM(m, 1, b2) + GF_IM(m, 0, b1) * GF_RE(m, 1, b2)
+                   - GF_RE(m, 0, b2) * GF_IM(m, 1, b1) - GF_IM(m, 0, b2) * GF_RE(m, 1, b1);
+        GF_RE(m, 2, b) = re;
+        GF_IM(m, 2, b) = -im;
+    }
+}
+
+// out = g U, rows 0..ROWS-1 only
+template <int ROWS, typename T>
+__device__ __forceinline__ void mul_g_U(const T (&g)[18], const T (&U)[18], T (&out)[18])
+{
+#pragma unroll
+    for (int a = 0; a < ROWS; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            T re = T(0), im = T(0);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                re += GF_RE(g, a, k) * GF_RE(U, k, b) - GF_IM(g, a, k) * GF_IM(U, k, b);
+                im += GF_RE(g, a, k) * GF_IM(U, k, b) + GF_IM(g, a, k) * GF_RE(U, k, b);
+            }
+            GF_RE(out, a, b) = re;
+            GF_IM(out, a, b) = im;
+        }
+}
+
+// out = U g^dagger, rows 0..ROWS-1 only:  out_ab = sum_k U_ak conj(g_bk)
+template <int ROWS, typename T>
+__device__ __forceinline__ void mul_U_gdag(const T (&U)[18], const T (&g)[18], T (&out)[18])
+{
+#pragma unroll
+    for (int a = 0; a < ROWS; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            T re = T(0), im = T(0);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                re += GF_RE(U, a, k) * GF_RE(g, b, k) + GF_IM(U, a, k) * GF_IM(g, b, k);
+                im += GF_IM(U, a, k) * GF_RE(g, b, k) - GF_RE(U, a, k) * GF_IM(g, b, k);
+            }
+            GF_RE(out, a, b) = re;
+            GF_IM(out, a, b) = im;
+        }
+}
+
+__device__ __forceinline__ float gf_rsqrt(float x) { return rsqrtf(x); }
+__device__ __forceinline__ double gf_rsqrt(double x) { return rsqrt(x); }
+
+// -------------------------------------------------------------------- the SU(2) subgroup step
+enum { ALGO_RELAX = 0, ALGO_OVERRELAX = 1, ALGO_STOCHASTIC = 2 };
+
+// One of the three SU(2) maximisations of PAPER.md:76 for the subgroup (I,J).  The 2x2 block of
+// K is projected on SU(2) x R+ :  Re tr[a K_sub] = a . v  for
+//   a = [[a0 + i a3, a2 + i a1], [-a2 + i a1, a0 - i a3]],
+//   v = (Re(K_II + K_JJ), -Im(K_IJ + K_JI), Re(K_JI - K_IJ), Im(K_JJ - K_II)),
+// so eq. 9 gives a = v/|v|.  Overrelaxation (first order):
+// a -> normalise(1 + omega (a - 1)) = normalise(omega v + (1 - omega)|v| e0).  Stochastic
+// relaxation: a -> a^2 when `square`.  Then K <- E K and g <- E g.
+template <int I, int J, typename T>
+__device__ __forceinline__ void su2_step(T (&K)[18], T (&g)[18], int algo, T omega, bool square)
+{
+    T v0 = GF_RE(K, I, I) + GF_RE(K, J, J);
+    T v1 = -(GF_IM(K, I, J) + GF_IM(K, J, I));
+    T v2 = GF_RE(K, J, I) - GF_RE(K, I, J);
+    T v3 = GF_IM(K, J, J) - GF_IM(K, I, I);
+    T nn = v0 * v0 + v1 * v1 + v2 * v2 + v3 * v3;
+    T a0 = T(1), a1 = T(0), a2 = T(0), a3 = T(0);
+    if (nn > T(0)) {
+        T rn = gf_rsqrt(nn);
+        if (algo == ALGO_OVERRELAX) {
+            const T n = nn * rn;
+            v0 = omega * v0 + (T(1) - omega) * n;
+            v1 *= omega;
+            v2 *= omega;
+            v3 *= omega;
+            nn = v0 * v0 + v1 * v1 + v2 * v2 + v3 * v3;
+            rn = gf_rsqrt(nn);
+        }
+        a0 = v0 * rn;
+        a1 = v1 * rn;
+        a2 = v2 * rn;
+        a3 = v3 * rn;
+        if (square) {
+            const T t = a0 + a0;
+            a0 = t * a0 - T(1);
+            a1 *= t;
+            a2 *= t;
+            a3 *= t;
+        }
+    }
+    // E_II = a0 + i a3, E_IJ = a2 + i a1, E_JI = -a2 + i a1, E_JJ = a0 - i a3
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        {
+            const T ir = GF_RE(K, I, b), ii = GF_IM(K, I, b), jr = GF_RE(K, J, b), ji = GF_IM(K, J, b);
+            GF_RE(K, I, b) = a0 * ir - a3 * ii + a2 * jr - a1 * ji;
+            GF_IM(K, I, b) = a0 * ii + a3 * ir + a2 * ji + a1 * jr;
+            GF_RE(K, J, b) = -a2 * ir - a1 * ii + a0 * jr + a3 * ji;
+            GF_IM(K, J, b) = -a2 * ii + a1 * ir + a0 * ji - a3 * jr;
+        }
+        {
+            const T ir = GF_RE(g, I, b), ii = GF_IM(g, I, b), jr = GF_RE(g, J, b), ji = GF_IM(g, J, b);
+            GF_RE(g, I, b) = a0 * ir - a3 * ii + a2 * jr - a1 * ji;
+            GF_IM(g, I, b) = a0 * ii + a3 * ir + a2 * ji + a1 * jr;
+            GF_RE(g, J, b) = -a2 * ir - a1 * ii + a0 * jr + a3 * ji;
+            GF_IM(g, J, b) = -a2 * ii + a1 * ir + a0 * ji - a3 * jr;
+        }
+    }
+}
+
+// --------------------------------------------------------------------------- Philox4x32-10
+// Salmon et al., SC'11 (public algorithm).  Counter-based: no state in memory.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              uint32_t k0, uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+}  // namespace gf

@@ -1,0 +1,49 @@
+// gf_internal.h -- host-side declarations shared by the translation units of libgf_b200.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "gf_device.cuh"
+
+namespace gf {
+
+enum { PREC_F32 = 0, PREC_F64 = 1 };
+
+struct SweepArgs {
+    void* links;            // internal field of the chosen precision
+    Geom G;
+    uint32_t parity;        // active parity
+    int mu0;                // first direction entering K: 0 Landau, 1 Coulomb
+    int algo;               // ALGO_*
+    double omega, p;
+    uint32_t key0, key1;    // Philox key = seed
+    uint32_t counter;       // half-sweep counter (Philox counter word 2)
+};
+
+struct MeasureGrid {
+    uint32_t Sh;            // sites per time slice per parity
+    uint32_t bpp;           // blocks per (slice, parity)
+    uint32_t block;         // threads per block
+};
+
+// every launcher returns cudaGetLastError() after the launch
+// solver_f64: with fp32 storage, accumulate K(x) and run the SU(2) solves in fp64 registers
+cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);
+bool sweep_config_valid(int lanes, int block);
+
+cudaError_t launch_measure(int precision, int recon, const void* links, const Geom& G, int mu0,
+                           const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
+cudaError_t launch_plaquette(int precision, int recon, const void* links, const Geom& G,
+                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
+cudaError_t launch_unitarity(int precision, int recon, const void* links, const Geom& G,
+                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
+cudaError_t launch_pack(int precision, int recon, void* links, const Geom& G, const void* canonical,
+                        int canonical_is_f64, cudaStream_t st);
+cudaError_t launch_unpack(int precision, int recon, const void* links, const Geom& G, void* canonical,
+                          int canonical_is_f64, cudaStream_t st);
+cudaError_t launch_cast(int from_precision, int to_precision, int recon, const void* src, void* dst,
+                        const Geom& G, int reproject, cudaStream_t st);
+cudaError_t launch_philox(int n, const uint32_t* ctr, const uint32_t* key, uint32_t* out, cudaStream_t st);
+
+}  // namespace gf

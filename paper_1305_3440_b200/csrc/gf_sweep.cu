@@ -1,0 +1,181 @@
+// gf_sweep.cu -- the checkerboard relaxation half-sweep, the hot kernel.
+//
+// Traffic: a half-sweep reads and writes every link exactly once (the V/2 active sites each own
+// 4 forward links and touch the 4 backward links U_mu(x-mu), which are stored on the other
+// parity), so the algorithmic bytes per site-update are 16 * RECON * sizeof(T) and the kernel is
+// HBM bound (0.9-2.8 flop/byte).  No tensor cores: there is no dense contraction here.
+//
+// Mapping: L = 1, 2 or 4 lanes cooperate on one site.  Lane j of a site owns the directions
+// mu = j*(4/L) .. and keeps U_mu(x) and U_mu(x-mu) in registers (fp64 with L = 1 would need 288
+// registers for the links alone).  A warp covers S = 32/L consecutive half-indices; lanes with
+// the same j are contiguous in h, so every 128-bit load instruction of a warp touches L fully
+// used contiguous runs of S*16 bytes.  The partial K's are combined with an xor-butterfly of
+// warp shuffles (bitwise identical in all lanes, additions commute), every lane then computes
+// the same g(x) redundantly and applies it to its own links.  The paper's kernel used 8 threads
+// per site through shared memory; that is prior art, not this design.
+#include "gf_internal.h"
+
+namespace gf {
+
+template <typename T, typename TK> struct SweepConsts {
+    T* links;
+    Geom G;
+    uint32_t parity;
+    int mu0, algo;
+    TK omega;
+    double p;
+    uint32_t key0, key1, counter;
+};
+
+template <typename T>
+__device__ __forceinline__ T shfl_xor_T(T v, int mask)
+{
+    return __shfl_xor_sync(0xffffffffu, v, mask);
+}
+
+// T: storage type and the type of the 3x3 products of step a6; TK: type in which K(x) is
+// accumulated and the SU(2) solves run (TK = double with T = float costs no bandwidth and removes
+// the amplification of fp32 rounding at sites with a small |v|).
+template <typename T, typename TK, int RECON, int L>
+__global__ void sweep_kernel(const SweepConsts<T, TK> P)
+{
+    constexpr int S = 32 / L;    // sites per warp
+    constexpr int ND = 4 / L;    // directions per lane
+    constexpr int ROWS = RECON == 12 ? 2 : 3;
+    const Geom& G = P.G;
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (warp * S >= G.Vh) return;                       // warp-uniform
+    uint32_t h = warp * S + (lane % S);
+    const int j = lane / S;
+    const bool live = h < G.Vh;
+    if (!live) h = G.Vh - 1u;                           // keeps the lane in the shuffles; no store
+    const Site s = decode_site(G, h, P.parity);
+
+    // a2: gather this lane's links
+    T Uf[ND][18], Ub[ND][18];
+    uint32_t hb[ND];
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+        const int mu = j * ND + d;
+        hb[d] = backward_index(G, s, mu);
+        load_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
+        load_link<RECON>(P.links + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
+    }
+    if (RECON == 12) {
+#pragma unroll
+        for (int d = 0; d < ND; ++d) {
+            reconstruct_row2(Uf[d]);
+            reconstruct_row2(Ub[d]);
+        }
+    }
+
+    // a3: K(x) = sum_mu [U_mu(x) + U_mu(x-mu)^dagger]  (eq. 8, neighbours' g = 1)
+    TK K[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) K[k] = TK(0);
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+        const int mu = j * ND + d;
+        if (mu >= P.mu0) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b) {
+                    GF_RE(K, a, b) += (TK)GF_RE(Uf[d], a, b) + (TK)GF_RE(Ub[d], b, a);
+                    GF_IM(K, a, b) += (TK)GF_IM(Uf[d], a, b) - (TK)GF_IM(Ub[d], b, a);
+                }
+        }
+    }
+#pragma unroll
+    for (int off = S; off < 32; off <<= 1) {
+#pragma unroll
+        for (int k = 0; k < 18; ++k) K[k] += shfl_xor_T(K[k], off);
+    }
+
+    // a5: the stochastic-relaxation draws, one Philox call per site visit
+    bool sq0 = false, sq1 = false, sq2 = false;
+    if (P.algo == ALGO_STOCHASTIC) {
+        uint32_t w[4];
+        philox4x32_10(2u * h + s.xodd, 0u, P.counter, 0u, P.key0, P.key1, w);
+        sq0 = (double)(w[0] >> 8) * (1.0 / 16777216.0) < P.p;
+        sq1 = (double)(w[1] >> 8) * (1.0 / 16777216.0) < P.p;
+        sq2 = (double)(w[2] >> 8) * (1.0 / 16777216.0) < P.p;
+    }
+
+    // a4: the three SU(2) subgroups, g = E3 E2 E1
+    TK gk[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) gk[k] = TK(0);
+    gk[0] = gk[8] = gk[16] = TK(1);
+    su2_step<0, 1>(K, gk, P.algo, P.omega, sq0);
+    su2_step<0, 2>(K, gk, P.algo, P.omega, sq1);
+    su2_step<1, 2>(K, gk, P.algo, P.omega, sq2);
+    T g[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) g[k] = (T)gk[k];
+
+    // a6: U_mu(x) <- g U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) g^dagger  (eq. 3)
+    if (!live) return;
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+        const int mu = j * ND + d;
+        T out[18];
+        mul_g_U<ROWS>(g, Uf[d], out);
+        store_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, out);
+        mul_U_gdag<ROWS>(Ub[d], g, out);
+        store_link<RECON>(P.links + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
+    }
+}
+
+template <typename T, typename TK, int RECON, int L>
+static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
+{
+    SweepConsts<T, TK> P;
+    P.links = static_cast<T*>(a.links);
+    P.G = a.G;
+    P.parity = a.parity;
+    P.mu0 = a.mu0;
+    P.algo = a.algo;
+    P.omega = (TK)a.omega;
+    P.p = a.p;
+    P.key0 = a.key0;
+    P.key1 = a.key1;
+    P.counter = a.counter;
+    const uint64_t threads = (uint64_t)a.G.Vh * L;
+    const uint32_t grid = (uint32_t)((threads + block - 1) / block);
+    sweep_kernel<T, TK, RECON, L><<<grid, block, 0, st>>>(P);
+    return cudaGetLastError();
+}
+
+bool sweep_config_valid(int lanes, int block)
+{
+    return (lanes == 1 || lanes == 2 || lanes == 4) && (block == 64 || block == 128 || block == 256 || block == 512);
+}
+
+template <typename T, typename TK, int RECON>
+static cudaError_t launch_lanes(int lanes, int block, const SweepArgs& a, cudaStream_t st)
+{
+    switch (lanes) {
+        case 1: return launch_one<T, TK, RECON, 1>(block, a, st);
+        case 2: return launch_one<T, TK, RECON, 2>(block, a, st);
+        case 4: return launch_one<T, TK, RECON, 4>(block, a, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <typename T, typename TK>
+static cudaError_t launch_recon(int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st)
+{
+    return recon == 12 ? launch_lanes<T, TK, 12>(lanes, block, a, st) : launch_lanes<T, TK, 18>(lanes, block, a, st);
+}
+
+cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st)
+{
+    if (!sweep_config_valid(lanes, block)) return cudaErrorInvalidValue;
+    if (precision == PREC_F64) return launch_recon<double, double>(recon, lanes, block, a, st);
+    return solver_f64 ? launch_recon<float, double>(recon, lanes, block, a, st)
+                      : launch_recon<float, float>(recon, lanes, block, a, st);
+}
+
+}  // namespace gf

@@ -1,0 +1,111 @@
+"""GaugeField: owns the torch buffers a gf_ctx borrows and forwards to the C ABI.
+
+No arithmetic here: allocation, pointer hand-over and dtype checks only.
+"""
+import torch
+
+from . import binding as B
+
+
+class GaugeField:
+    """A lattice on one GPU.
+
+    dims = (Nt, Nx, Ny, Nz); precisions: any of ("f32", "f64") to allocate storage for
+    (GF_MIXED needs both).  Canonical tensors are complex, shape (Nt, Nz, Ny, Nx, 4, 3, 3).
+    """
+
+    def __init__(self, dims, gauge=B.GF_LANDAU, recon=B.GF_RECON18, precisions=("f64",), seed=0,
+                 device="cuda:0", staging=False):
+        self.dims = tuple(int(d) for d in dims)
+        self.gauge, self.recon = gauge, recon
+        self.device = torch.device(device)
+        self.n_out = self.dims[0] if gauge == B.GF_COULOMB else 1
+        self.shape = (self.dims[0], self.dims[3], self.dims[2], self.dims[1], 4, 3, 3)
+        self._bufs = {}
+        for name, prec in (("f32", B.GF_F32), ("f64", B.GF_F64)):
+            if name in precisions:
+                n = B.gf_storage_bytes(self.dims, prec, recon)
+                if n == 0:
+                    raise ValueError("invalid dims/recon %r %r" % (dims, recon))
+                self._bufs[prec] = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._ws = torch.empty(B.gf_workspace_bytes(self.dims), dtype=torch.uint8, device=self.device)
+        self._staging = None
+        if staging:
+            self._staging = torch.empty(self.shape, dtype=torch.complex128, device=self.device)
+        with torch.cuda.device(self.device):
+            self.stream = torch.cuda.current_stream()
+            self.ctx = B.gf_init_lattice(
+                self.dims, gauge, recon,
+                self._bufs[B.GF_F64].data_ptr() if B.GF_F64 in self._bufs else 0,
+                self._bufs[B.GF_F32].data_ptr() if B.GF_F32 in self._bufs else 0,
+                self._ws.data_ptr(), self.stream.cuda_stream, seed)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            torch.cuda.synchronize(self.device)
+            B.gf_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- layout conversion
+    def _canon(self, t):
+        if t.dtype not in (torch.complex128, torch.complex64) or tuple(t.shape) != self.shape \
+                or not t.is_contiguous() or t.device != self.device:
+            raise ValueError("canonical tensor must be contiguous complex %r on %s" % (self.shape, self.device))
+        return t.data_ptr(), t.dtype == torch.complex128
+
+    def pack(self, canonical, precision):
+        ptr, is64 = self._canon(canonical)
+        B.gf_pack(self.ctx, ptr, is64, precision)
+
+    def unpack(self, precision, dtype=torch.complex128):
+        out = torch.empty(self.shape, dtype=dtype, device=self.device)
+        B.gf_unpack(self.ctx, out.data_ptr(), dtype == torch.complex128, precision)
+        return out
+
+    def load_host(self, host_canonical, precision):
+        """host_canonical: CPU (ideally pinned) complex tensor; needs staging=True."""
+        B.gf_load_host(self.ctx, host_canonical.data_ptr(), host_canonical.dtype == torch.complex128, precision,
+                       self._staging.data_ptr())
+
+    def store_host(self, host_canonical, precision):
+        B.gf_store_host(self.ctx, host_canonical.data_ptr(), host_canonical.dtype == torch.complex128, precision,
+                        self._staging.data_ptr())
+
+    # ---- the method
+    def sweep(self, parity, algo, omega, p, precision):
+        B.gf_sweep(self.ctx, parity, algo, omega, p, precision)
+
+    def iterate(self, n, algo, omega, p, precision):
+        for _ in range(n):
+            B.gf_sweep(self.ctx, 0, algo, omega, p, precision)
+            B.gf_sweep(self.ctx, 1, algo, omega, p, precision)
+
+    def functional(self, precision):
+        return B.gf_functional(self.ctx, precision, self.n_out)
+
+    def theta(self, precision):
+        return B.gf_theta(self.ctx, precision, self.n_out)
+
+    def measure(self, precision):
+        return B.gf_measure(self.ctx, precision, self.n_out)
+
+    def fix_until(self, algo, omega, p, precision, theta_target, max_iter, check_every=1):
+        return B.gf_fix_until(self.ctx, algo, omega, p, precision, theta_target, max_iter, check_every)
+
+    def plaquette(self, precision):
+        return B.gf_plaquette(self.ctx, precision)
+
+    def unitarity(self, precision):
+        return B.gf_unitarity(self.ctx, precision)
+
+    def set_tuning(self, precision, lanes, block):
+        B.gf_set_tuning(self.ctx, precision, lanes, block)
+
+    def set_solver_precision(self, solver_precision):
+        B.gf_set_solver_precision(self.ctx, solver_precision)
