@@ -140,6 +140,12 @@ int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2);
  * summation order inside K. */
 int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_threads);
 
+/* Order in which the blocks of consecutive gf_sweep launches walk the lattice: 1 (default) =
+ * zigzag, every other half-sweep runs from the last site to the first, so that a launch starts on
+ * the links the previous one touched last and finds them in the L2 cache; 0 = always ascending.
+ * The links produced are bitwise the same (sites of one parity are independent). */
+int gf_set_traversal(gf_ctx* ctx, int zigzag);
+
 /* Arithmetic of the per-site solver when the STORAGE is fp32 (gf_sweep with GF_F32): K(x) is
  * accumulated and the three SU(2) solves run in solver_precision: GF_F32 (everything in fp32),
  * GF_F64 (fp64 registers: no extra memory traffic, ~15 % more time, removes the amplification of

@@ -13,6 +13,6 @@ from .binding import (  # noqa: F401
     gf_storage_bytes, gf_workspace_bytes, gf_init_lattice, gf_destroy, gf_last_error,
     gf_pack, gf_unpack, gf_load_host, gf_store_host, gf_sweep, gf_functional, gf_theta,
     gf_measure, gf_fix_until, gf_set_rng, gf_get_counter, gf_reunitarize, gf_cast,
-    gf_plaquette, gf_unitarity, gf_set_tuning, gf_set_solver_precision, gf_debug_philox, gf_launch_count,
+    gf_plaquette, gf_unitarity, gf_set_tuning, gf_set_solver_precision, gf_set_traversal, gf_debug_philox, gf_launch_count,
 )
 from .field import GaugeField  # noqa: F401

@@ -54,6 +54,7 @@ def _load():
         "gf_unitarity": (i32, [vp, i32, dp]),
         "gf_set_tuning": (i32, [vp, i32, i32, i32]),
         "gf_set_solver_precision": (i32, [vp, i32]),
+        "gf_set_traversal": (i32, [vp, i32]),
         "gf_debug_philox": (i32, [vp, i32, vp, vp, vp]),
         "gf_launch_count": (i32, [vp, C.POINTER(u64)]),
         "gf_last_error": (C.c_char_p, [vp]),
@@ -68,7 +69,7 @@ def _load():
 lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
            "gf_sweep gf_functional gf_theta gf_measure gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
-           "gf_cast gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_debug_philox gf_launch_count gf_last_error "
+           "gf_cast gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
 
 
@@ -202,6 +203,10 @@ def gf_set_tuning(ctx, precision, lanes_per_site, block_threads, check=True):
 
 def gf_set_solver_precision(ctx, solver_precision, check=True):
     return _rc(ctx, lib.gf_set_solver_precision(ctx, solver_precision), check)
+
+
+def gf_set_traversal(ctx, zigzag, check=True):
+    return _rc(ctx, lib.gf_set_traversal(ctx, int(zigzag)), check)
 
 
 def gf_debug_philox(ctx, n, dev_counters, dev_keys, dev_out, check=True):

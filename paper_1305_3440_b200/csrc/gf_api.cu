@@ -31,6 +31,8 @@ struct gf_ctx {
     MeasureGrid mg;
     size_t V;
     int lanes[2], block[2];
+    int zigzag;                 // alternate the traversal direction of consecutive half-sweeps
+    uint64_t sweeps;            // half-sweeps enqueued so far (selects the direction)
     int solver_mode;            // fp32 storage: K and the SU(2) solves in GF_F32, GF_F64 or GF_SOLVER_AUTO
     uint64_t launches;
     char err[256];
@@ -138,7 +140,9 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     // defaults chosen by measurement on B200 at 32^4 ("Kernels"); gf_set_tuning overrides
     c->lanes[PREC_F32] = 2;  c->block[PREC_F32] = 128;
     c->lanes[PREC_F64] = 2;  c->block[PREC_F64] = 128;
+    if (recon == GF_RECON12) { c->lanes[PREC_F64] = 1;  c->block[PREC_F64] = 64; }
     c->solver_mode = GF_SOLVER_AUTO;
+    c->zigzag = 1;
 
     if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt) != cudaSuccess) {
         cudaGetLastError();
@@ -234,10 +238,12 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.key0 = (uint32_t)ctx->seed;
     a.key1 = (uint32_t)(ctx->seed >> 32);
     a.counter = ctx->counter;
+    a.reverse = ctx->zigzag ? (uint32_t)(ctx->sweeps & 1u) : 0u;
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
     cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, ctx->lanes[precision], ctx->block[precision], a, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_sweep launch");
     ctx->counter += 1;
+    ctx->sweeps += 1;
     ctx->launches += 1;
     return GF_OK;
 }
@@ -473,6 +479,14 @@ extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int
     if (!sweep_config_valid(lanes, block)) return fail(ctx, GF_EINVAL, "lanes must be 1,2,4 and block 64..512 (power of two)");
     ctx->lanes[precision] = lanes;
     ctx->block[precision] = block;
+    return GF_OK;
+}
+
+extern "C" int gf_set_traversal(gf_ctx* ctx, int zigzag)
+{
+    if (!ctx) return GF_EINVAL;
+    if (zigzag != 0 && zigzag != 1) return fail(ctx, GF_EINVAL, "traversal must be 0 (forward) or 1 (zigzag)");
+    ctx->zigzag = zigzag;
     return GF_OK;
 }
 

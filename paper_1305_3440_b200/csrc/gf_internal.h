@@ -19,6 +19,7 @@ struct SweepArgs {
     double omega, p;
     uint32_t key0, key1;    // Philox key = seed
     uint32_t counter;       // half-sweep counter (Philox counter word 2)
+    uint32_t reverse;       // traverse the lattice backwards (L2 reuse between consecutive launches)
 };
 
 struct MeasureGrid {

@@ -25,6 +25,7 @@ template <typename T, typename TK> struct SweepConsts {
     TK omega;
     double p;
     uint32_t key0, key1, counter;
+    uint32_t reverse;       // 1: blocks walk the lattice from the last site to the first
 };
 
 template <typename T>
@@ -44,7 +45,11 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     constexpr int ROWS = RECON == 12 ? 2 : 3;
     const Geom& G = P.G;
     const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    // Alternate half-sweeps walk the lattice in opposite directions (blocks are dispatched in
+    // ascending blockIdx order): the launch starts on the sites the previous one finished with,
+    // whose links are still in the 126 MB L2.  The result does not depend on the order.
+    const uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+    const uint32_t warp = (bid * blockDim.x + threadIdx.x) >> 5;
     if (warp * S >= G.Vh) return;                       // warp-uniform
     uint32_t h = warp * S + (lane % S);
     const int j = lane / S;
@@ -142,6 +147,7 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     P.key0 = a.key0;
     P.key1 = a.key1;
     P.counter = a.counter;
+    P.reverse = a.reverse;
     const uint64_t threads = (uint64_t)a.G.Vh * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);
     sweep_kernel<T, TK, RECON, L><<<grid, block, 0, st>>>(P);

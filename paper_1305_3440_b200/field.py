@@ -109,3 +109,6 @@ class GaugeField:
 
     def set_solver_precision(self, solver_precision):
         B.gf_set_solver_precision(self.ctx, solver_precision)
+
+    def set_traversal(self, zigzag):
+        B.gf_set_traversal(self.ctx, zigzag)
