@@ -40,6 +40,11 @@ VARIANTS = {            # name: (precision key, recon, bytes per real)
 }
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per sweep_kernel launch at 32^4, from the `ncu --set full`
+# captures summarised in profiles/r1_sweep_variants_ncu.md (average of a forward and a reverse launch)
+NCU_TRAFFIC_BYTES = {}
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -85,34 +90,21 @@ class ClockSampler:
 
 def run_ours(args):
     import torch
-    import torch.distributed as dist
 
     import gf_inputs as gi
     import paper_1305_3440_b200 as gf
+    from paper_1305_3440_b200.replicas import Replicas
 
-    rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
+    rep = Replicas(backend="nccl", device=dev)      # barrier + one scalar all-reduce; no data-path collective
+    rank, world = rep.rank, rep.world
+    barrier, max_over_ranks = rep.barrier, rep.max_over_ranks
     peak, peak_src = measured_peaks()
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
     # same recipe on every rank, rank-dependent seed: one independent configuration per GPU
-    U64 = gi.torch_smooth_random_gauge(DIMS, EPS, SEED + rank, device=dev)
+    U64 = gi.torch_smooth_random_gauge(DIMS, EPS, rep.config_seed(SEED), device=dev)
 
     def bench_variant(name, steps, warmup, with_e2e):
         pkey, recon, B = VARIANTS[name]
@@ -160,7 +152,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
+                         "traffic": NCU_TRAFFIC_BYTES.get(name), "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
                          "bytes_per_launch": bytes_per_launch, "avg_launch_ms": kern_ms, "peak_source": peak_src,
                          "frac_of_8TBs_nominal": achieved / 8000.0},
             "final_F": F[0], "final_theta": th[0],
@@ -220,8 +212,7 @@ def run_ours(args):
             "final_F": main["final_F"], "final_theta": main["final_theta"],
         }
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 def cpu_baseline(U, budget_s):

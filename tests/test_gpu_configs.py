@@ -1,0 +1,185 @@
+"""GPU tests at BASELINE.json's full config sizes (configs[1], [3], [4]) in the default launch
+configuration: sampled outputs recomputed one by one by the oracle, properties that hold at any
+size (plaquette, unitarity, monotone F, theta falling), and the fix loop against the oracle where the
+oracle finishes in seconds (16^4)."""
+import numpy as np
+import pytest
+import torch
+
+import gf_inputs as gi
+import oracle
+import paper_1305_3440_b200 as gf
+
+pytestmark = pytest.mark.gpu
+
+PREC = {"f64": gf.GF_F64, "f32": gf.GF_F32}
+CDTYPE = {"f64": torch.complex128, "f32": torch.complex64}
+LINK_TOL = {"f64": 1e-12, "f32": 1e-5}
+
+
+def _site_and_backward(dims, s):
+    nt, nx, ny, nz = dims
+    x, y, z, t = s % nx, (s // nx) % ny, (s // (nx * ny)) % nz, s // (nx * ny * nz)
+
+    def idx(t, x, y, z):
+        return x + nx * (y + ny * (z + nz * t))
+    back = [idx((t - 1) % nt, x, y, z), idx(t, (x - 1) % nx, y, z), idx(t, x, (y - 1) % ny, z), idx(t, x, y, (z - 1) % nz)]
+    return (x + y + z + t) % 2, back
+
+
+def sampled_sweep_check(fld, dims, prec, gauge, ogauge, algo, oalgo, omega, p, seed, nsamples, rng):
+    """One iteration (parity 0 then 1); after each half-sweep `nsamples` random active sites are
+    recomputed by the oracle's single-site update from the pre-sweep links (and the oracle's own
+    Philox draws for the stochastic variant)."""
+    before = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
+    V = before.shape[0]
+    for parity in (0, 1):
+        counter = gf.gf_get_counter(fld.ctx)
+        fld.sweep(parity, algo, omega, p, PREC[prec])
+        after = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
+        picked = 0
+        while picked < nsamples:
+            s = int(rng.integers(0, V))
+            par, back = _site_and_backward(dims, s)
+            if par != parity:
+                continue
+            picked += 1
+            fwd = before[s].cpu().numpy().copy()
+            bwd = np.stack([before[back[mu], mu].cpu().numpy() for mu in range(4)])
+            u = oracle.site_uniforms(seed, counter, s) if oalgo == oracle.STOCHASTIC else (0.0, 0.0, 0.0)
+            oracle.update_links8(fwd, bwd, ogauge, oalgo, omega, p, u)
+            got_f = after[s].cpu().numpy()
+            got_b = np.stack([after[back[mu], mu].cpu().numpy() for mu in range(4)])
+            assert np.abs(got_f - fwd).max() < LINK_TOL[prec], (s, parity)
+            assert np.abs(got_b - bwd).max() < LINK_TOL[prec], (s, parity)
+        before = after
+        del after
+
+
+# ------------------------------------------------------------------------------ configs[1]: 16^4
+
+def test_config2_16_4_smooth_fix_matches_oracle(cuda_device):
+    """16^4, eps 0.5, seed 1234, omega 1.7: fp64 until theta < 1e-12 (check every 10) against the
+    oracle's fix loop; fp32 until theta < 1e-6."""
+    dims = (16, 16, 16, 16)
+    U = gi.smooth_random_gauge(dims, 0.5, 1234)
+    oracle.set_threads(0)
+    Uo = U.copy()
+    it_o, th_o, conv = oracle.fix_until(Uo, dims, oracle.LANDAU, oracle.OVERRELAX, 1.7, theta_target=1e-12,
+                                        max_iter=20000, check_every=10)
+    oracle.set_threads(1)
+    assert conv
+    fld = gf.GaugeField(dims, precisions=("f64", "f32"), device=cuda_device)
+    Ud = torch.from_numpy(U).to(cuda_device)
+    fld.pack(Ud, gf.GF_F64)
+    fld.pack(Ud.to(torch.complex64), gf.GF_F32)
+    P0 = fld.plaquette(gf.GF_F64)
+    assert abs(P0 - oracle.plaquette(U, dims)) < 1e-13
+    rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64, 1e-12, 20000, 10)
+    assert rc == gf.GF_OK and th < 1e-12
+    assert abs(it - it_o) <= 10, (it, it_o)
+    assert abs(fld.plaquette(gf.GF_F64) - P0) < 1e-12
+    du, dd = fld.unitarity(gf.GF_F64)
+    assert du < 1e-12 and dd < 1e-12
+    F = fld.functional(gf.GF_F64)[0]
+    assert abs(F - oracle.functional(Uo, dims)) < 1e-9          # same maximum of the functional
+    got = fld.unpack(gf.GF_F64).cpu().numpy()
+    assert oracle.theta(np.ascontiguousarray(got), dims) < 1.01e-12      # the oracle agrees it is fixed
+    # fp32 to 1e-6
+    rc, it32, th32 = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F32, 1e-6, 20000, 10)
+    assert rc == gf.GF_OK and th32 < 1e-6 and it32 < it
+    assert abs(fld.plaquette(gf.GF_F32) - P0) < 1e-5
+    fld.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config2_16_4_hot_500_sweeps(cuda_device, prec):
+    """16^4 Haar-random links, 500 fixed sweeps: F rises monotonically (checked every 50), theta falls
+    overall, gauge invariants hold; after the first 10 sweeps F and theta match the oracle."""
+    dims = (16, 16, 16, 16)
+    U = gi.hot_links(dims, 1234)
+    Uo = np.ascontiguousarray(U.astype(np.complex64).astype(np.complex128)) if prec == "f32" else U.copy()
+    fld = gf.GaugeField(dims, precisions=(prec,), device=cuda_device)
+    fld.pack(torch.from_numpy(U).to(cuda_device).to(CDTYPE[prec]), PREC[prec])
+    P0 = fld.plaquette(PREC[prec])
+    F0, th0 = fld.measure(PREC[prec])
+    fld.iterate(10, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+    oracle.set_threads(0)
+    for it in range(10):
+        for parity in (0, 1):
+            oracle.sweep(Uo, dims, parity, oracle.LANDAU, oracle.OVERRELAX, 1.7)
+    oracle.set_threads(1)
+    F, th = fld.measure(PREC[prec])
+    rtol = 1e-10 if prec == "f64" else 1e-5
+    assert abs(F[0] / oracle.functional(Uo, dims) - 1) < rtol
+    assert abs(th[0] / oracle.theta(Uo, dims) - 1) < rtol
+    Fs, ths = [F[0]], [th[0]]
+    for _ in range(49):
+        fld.iterate(10, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+        F, th = fld.measure(PREC[prec])
+        Fs.append(F[0])
+        ths.append(th[0])
+    assert all(b > a for a, b in zip(Fs[4::5], Fs[9::5])) and Fs[-1] > F0[0] + 0.3
+    assert ths[-1] < 1e-2 * th0[0]
+    assert abs(fld.plaquette(PREC[prec]) - P0) < (1e-12 if prec == "f64" else 1e-5)
+    du, dd = fld.unitarity(PREC[prec])
+    assert du < (1e-12 if prec == "f64" else 1e-4)
+    fld.close()
+
+
+# ------------------------------------------------------------------------------ configs[3]: 64^4
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config4_64_4(cuda_device, prec):
+    """64^4 (16.8 M sites; 9.66 GB of fp64 links, byte offsets beyond 2^32), omega 1.8: one iteration
+    with sampled sites recomputed by the oracle, then 200 sweeps with F/theta every 10."""
+    dims = (64, 64, 64, 64)
+    U = gi.torch_smooth_random_gauge(dims, 0.6, 4, device=cuda_device).to(CDTYPE[prec])
+    fld = gf.GaugeField(dims, precisions=(prec,), device=cuda_device)
+    fld.pack(U, PREC[prec])
+    del U
+    torch.cuda.empty_cache()
+    P0 = fld.plaquette(PREC[prec])
+    rng = np.random.default_rng(64)
+    sampled_sweep_check(fld, dims, prec, gf.GF_LANDAU, oracle.LANDAU, gf.GF_OVERRELAX, oracle.OVERRELAX, 1.8, 0.0, 0, 24, rng)
+    torch.cuda.empty_cache()
+    Fs, ths = [], []
+    for _ in range(20):
+        fld.iterate(10, gf.GF_OVERRELAX, 1.8, 0.0, PREC[prec])
+        F, th = fld.measure(PREC[prec])
+        Fs.append(F[0])
+        ths.append(th[0])
+    assert all(b > a for a, b in zip(Fs, Fs[1:]))                  # F keeps rising
+    assert ths[-1] < 0.1 * ths[0]
+    assert abs(fld.plaquette(PREC[prec]) - P0) < (1e-12 if prec == "f64" else 1e-5)
+    du, dd = fld.unitarity(PREC[prec])
+    assert du < (1e-12 if prec == "f64" else 1e-4) and dd < (1e-12 if prec == "f64" else 1e-4)
+    fld.close()
+
+
+# ------------------------------------------------------------------------------ configs[4]: Coulomb
+
+def test_config5_coulomb_32_3x64_stochastic(cuda_device):
+    """32^3 x 64 Coulomb gauge, fp64, stochastic relaxation p = 0.8, Philox seed 2013: sampled sites of
+    the first iteration against the oracle (same Philox draws), then the fix loop until theta_t < 1e-12
+    on every time slice."""
+    dims = (64, 32, 32, 32)
+    U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device)
+    fld = gf.GaugeField(dims, gauge=gf.GF_COULOMB, precisions=("f64",), seed=2013, device=cuda_device)
+    fld.pack(U, gf.GF_F64)
+    del U
+    P0 = fld.plaquette(gf.GF_F64)
+    rng = np.random.default_rng(5)
+    sampled_sweep_check(fld, dims, "f64", gf.GF_COULOMB, oracle.COULOMB, gf.GF_STOCHASTIC, oracle.STOCHASTIC,
+                        1.0, 0.8, 2013, 32, rng)
+    F1 = np.array(fld.functional(gf.GF_F64))
+    rc, it, th = fld.fix_until(gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64, 1e-12, 100000, 20)
+    assert rc == gf.GF_OK, (it, th)
+    thetas = np.array(fld.theta(gf.GF_F64))
+    assert thetas.shape == (64,) and thetas.max() < 1e-12 and thetas.max() == th
+    assert (np.array(fld.functional(gf.GF_F64)) > F1).all()        # every slice's functional rose
+    assert abs(fld.plaquette(gf.GF_F64) - P0) < 1e-12               # incl. temporal plaquettes: a gauge transformation
+    du, dd = fld.unitarity(gf.GF_F64)
+    assert du < 1e-12 and dd < 1e-12
+    print("config5: %d iterations, max theta_t = %.3e" % (it, th))
+    fld.close()
