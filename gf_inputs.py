@@ -127,6 +127,19 @@ def _torch_haar_su3(torch, gen, shape, device):
     return Q / phase[..., None, None]
 
 
+def _torch_polish_unitary(torch, U, slab=4):
+    """Two Newton-Schulz steps U <- U (3 - U^dagger U)/2, in place, slab by slab.  Classical
+    Gram-Schmidt on an ill-conditioned Gaussian draw leaves |UU^dagger - 1| ~ 1e-12 on the worst of
+    10^7 matrices; each step squares the defect, so the field ends at rounding level."""
+    eye3 = 3.0 * torch.eye(3, dtype=U.dtype, device=U.device)
+    for t0 in range(0, U.shape[0], slab):
+        W = U[t0:t0 + slab]
+        for _ in range(2):
+            W = 0.5 * (W @ (eye3 - W.mH @ W))
+        U[t0:t0 + slab] = W
+    return U
+
+
 def torch_smooth_random_gauge(dims, eps, seed, device="cuda", slab=4):
     import torch
     nt, nx, ny, nz = dims
@@ -148,11 +161,12 @@ def torch_smooth_random_gauge(dims, eps, seed, device="cuda", slab=4):
         g_fwd = torch.roll(g, -1, dims=AXIS_OF_MU[mu])
         U[..., mu, :, :] = g @ U[..., mu, :, :] @ g_fwd.mH
         del g_fwd
-    return U
+    del g
+    return _torch_polish_unitary(torch, U, slab)
 
 
 def torch_hot_links(dims, seed, device="cuda"):
     import torch
     gen = torch.Generator(device=device)
     gen.manual_seed(int(seed))
-    return _torch_haar_su3(torch, gen, field_shape(dims) + (4,), device).contiguous()
+    return _torch_polish_unitary(torch, _torch_haar_su3(torch, gen, field_shape(dims) + (4,), device).contiguous())

@@ -137,10 +137,9 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     G.div_ny = make_fastdiv(G.ny);
     G.div_nz = make_fastdiv(G.nz);
 
-    // defaults chosen by measurement on B200 at 32^4 ("Kernels"); gf_set_tuning overrides
-    c->lanes[PREC_F32] = 2;  c->block[PREC_F32] = 128;
-    c->lanes[PREC_F64] = 2;  c->block[PREC_F64] = 128;
-    if (recon == GF_RECON12) { c->lanes[PREC_F64] = 1;  c->block[PREC_F64] = 64; }
+    // 0 = automatic (default_tuning below); gf_set_tuning overrides
+    c->lanes[PREC_F32] = c->lanes[PREC_F64] = 0;
+    c->block[PREC_F32] = c->block[PREC_F64] = 0;
     c->solver_mode = GF_SOLVER_AUTO;
     c->zigzag = 1;
 
@@ -225,6 +224,19 @@ static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
     return GF_OK;
 }
 
+// Launch configuration chosen by measurement on B200 at 32^4 (profiles/r1_tune_32x32x32x32.txt,
+// DESIGN.md "Kernels"): two lanes per site everywhere except fp64 / 12-real (four).
+static void default_tuning(int precision, int recon, int solver_f64, int* lanes, int* block)
+{
+    if (precision == GF_F64) {
+        *lanes = recon == GF_RECON12 ? 4 : 2;
+        *block = recon == GF_RECON12 ? 64 : 128;
+    } else {
+        *lanes = 2;
+        *block = (recon == GF_RECON18 && !solver_f64) ? 128 : 64;
+    }
+}
+
 static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
 {
     SweepArgs a;
@@ -240,7 +252,11 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.counter = ctx->counter;
     a.reverse = ctx->zigzag ? (uint32_t)(ctx->sweeps & 1u) : 0u;
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
-    cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, ctx->lanes[precision], ctx->block[precision], a, ctx->stream);
+    int lanes, block;
+    default_tuning(precision, ctx->recon, solver_f64, &lanes, &block);
+    if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
+    if (ctx->block[precision]) block = ctx->block[precision];
+    cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, lanes, block, a, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_sweep launch");
     ctx->counter += 1;
     ctx->sweeps += 1;
@@ -474,11 +490,10 @@ extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int
 {
     if (!ctx) return GF_EINVAL;
     if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
-    const int lanes = lanes_per_site ? lanes_per_site : ctx->lanes[precision];
-    const int block = block_threads ? block_threads : ctx->block[precision];
-    if (!sweep_config_valid(lanes, block)) return fail(ctx, GF_EINVAL, "lanes must be 1,2,4 and block 64..512 (power of two)");
-    ctx->lanes[precision] = lanes;
-    ctx->block[precision] = block;
+    if (!sweep_config_valid(lanes_per_site ? lanes_per_site : 1, block_threads ? block_threads : 64))
+        return fail(ctx, GF_EINVAL, "lanes must be 0,1,2,4 and block 0 or 64..512 (power of two)");
+    ctx->lanes[precision] = lanes_per_site;
+    ctx->block[precision] = block_threads;
     return GF_OK;
 }
 
