@@ -181,6 +181,13 @@ __device__ __forceinline__ void reconstruct_row2(T (&m)[18])
     }
 }
 
+__device__ __forceinline__ float gf_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double gf_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
+
+// The products below are written as explicit fma chains (one multiply, then fused multiply-adds):
+// two instructions per complex multiply-accumulate term instead of the three (mul, fma, add) the
+// compiler emits for  re += a*b - c*d.
+
 // out = g U, rows 0..ROWS-1 only
 template <int ROWS, typename T>
 __device__ __forceinline__ void mul_g_U(const T (&g)[18], const T (&U)[18], T (&out)[18])
@@ -189,11 +196,16 @@ __device__ __forceinline__ void mul_g_U(const T (&g)[18], const T (&U)[18], T (&
     for (int a = 0; a < ROWS; ++a)
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            T re = T(0), im = T(0);
+            T re = GF_RE(g, a, 0) * GF_RE(U, 0, b);
+            T im = GF_RE(g, a, 0) * GF_IM(U, 0, b);
+            re = gf_fma(-GF_IM(g, a, 0), GF_IM(U, 0, b), re);
+            im = gf_fma(GF_IM(g, a, 0), GF_RE(U, 0, b), im);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                re += GF_RE(g, a, k) * GF_RE(U, k, b) - GF_IM(g, a, k) * GF_IM(U, k, b);
-                im += GF_RE(g, a, k) * GF_IM(U, k, b) + GF_IM(g, a, k) * GF_RE(U, k, b);
+            for (int k = 1; k < 3; ++k) {
+                re = gf_fma(GF_RE(g, a, k), GF_RE(U, k, b), re);
+                im = gf_fma(GF_RE(g, a, k), GF_IM(U, k, b), im);
+                re = gf_fma(-GF_IM(g, a, k), GF_IM(U, k, b), re);
+                im = gf_fma(GF_IM(g, a, k), GF_RE(U, k, b), im);
             }
             GF_RE(out, a, b) = re;
             GF_IM(out, a, b) = im;
@@ -208,11 +220,16 @@ __device__ __forceinline__ void mul_U_gdag(const T (&U)[18], const T (&g)[18], T
     for (int a = 0; a < ROWS; ++a)
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
-            T re = T(0), im = T(0);
+            T re = GF_RE(U, a, 0) * GF_RE(g, b, 0);
+            T im = GF_IM(U, a, 0) * GF_RE(g, b, 0);
+            re = gf_fma(GF_IM(U, a, 0), GF_IM(g, b, 0), re);
+            im = gf_fma(-GF_RE(U, a, 0), GF_IM(g, b, 0), im);
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                re += GF_RE(U, a, k) * GF_RE(g, b, k) + GF_IM(U, a, k) * GF_IM(g, b, k);
-                im += GF_IM(U, a, k) * GF_RE(g, b, k) - GF_RE(U, a, k) * GF_IM(g, b, k);
+            for (int k = 1; k < 3; ++k) {
+                re = gf_fma(GF_RE(U, a, k), GF_RE(g, b, k), re);
+                im = gf_fma(GF_IM(U, a, k), GF_RE(g, b, k), im);
+                re = gf_fma(GF_IM(U, a, k), GF_IM(g, b, k), re);
+                im = gf_fma(-GF_RE(U, a, k), GF_IM(g, b, k), im);
             }
             GF_RE(out, a, b) = re;
             GF_IM(out, a, b) = im;
@@ -231,16 +248,17 @@ enum { ALGO_RELAX = 0, ALGO_OVERRELAX = 1, ALGO_STOCHASTIC = 2 };
 //   v = (Re(K_II + K_JJ), -Im(K_IJ + K_JI), Re(K_JI - K_IJ), Im(K_JJ - K_II)),
 // so eq. 9 gives a = v/|v|.  Overrelaxation (first order):
 // a -> normalise(1 + omega (a - 1)) = normalise(omega v + (1 - omega)|v| e0).  Stochastic
-// relaxation: a -> a^2 when `square`.  Then K <- E K and g <- E g.
+// relaxation: a -> a^2 when `square`.
 template <int I, int J, typename T>
-__device__ __forceinline__ void su2_step(T (&K)[18], T (&g)[18], int algo, T omega, bool square)
+__device__ __forceinline__ void su2_vector(const T (&K)[18], int algo, T omega, bool square, T (&a)[4])
 {
     T v0 = GF_RE(K, I, I) + GF_RE(K, J, J);
     T v1 = -(GF_IM(K, I, J) + GF_IM(K, J, I));
     T v2 = GF_RE(K, J, I) - GF_RE(K, I, J);
     T v3 = GF_IM(K, J, J) - GF_IM(K, I, I);
     T nn = v0 * v0 + v1 * v1 + v2 * v2 + v3 * v3;
-    T a0 = T(1), a1 = T(0), a2 = T(0), a3 = T(0);
+    a[0] = T(1);
+    a[1] = a[2] = a[3] = T(0);
     if (nn > T(0)) {
         T rn = gf_rsqrt(nn);
         if (algo == ALGO_OVERRELAX) {
@@ -252,36 +270,94 @@ __device__ __forceinline__ void su2_step(T (&K)[18], T (&g)[18], int algo, T ome
             nn = v0 * v0 + v1 * v1 + v2 * v2 + v3 * v3;
             rn = gf_rsqrt(nn);
         }
-        a0 = v0 * rn;
-        a1 = v1 * rn;
-        a2 = v2 * rn;
-        a3 = v3 * rn;
+        a[0] = v0 * rn;
+        a[1] = v1 * rn;
+        a[2] = v2 * rn;
+        a[3] = v3 * rn;
         if (square) {
-            const T t = a0 + a0;
-            a0 = t * a0 - T(1);
-            a1 *= t;
-            a2 *= t;
-            a3 *= t;
+            const T t = a[0] + a[0];
+            a[0] = t * a[0] - T(1);
+            a[1] *= t;
+            a[2] *= t;
+            a[3] *= t;
         }
     }
-    // E_II = a0 + i a3, E_IJ = a2 + i a1, E_JI = -a2 + i a1, E_JJ = a0 - i a3
+}
+
+// K <- E K with E the embedding of a in the subgroup (I,J):
+// E_II = a0 + i a3, E_IJ = a2 + i a1, E_JI = -a2 + i a1, E_JJ = a0 - i a3
+template <int I, int J, typename T>
+__device__ __forceinline__ void su2_apply(T (&K)[18], const T (&a)[4])
+{
 #pragma unroll
     for (int b = 0; b < 3; ++b) {
-        {
-            const T ir = GF_RE(K, I, b), ii = GF_IM(K, I, b), jr = GF_RE(K, J, b), ji = GF_IM(K, J, b);
-            GF_RE(K, I, b) = a0 * ir - a3 * ii + a2 * jr - a1 * ji;
-            GF_IM(K, I, b) = a0 * ii + a3 * ir + a2 * ji + a1 * jr;
-            GF_RE(K, J, b) = -a2 * ir - a1 * ii + a0 * jr + a3 * ji;
-            GF_IM(K, J, b) = -a2 * ii + a1 * ir + a0 * ji - a3 * jr;
-        }
-        {
-            const T ir = GF_RE(g, I, b), ii = GF_IM(g, I, b), jr = GF_RE(g, J, b), ji = GF_IM(g, J, b);
-            GF_RE(g, I, b) = a0 * ir - a3 * ii + a2 * jr - a1 * ji;
-            GF_IM(g, I, b) = a0 * ii + a3 * ir + a2 * ji + a1 * jr;
-            GF_RE(g, J, b) = -a2 * ir - a1 * ii + a0 * jr + a3 * ji;
-            GF_IM(g, J, b) = -a2 * ii + a1 * ir + a0 * ji - a3 * jr;
-        }
+        const T ir = GF_RE(K, I, b), ii = GF_IM(K, I, b), jr = GF_RE(K, J, b), ji = GF_IM(K, J, b);
+        GF_RE(K, I, b) = a[0] * ir - a[3] * ii + a[2] * jr - a[1] * ji;
+        GF_IM(K, I, b) = a[0] * ii + a[3] * ir + a[2] * ji + a[1] * jr;
+        GF_RE(K, J, b) = -a[2] * ir - a[1] * ii + a[0] * jr + a[3] * ji;
+        GF_IM(K, J, b) = -a[2] * ii + a[1] * ir + a[0] * ji - a[3] * jr;
     }
+}
+
+// (xr + i xi) (yr + i yi)
+template <typename T>
+__device__ __forceinline__ void cmul(T xr, T xi, T yr, T yi, T& zr, T& zi)
+{
+    zr = gf_fma(-xi, yi, xr * yr);
+    zi = gf_fma(xi, yr, xr * yi);
+}
+
+// z += (xr + i xi) (yr + i yi)
+template <typename T>
+__device__ __forceinline__ void cmac(T xr, T xi, T yr, T yi, T& zr, T& zi)
+{
+    zr = gf_fma(-xi, yi, gf_fma(xr, yr, zr));
+    zi = gf_fma(xi, yr, gf_fma(xr, yi, zi));
+}
+
+// g = E3 E2 E1 for the subgroups (0,1), (0,2), (1,2) with SU(2) vectors a, b, c, multiplied out
+// using the zeros of the factors (56 instead of 144 fused multiply-adds for three dense updates
+// of a matrix that starts as the identity).
+template <typename T>
+__device__ __forceinline__ void compose_g(const T (&a)[4], const T (&b)[4], const T (&c)[4], T (&g)[18])
+{
+    // after E1: row0 = (p, q, 0), row1 = (r, s, 0), row2 = (0, 0, 1)
+    const T pr = a[0], pi = a[3], qr = a[2], qi = a[1], rr = -a[2], ri = a[1], sr = a[0], si = -a[3];
+    // E2 on rows (0,2): row0' = P row0 + Q row2 = (P p, P q, Q);  row2' = R row0 + S row2 = (R p, R q, S)
+    const T Pr = b[0], Pi = b[3], Qr = b[2], Qi = b[1], Rr = -b[2], Ri = b[1], Sr = b[0], Si = -b[3];
+    cmul(Pr, Pi, pr, pi, GF_RE(g, 0, 0), GF_IM(g, 0, 0));
+    cmul(Pr, Pi, qr, qi, GF_RE(g, 0, 1), GF_IM(g, 0, 1));
+    GF_RE(g, 0, 2) = Qr;
+    GF_IM(g, 0, 2) = Qi;
+    T x0r, x0i, x1r, x1i;            // row2' entries 0, 1 (entry 2 is S)
+    cmul(Rr, Ri, pr, pi, x0r, x0i);
+    cmul(Rr, Ri, qr, qi, x1r, x1i);
+    // E3 on rows (1,2): row1'' = P3 row1 + Q3 row2';  row2'' = R3 row1 + S3 row2'
+    const T P3r = c[0], P3i = c[3], Q3r = c[2], Q3i = c[1], R3r = -c[2], R3i = c[1], S3r = c[0], S3i = -c[3];
+    cmul(P3r, P3i, rr, ri, GF_RE(g, 1, 0), GF_IM(g, 1, 0));
+    cmac(Q3r, Q3i, x0r, x0i, GF_RE(g, 1, 0), GF_IM(g, 1, 0));
+    cmul(P3r, P3i, sr, si, GF_RE(g, 1, 1), GF_IM(g, 1, 1));
+    cmac(Q3r, Q3i, x1r, x1i, GF_RE(g, 1, 1), GF_IM(g, 1, 1));
+    cmul(Q3r, Q3i, Sr, Si, GF_RE(g, 1, 2), GF_IM(g, 1, 2));
+    cmul(R3r, R3i, rr, ri, GF_RE(g, 2, 0), GF_IM(g, 2, 0));
+    cmac(S3r, S3i, x0r, x0i, GF_RE(g, 2, 0), GF_IM(g, 2, 0));
+    cmul(R3r, R3i, sr, si, GF_RE(g, 2, 1), GF_IM(g, 2, 1));
+    cmac(S3r, S3i, x1r, x1i, GF_RE(g, 2, 1), GF_IM(g, 2, 1));
+    cmul(S3r, S3i, Sr, Si, GF_RE(g, 2, 2), GF_IM(g, 2, 2));
+}
+
+// a4: the local maximiser g(x) = E3 E2 E1 of Re tr[g K] over the three SU(2) subgroups in the
+// order (0,1), (0,2), (1,2), K refreshed between the steps.  K is destroyed.
+template <typename T>
+__device__ __forceinline__ void solve_site(T (&K)[18], int algo, T omega, bool sq0, bool sq1, bool sq2, T (&g)[18])
+{
+    T a[4], b[4], c[4];
+    su2_vector<0, 1>(K, algo, omega, sq0, a);
+    su2_apply<0, 1>(K, a);
+    su2_vector<0, 2>(K, algo, omega, sq1, b);
+    su2_apply<0, 2>(K, b);
+    su2_vector<1, 2>(K, algo, omega, sq2, c);
+    compose_g(a, b, c, g);
 }
 
 // --------------------------------------------------------------------------- Philox4x32-10

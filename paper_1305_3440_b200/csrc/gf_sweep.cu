@@ -110,12 +110,7 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
 
     // a4: the three SU(2) subgroups, g = E3 E2 E1
     TK gk[18];
-#pragma unroll
-    for (int k = 0; k < 18; ++k) gk[k] = TK(0);
-    gk[0] = gk[8] = gk[16] = TK(1);
-    su2_step<0, 1>(K, gk, P.algo, P.omega, sq0);
-    su2_step<0, 2>(K, gk, P.algo, P.omega, sq1);
-    su2_step<1, 2>(K, gk, P.algo, P.omega, sq2);
+    solve_site(K, P.algo, P.omega, sq0, sq1, sq2, gk);
     T g[18];
 #pragma unroll
     for (int k = 0; k < 18; ++k) g[k] = (T)gk[k];
