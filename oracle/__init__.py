@@ -46,6 +46,9 @@ def load():
     lib.oracle_sweep_ordered.argtypes = [cd_p, i4, C.c_int, C.c_int, C.c_int, C.c_double,
                                          C.c_double, C.c_uint64, C.c_uint32, C.c_int]
     lib.oracle_sweep.argtypes = lib.oracle_sweep_ordered.argtypes[:-1]
+    lib.oracle_sweep_accumulate.argtypes = [cd_p, cd_p, i4, C.c_int, C.c_int, C.c_int, C.c_double,
+                                            C.c_double, C.c_uint64, C.c_uint32]
+    lib.oracle_apply_transform.argtypes = [cd_p, cd_p, i4, cd_p]
     lib.oracle_fix_until.argtypes = [cd_p, i4, C.c_int, C.c_int, C.c_double, C.c_double,
                                      C.c_uint64, C.c_uint32, C.c_double, C.c_int, C.c_int,
                                      dbl_p, C.POINTER(C.c_int)]
@@ -166,6 +169,34 @@ def sweep(U, dims, parity, gauge=LANDAU, algo=OVERRELAX, omega=1.0, p=0.0, seed=
           half_sweep_counter=0, reverse_order=False):
     load().oracle_sweep_ordered(_field(U, dims), _dims(dims), gauge, parity, algo, omega, p,
                                 int(seed), int(half_sweep_counter), int(bool(reverse_order)))
+
+
+def _transform(G, dims):
+    nt, nx, ny, nz = dims
+    assert isinstance(G, np.ndarray) and G.dtype == np.complex128 and G.flags.c_contiguous
+    assert G.shape == (nt, nz, ny, nx, 3, 3), (G.shape, dims)
+    return G.ctypes.data_as(C.c_void_p)
+
+
+def identity_transform(dims):
+    nt, nx, ny, nz = dims
+    G = np.zeros((nt, nz, ny, nx, 3, 3), np.complex128)
+    G[..., 0, 0] = G[..., 1, 1] = G[..., 2, 2] = 1.0
+    return G
+
+
+def sweep_accumulate(U, G, dims, parity, gauge=LANDAU, algo=OVERRELAX, omega=1.0, p=0.0, seed=0,
+                     half_sweep_counter=0):
+    """The half-sweep of ``sweep`` that also records Gtot(x) <- g(x) Gtot(x); U and G in place."""
+    load().oracle_sweep_accumulate(_field(U, dims), _transform(G, dims), _dims(dims), gauge, parity,
+                                   algo, omega, p, int(seed), int(half_sweep_counter))
+
+
+def apply_transform(U, G, dims):
+    """Returns G(x) U_mu(x) G(x+mu)^dagger (eq. 3) as a new array."""
+    out = np.empty_like(U)
+    load().oracle_apply_transform(_field(U, dims), _transform(G, dims), _dims(dims), _field(out, dims))
+    return out
 
 
 def fix_until(U, dims, gauge=LANDAU, algo=OVERRELAX, omega=1.0, p=0.0, seed=0, first_counter=0,

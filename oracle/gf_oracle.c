@@ -378,7 +378,10 @@ void oracle_update_links8(cd fwd[4][9], cd bwd[4][9], int gauge, int algo,
     update_site(f, b, gauge, algo, omega, p, u, g_out);
 }
 
-static void visit_site(cd *U, const int dims[4], int gauge, int parity, int algo,
+/* Gtot (may be NULL): the accumulated transformation, one 3x3 matrix per site,
+ * Gtot[s][a][b].  A site visit applies g(x) on top of what was applied before,
+ * so by PAPER.md:43 (eq. 3) the total transformation becomes g(x) Gtot(x). */
+static void visit_site(cd *U, cd *Gtot, const int dims[4], int gauge, int parity, int algo,
                        double omega, double p, uint64_t seed, uint32_t half_sweep_counter, size_t s)
 {
     int c[4];
@@ -391,27 +394,64 @@ static void visit_site(cd *U, const int dims[4], int gauge, int parity, int algo
     }
     double u[3] = { 0.0, 0.0, 0.0 };
     if (algo == ORACLE_STOCHASTIC) oracle_site_uniforms(seed, half_sweep_counter, (uint64_t)s, u);
-    update_site(fwd, bwd, gauge, algo, omega, p, u, NULL);
+    cd g[9], tmp[9];
+    update_site(fwd, bwd, gauge, algo, omega, p, u, g);
+    if (Gtot) {
+        mat_mul(g, Gtot + s * 9, tmp);
+        for (int k = 0; k < 9; ++k) Gtot[s * 9 + k] = tmp[k];
+    }
 }
 
 /* all sites of one parity subset can be optimised at the same
  * time; the sites are visited in lexicographic order (reverse_order != 0: in
  * the opposite order -- same-parity sites share no link, so the result must be
  * bitwise the same; that is one of the pins). */
-void oracle_sweep_ordered(cd *U, const int dims[4], int gauge, int parity, int algo, double omega,
-                          double p, uint64_t seed, uint32_t half_sweep_counter, int reverse_order)
+static void sweep_impl(cd *U, cd *Gtot, const int dims[4], int gauge, int parity, int algo, double omega,
+                       double p, uint64_t seed, uint32_t half_sweep_counter, int reverse_order)
 {
     const size_t V = volume(dims);
     if (reverse_order) {
         for (size_t k = V; k-- > 0;)
-            visit_site(U, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, k);
+            visit_site(U, Gtot, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, k);
         return;
     }
 #ifdef _OPENMP
 #pragma omp parallel for num_threads(g_threads) schedule(static)
 #endif
     for (size_t s = 0; s < V; ++s)
-        visit_site(U, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, s);
+        visit_site(U, Gtot, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, s);
+}
+
+void oracle_sweep_ordered(cd *U, const int dims[4], int gauge, int parity, int algo, double omega,
+                          double p, uint64_t seed, uint32_t half_sweep_counter, int reverse_order)
+{
+    sweep_impl(U, NULL, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, reverse_order);
+}
+
+/* The same half-sweep, also recording the transformation: Gtot(x) <- g(x) Gtot(x)
+ * on the visited sites.  Starting from Gtot = 1 the swept links always equal
+ * Gtot(x) U^(0)_mu(x) Gtot(x + mu_hat)^dagger of the initial links U^(0) (eq. 3);
+ * that identity is one of the pins. */
+void oracle_sweep_accumulate(cd *U, cd *Gtot, const int dims[4], int gauge, int parity, int algo,
+                             double omega, double p, uint64_t seed, uint32_t half_sweep_counter)
+{
+    sweep_impl(U, Gtot, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, 0);
+}
+
+/* PAPER.md:43 (eq. 3) written out: U_out_mu(x) = G(x) U_mu(x) G(x + mu_hat)^dagger. */
+void oracle_apply_transform(const cd *U, const cd *G, const int dims[4], cd *U_out)
+{
+    const size_t V = volume(dims);
+    for (size_t s = 0; s < V; ++s) {
+        int c[4];
+        site_coords(dims, s, c);
+        for (int mu = 0; mu < 4; ++mu) {
+            cd gd[9], tmp[9];
+            mat_dagger(G + neighbour(dims, c, mu, +1) * 9, gd);
+            mat_mul(G + s * 9, link_cptr(U, s, mu), tmp);
+            mat_mul(tmp, gd, U_out + (s * 4 + (size_t)mu) * 9);
+        }
+    }
 }
 
 void oracle_sweep(cd *U, const int dims[4], int gauge, int parity, int algo, double omega,

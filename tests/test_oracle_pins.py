@@ -427,3 +427,50 @@ def test_coulomb_slices_are_decoupled():
             oracle.sweep(W, dims, parity, oracle.COULOMB, oracle.OVERRELAX, 1.6)
     assert np.array_equal(U[1, ..., 1:, :, :], W[1, ..., 1:, :, :])     # spatial links of slice 1
     assert not np.allclose(U[3], W[3])
+
+
+# ----------------------------------------- the accumulated transformation (eq. 3)
+
+def test_apply_transform_is_eq3_and_a_gauge_transformation():
+    """oracle.apply_transform (C loops) against the input generator's independent numpy statement of
+    eq. 3; identity and composition laws; the plaquette does not see it."""
+    dims = (4, 6, 4, 8)
+    U = gi.smooth_random_gauge(dims, 0.4, 3)
+    G = gi.random_gauge(dims, 11)
+    out = oracle.apply_transform(U, G, dims)
+    assert np.abs(out - gi.gauge_transform(U, G)).max() < 1e-14
+    assert np.array_equal(oracle.apply_transform(U, oracle.identity_transform(dims), dims), U)
+    H = gi.random_gauge(dims, 12)
+    HG = np.ascontiguousarray(np.einsum("...ab,...bc->...ac", H, G))
+    assert np.abs(oracle.apply_transform(out, H, dims) - oracle.apply_transform(U, HG, dims)).max() < 1e-14
+    assert abs(oracle.plaquette(out, dims) - oracle.plaquette(U, dims)) < 1e-14
+    # a transposed or un-daggered neighbour matrix would break both
+    x = (1, 2, 3, 4)          # (t, z, y, x)
+    xp = (1, 2, 3, 5)         # x + x_hat
+    assert np.abs(out[x][1] - G[x] @ U[x][1] @ G[xp].conj().T).max() < 1e-14
+
+
+@pytest.mark.parametrize("gauge,algo", [(oracle.LANDAU, oracle.OVERRELAX), (oracle.COULOMB, oracle.STOCHASTIC)])
+def test_accumulated_transformation_reproduces_the_swept_links(gauge, algo):
+    """Gtot(x) <- g(x) Gtot(x): after any number of half-sweeps the links are
+    Gtot(x) U0_mu(x) Gtot(x+mu)^dagger of the initial links (eq. 3), Gtot stays in SU(3), and the
+    links are bitwise those of the plain sweep."""
+    dims = (4, 4, 6, 4)
+    U0 = gi.smooth_random_gauge(dims, 0.5, 21)
+    U, Uplain = U0.copy(), U0.copy()
+    G = oracle.identity_transform(dims)
+    for it in range(3):
+        for parity in (0, 1):
+            kw = dict(gauge=gauge, algo=algo, omega=1.7, p=0.7, seed=5, half_sweep_counter=2 * it + parity)
+            oracle.sweep_accumulate(U, G, dims, parity, **kw)
+            oracle.sweep(Uplain, dims, parity, **kw)
+            if it == 0 and parity == 0:
+                # only the visited parity has moved away from the identity
+                par = np.indices(G.shape[:4]).sum(axis=0) % 2
+                assert np.all(G[par == 1] == np.eye(3))
+                assert np.abs(G[par == 0] - np.eye(3)).max() > 1e-3
+    assert np.array_equal(U, Uplain)
+    assert np.abs(oracle.apply_transform(U0, G, dims) - U).max() < 1e-13
+    GG = np.einsum("...ab,...cb->...ac", G, G.conj())
+    assert np.abs(GG - np.eye(3)).max() < 1e-13
+    assert np.abs(np.linalg.det(G) - 1).max() < 1e-13
