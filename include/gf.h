@@ -47,7 +47,7 @@ typedef struct gf_ctx gf_ctx; /* opaque; owned by the library; freed by gf_destr
 
 enum { GF_OK = 0, GF_NOT_CONVERGED = 1, GF_EINVAL = -1, GF_ENOMEM = -2, GF_ECUDA = -3, GF_ESTATE = -4 };
 enum { GF_LANDAU = 0, GF_COULOMB = 1 };                   /* gauge */
-enum { GF_F32 = 0, GF_F64 = 1, GF_MIXED = 2 };            /* precision */
+enum { GF_F32 = 0, GF_F64 = 1, GF_MIXED = 2, GF_MIXED_EXACT = 3 }; /* precision */
 enum { GF_RELAX = 0, GF_OVERRELAX = 1, GF_STOCHASTIC = 2 }; /* algo: PAPER.md:73, :80, :84 */
 enum { GF_RECON18 = 18, GF_RECON12 = 12 };                /* reals stored per link */
 
@@ -113,10 +113,46 @@ int gf_measure(gf_ctx* ctx, int precision, double* host_functional, double* host
  * max over slices) and stops when it is below theta_target.  precision GF_MIXED: fp32
  * iterations until theta < max(theta_target, 1e-6), then gf_cast fp32->fp64 (with SU(3)
  * re-projection) and fp64 iterations; the fp32 field must hold the input and the result is in
- * the fp64 field.  *iters_out = iterations done (both phases), *theta_out = last theta.
+ * the fp64 field.  precision GF_MIXED_EXACT (needs both link fields and both transformation
+ * buffers): the fp64 field holds the input and is not rounded; it is copied to fp32, fp32
+ * iterations record G(x) from the identity until theta < max(theta_target, 1e-6), then the
+ * untouched fp64 input is transformed by the re-projected G (gf_transform_cast +
+ * gf_apply_transform), and fp64 iterations continue, accumulating into the fp64 transformation:
+ * the result equals G(x) U_mu(x) G(x+mu)^dagger of the input to fp64 accuracy and G is returned
+ * in the fp64 transformation buffer.  *iters_out = iterations done (both phases), *theta_out = last theta.
  * Returns GF_OK, or GF_NOT_CONVERGED (valid outputs) when max_iter was reached.  Synchronises. */
 int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int precision, double theta_target,
                  int max_iter, int check_every, int* iters_out, double* theta_out);
+
+/* ---- The accumulated gauge transformation G(x) (eq. 3).
+ * A relaxation sweep replaces the links by g(x) U_mu(x) g(x+mu)^dagger site after site; the
+ * product of all g(x) applied to a site so far, G(x), is what a user needs to transform other
+ * fields, and what lets a low-precision run be replayed on the untouched input.
+ *
+ * gf_transform_bytes: device bytes of one transformation field (one 3x3 matrix per site, stored
+ * like a link with `recon` reals) = gf_storage_bytes / 4.
+ * gf_set_transform: lends the context one buffer per precision (either may be NULL; both NULL
+ * detaches).  While a buffer for precision P is attached, every gf_sweep / gf_fix_until sweep of
+ * precision P also does G(x) <- g(x) G(x) on the sites it visits (one more matrix read and
+ * written per site-update: +12.5 % memory traffic).  Attaching does not initialise the buffer.
+ * gf_transform_identity: G(x) = 1.  gf_transform_pack / gf_transform_unpack: canonical (device)
+ * <-> internal; canonical = contiguous complex array (N_t, N_z, N_y, N_x, 3, 3), complex128 or
+ * complex64.  gf_transform_cast: copies G between the precisions; fp32 -> fp64 re-projects every
+ * matrix onto SU(3) (Gram-Schmidt) in fp64.  All asynchronous on the context's stream.
+ * Errors: GF_EINVAL (alignment, enum, null pointer), GF_ESTATE (no buffer for that precision). */
+size_t gf_transform_bytes(const int dims[4], int precision, int recon);
+int gf_set_transform(gf_ctx* ctx, void* dev_g_f64, void* dev_g_f32);
+int gf_transform_identity(gf_ctx* ctx, int precision);
+int gf_transform_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision);
+int gf_transform_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision);
+int gf_transform_cast(gf_ctx* ctx, int from_precision, int to_precision);
+
+/* Link field of dst_precision <- G(x) U_mu(x) G(x+mu)^dagger of the link field of src_precision
+ * (eq. 3), with G the transformation of g_precision.  The products are formed in fp64 whatever
+ * the storage; an fp32 G is re-projected onto SU(3) in fp64 first, so the result is gauge
+ * equivalent to the source to fp64 accuracy.  src_precision == dst_precision works in place.
+ * Asynchronous.  Errors as above. */
+int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precision, int dst_precision);
 
 /* Sets the Philox key and the half-sweep counter (checkpoint/resume: the RNG state is just these). */
 int gf_set_rng(gf_ctx* ctx, uint64_t seed, uint32_t half_sweep_counter);

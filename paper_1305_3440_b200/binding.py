@@ -10,7 +10,7 @@ import os
 GF_OK, GF_NOT_CONVERGED = 0, 1
 GF_EINVAL, GF_ENOMEM, GF_ECUDA, GF_ESTATE = -1, -2, -3, -4
 GF_LANDAU, GF_COULOMB = 0, 1
-GF_F32, GF_F64, GF_MIXED = 0, 1, 2
+GF_F32, GF_F64, GF_MIXED, GF_MIXED_EXACT = 0, 1, 2, 3
 GF_RELAX, GF_OVERRELAX, GF_STOCHASTIC = 0, 1, 2
 GF_RECON18, GF_RECON12 = 18, 12
 GF_SOLVER_AUTO = -1
@@ -46,6 +46,13 @@ def _load():
         "gf_theta": (i32, [vp, i32, dp]),
         "gf_measure": (i32, [vp, i32, dp, dp]),
         "gf_fix_until": (i32, [vp, i32, dbl, dbl, i32, dbl, i32, i32, ip, dp]),
+        "gf_transform_bytes": (C.c_size_t, [ip, i32, i32]),
+        "gf_set_transform": (i32, [vp, vp, vp]),
+        "gf_transform_identity": (i32, [vp, i32]),
+        "gf_transform_pack": (i32, [vp, vp, i32, i32]),
+        "gf_transform_unpack": (i32, [vp, vp, i32, i32]),
+        "gf_transform_cast": (i32, [vp, i32, i32]),
+        "gf_apply_transform": (i32, [vp, i32, i32, i32]),
         "gf_set_rng": (i32, [vp, u64, u32]),
         "gf_get_counter": (i32, [vp, C.POINTER(u32)]),
         "gf_reunitarize": (i32, [vp, i32]),
@@ -69,7 +76,8 @@ def _load():
 lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
            "gf_sweep gf_functional gf_theta gf_measure gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
-           "gf_cast gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_debug_philox gf_launch_count gf_last_error "
+           "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
+           "gf_transform_cast gf_apply_transform gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
 
 
@@ -183,6 +191,34 @@ def gf_reunitarize(ctx, precision, check=True):
 
 def gf_cast(ctx, from_precision, to_precision, check=True):
     return _rc(ctx, lib.gf_cast(ctx, from_precision, to_precision), check)
+
+
+def gf_transform_bytes(dims, precision, recon):
+    return lib.gf_transform_bytes(_dims(dims), precision, recon)
+
+
+def gf_set_transform(ctx, dev_g_f64, dev_g_f32, check=True):
+    return _rc(ctx, lib.gf_set_transform(ctx, dev_g_f64 or None, dev_g_f32 or None), check)
+
+
+def gf_transform_identity(ctx, precision, check=True):
+    return _rc(ctx, lib.gf_transform_identity(ctx, precision), check)
+
+
+def gf_transform_pack(ctx, dev_canonical, canonical_is_f64, precision, check=True):
+    return _rc(ctx, lib.gf_transform_pack(ctx, dev_canonical, int(canonical_is_f64), precision), check)
+
+
+def gf_transform_unpack(ctx, dev_canonical, canonical_is_f64, precision, check=True):
+    return _rc(ctx, lib.gf_transform_unpack(ctx, dev_canonical, int(canonical_is_f64), precision), check)
+
+
+def gf_transform_cast(ctx, from_precision, to_precision, check=True):
+    return _rc(ctx, lib.gf_transform_cast(ctx, from_precision, to_precision), check)
+
+
+def gf_apply_transform(ctx, g_precision, src_precision, dst_precision, check=True):
+    return _rc(ctx, lib.gf_apply_transform(ctx, g_precision, src_precision, dst_precision), check)
 
 
 def gf_plaquette(ctx, precision, check=True):

@@ -20,6 +20,7 @@ struct gf_ctx {
     int dims[4];
     int gauge, recon;
     void* links[2];             // [PREC_F32], [PREC_F64]
+    void* gtrans[2];            // accumulated transformation per precision (gf_set_transform), or NULL
     double* workspace;
     double* partials;           // workspace: per-block partial sums
     double* slice_out;          // workspace: 2 doubles per time slice
@@ -79,6 +80,11 @@ extern "C" size_t gf_storage_bytes(const int dims[4], int precision, int recon)
     if (!dims_ok(dims) || (precision != GF_F32 && precision != GF_F64) || (recon != 18 && recon != 12)) return 0;
     const size_t V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
     return V * 4 * (size_t)recon * (precision == GF_F64 ? 8 : 4);
+}
+
+extern "C" size_t gf_transform_bytes(const int dims[4], int precision, int recon)
+{
+    return gf_storage_bytes(dims, precision, recon) / 4;      // one matrix per site, links have four
 }
 
 extern "C" size_t gf_workspace_bytes(const int dims[4])
@@ -241,6 +247,7 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
 {
     SweepArgs a;
     a.links = ctx->links[precision];
+    a.gtrans = ctx->gtrans[precision];
     a.G = ctx->G;
     a.parity = (uint32_t)parity;
     a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
@@ -367,10 +374,13 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
                             int max_iter, int check_every, int* iters_out, double* theta_out)
 {
     if (!ctx) return GF_EINVAL;
-    if (precision != GF_F32 && precision != GF_F64 && precision != GF_MIXED) return fail(ctx, GF_EINVAL, "bad precision");
-    if (precision == GF_MIXED && (!ctx->links[PREC_F32] || !ctx->links[PREC_F64]))
-        return fail(ctx, GF_ESTATE, "GF_MIXED needs both fp32 and fp64 storage");
-    if (precision != GF_MIXED && !ctx->links[precision]) return fail(ctx, GF_ESTATE, "no link storage for precision %d", precision);
+    const bool mixed = precision == GF_MIXED || precision == GF_MIXED_EXACT;
+    if (precision != GF_F32 && precision != GF_F64 && !mixed) return fail(ctx, GF_EINVAL, "bad precision");
+    if (mixed && (!ctx->links[PREC_F32] || !ctx->links[PREC_F64]))
+        return fail(ctx, GF_ESTATE, "GF_MIXED / GF_MIXED_EXACT need both fp32 and fp64 storage");
+    if (precision == GF_MIXED_EXACT && (!ctx->gtrans[PREC_F32] || !ctx->gtrans[PREC_F64]))
+        return fail(ctx, GF_ESTATE, "GF_MIXED_EXACT needs both transformation buffers (gf_set_transform)");
+    if (!mixed && !ctx->links[precision]) return fail(ctx, GF_ESTATE, "no link storage for precision %d", precision);
     int rc = check_algo(ctx, algo, omega, p);
     if (rc) return rc;
     if (max_iter < 0 || check_every < 1 || !(theta_target >= 0.0)) return fail(ctx, GF_EINVAL, "bad max_iter / check_every / theta_target");
@@ -388,6 +398,26 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
             e = measure_to_host(ctx, GF_F64);
             if (e != GF_OK) return e;
             theta = finish_measure(ctx, nullptr, nullptr);
+        }
+    } else if (precision == GF_MIXED_EXACT) {
+        // fp32 sweeps on a copy, recording G(x); then the untouched fp64 input is transformed by the
+        // re-projected G (gauge equivalent to the input at fp64 accuracy) and the fp64 phase goes on
+        // accumulating into the fp64 transformation.
+        int e = gf_cast(ctx, GF_F64, GF_F32);
+        if (e == GF_OK) e = gf_transform_identity(ctx, GF_F32);
+        if (e != GF_OK) return e;
+        const double t32 = theta_target > 1e-6 ? theta_target : 1e-6;
+        rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta);
+        if (rc < 0) return rc;
+        e = gf_transform_cast(ctx, GF_F32, GF_F64);
+        if (e == GF_OK) e = gf_apply_transform(ctx, GF_F64, GF_F64, GF_F64);
+        if (e != GF_OK) return e;
+        if (rc == GF_OK && !(theta < theta_target)) rc = fix_phase(ctx, algo, omega, p, GF_F64, theta_target, max_iter, check_every, &it, &theta);
+        else {
+            e = measure_to_host(ctx, GF_F64);
+            if (e != GF_OK) return e;
+            theta = finish_measure(ctx, nullptr, nullptr);
+            if (rc == GF_OK && !(theta < theta_target)) rc = GF_NOT_CONVERGED;
         }
     } else {
         if (max_iter == 0) {
@@ -424,7 +454,7 @@ extern "C" int gf_reunitarize(gf_ctx* ctx, int precision)
 {
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
-    cudaError_t e = launch_cast(precision, precision, ctx->recon, ctx->links[precision], ctx->links[precision], ctx->G, 1, ctx->stream);
+    cudaError_t e = launch_cast(precision, precision, ctx->recon, ctx->links[precision], ctx->links[precision], ctx->G, 1, 8, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_reunitarize");
     ctx->launches += 1;
     return GF_OK;
@@ -439,8 +469,88 @@ extern "C" int gf_cast(gf_ctx* ctx, int from_precision, int to_precision)
     if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_cast needs two different precisions");
     const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
     cudaError_t e = launch_cast(from_precision, to_precision, ctx->recon, ctx->links[from_precision], ctx->links[to_precision],
-                                ctx->G, reproject, ctx->stream);
+                                ctx->G, reproject, 8, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_cast");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+// ---------------------------------------------------------- the accumulated transformation
+extern "C" int gf_set_transform(gf_ctx* ctx, void* dev_g_f64, void* dev_g_f32)
+{
+    if (!ctx) return GF_EINVAL;
+    if (((uintptr_t)dev_g_f64 | (uintptr_t)dev_g_f32) & 15u) return fail(ctx, GF_EINVAL, "transformation buffers must be 16-byte aligned");
+    ctx->gtrans[PREC_F64] = dev_g_f64;
+    ctx->gtrans[PREC_F32] = dev_g_f32;
+    return GF_OK;
+}
+
+static int check_transform(gf_ctx* ctx, int precision)
+{
+    if (!ctx) return GF_EINVAL;
+    if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
+    if (!ctx->gtrans[precision]) return fail(ctx, GF_ESTATE, "no transformation buffer for precision %d (gf_set_transform)", precision);
+    return GF_OK;
+}
+
+extern "C" int gf_transform_identity(gf_ctx* ctx, int precision)
+{
+    int rc = check_transform(ctx, precision);
+    if (rc) return rc;
+    cudaError_t e = launch_transform_identity(precision, ctx->recon, ctx->gtrans[precision], ctx->G, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_identity");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_transform_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision)
+{
+    int rc = check_transform(ctx, precision);
+    if (rc) return rc;
+    if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    cudaError_t e = launch_transform_pack(precision, ctx->recon, ctx->gtrans[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_pack");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_transform_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision)
+{
+    int rc = check_transform(ctx, precision);
+    if (rc) return rc;
+    if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    cudaError_t e = launch_transform_unpack(precision, ctx->recon, ctx->gtrans[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_unpack");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_transform_cast(gf_ctx* ctx, int from_precision, int to_precision)
+{
+    int rc = check_transform(ctx, from_precision);
+    if (rc) return rc;
+    rc = check_transform(ctx, to_precision);
+    if (rc) return rc;
+    if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_transform_cast needs two different precisions");
+    const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
+    cudaError_t e = launch_cast(from_precision, to_precision, ctx->recon, ctx->gtrans[from_precision], ctx->gtrans[to_precision],
+                                ctx->G, reproject, 2, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_cast");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precision, int dst_precision)
+{
+    int rc = check_transform(ctx, g_precision);
+    if (rc) return rc;
+    rc = check_prec(ctx, src_precision);
+    if (rc) return rc;
+    rc = check_prec(ctx, dst_precision);
+    if (rc) return rc;
+    cudaError_t e = launch_apply_transform(g_precision, src_precision, dst_precision, ctx->recon, ctx->gtrans[g_precision],
+                                           ctx->links[src_precision], ctx->links[dst_precision], ctx->G, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_apply_transform");
     ctx->launches += 1;
     return GF_OK;
 }

@@ -406,10 +406,10 @@ cudaError_t launch_unpack(int precision, int recon, const void* links, const Geo
 }
 
 template <typename TS, typename TD>
-static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G, int reproject, cudaStream_t st)
+static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G, int reproject, int nblocks, cudaStream_t st)
 {
     const uint32_t block = 128;
-    const dim3 grid((G.Vh + block - 1) / block, 8, 1);
+    const dim3 grid((G.Vh + block - 1) / block, (uint32_t)nblocks, 1);
     if (recon == 12)
         cast_kernel<TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
     else
@@ -418,12 +418,161 @@ static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G
 }
 
 cudaError_t launch_cast(int from_precision, int to_precision, int recon, const void* src, void* dst,
-                        const Geom& G, int reproject, cudaStream_t st)
+                        const Geom& G, int reproject, int nblocks, cudaStream_t st)
 {
-    if (from_precision == PREC_F32 && to_precision == PREC_F64) return cast_run<float, double>(recon, src, dst, G, reproject, st);
-    if (from_precision == PREC_F64 && to_precision == PREC_F32) return cast_run<double, float>(recon, src, dst, G, reproject, st);
-    if (from_precision == PREC_F64) return cast_run<double, double>(recon, src, dst, G, reproject, st);
-    return cast_run<float, float>(recon, src, dst, G, reproject, st);
+    if (from_precision == PREC_F32 && to_precision == PREC_F64) return cast_run<float, double>(recon, src, dst, G, reproject, nblocks, st);
+    if (from_precision == PREC_F64 && to_precision == PREC_F32) return cast_run<double, float>(recon, src, dst, G, reproject, nblocks, st);
+    if (from_precision == PREC_F64) return cast_run<double, double>(recon, src, dst, G, reproject, nblocks, st);
+    return cast_run<float, float>(recon, src, dst, G, reproject, nblocks, st);
+}
+
+// ------------------------------------------------------- the accumulated transformation G(x)
+// G[parity][chunk][h]: one link-shaped block per parity.  Canonical form: (V,3,3) complex, site-major.
+template <typename T, int RECON, typename TC, bool TO_INTERNAL>
+__global__ void transform_convert_kernel(T* __restrict__ gtrans, const Geom G, TC* __restrict__ canonical)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    const Site s = decode_site(G, h, parity);
+    TC* c = canonical + (2u * (size_t)h + s.xodd) * 18;
+    T* blk = gtrans + (size_t)parity * RECON * G.Vh;
+    T m[18];
+    if (TO_INTERNAL) {
+#pragma unroll
+        for (int k = 0; k < 18; ++k) m[k] = (T)c[k];
+        store_link<RECON>(blk, G.Vh, h, m);
+    } else {
+        load_link<RECON>(blk, G.Vh, h, m);
+        if (RECON == 12) reconstruct_row2(m);
+#pragma unroll
+        for (int k = 0; k < 18; ++k) c[k] = (TC)m[k];
+    }
+}
+
+template <typename T, int RECON>
+__global__ void transform_identity_kernel(T* __restrict__ gtrans, const Geom G)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    T m[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m[k] = T(0);
+    m[0] = m[8] = m[16] = T(1);
+    store_link<RECON>(gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, m);
+}
+
+template <typename T, int RECON, bool TO_INTERNAL>
+static cudaError_t transform_convert_run(void* gtrans, const Geom& G, void* canonical, int canonical_is_f64, cudaStream_t st)
+{
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    if (canonical_is_f64)
+        transform_convert_kernel<T, RECON, double, TO_INTERNAL><<<grid, block, 0, st>>>(static_cast<T*>(gtrans), G, static_cast<double*>(canonical));
+    else
+        transform_convert_kernel<T, RECON, float, TO_INTERNAL><<<grid, block, 0, st>>>(static_cast<T*>(gtrans), G, static_cast<float*>(canonical));
+    return cudaGetLastError();
+}
+
+template <bool TO_INTERNAL>
+static cudaError_t transform_convert(int precision, int recon, void* gtrans, const Geom& G, void* canonical, int is_f64, cudaStream_t st)
+{
+    if (precision == PREC_F64)
+        return recon == 12 ? transform_convert_run<double, 12, TO_INTERNAL>(gtrans, G, canonical, is_f64, st)
+                           : transform_convert_run<double, 18, TO_INTERNAL>(gtrans, G, canonical, is_f64, st);
+    return recon == 12 ? transform_convert_run<float, 12, TO_INTERNAL>(gtrans, G, canonical, is_f64, st)
+                       : transform_convert_run<float, 18, TO_INTERNAL>(gtrans, G, canonical, is_f64, st);
+}
+
+cudaError_t launch_transform_pack(int precision, int recon, void* gtrans, const Geom& G, const void* canonical,
+                                  int canonical_is_f64, cudaStream_t st)
+{
+    return transform_convert<true>(precision, recon, gtrans, G, const_cast<void*>(canonical), canonical_is_f64, st);
+}
+
+cudaError_t launch_transform_unpack(int precision, int recon, const void* gtrans, const Geom& G, void* canonical,
+                                    int canonical_is_f64, cudaStream_t st)
+{
+    return transform_convert<false>(precision, recon, const_cast<void*>(gtrans), G, canonical, canonical_is_f64, st);
+}
+
+cudaError_t launch_transform_identity(int precision, int recon, void* gtrans, const Geom& G, cudaStream_t st)
+{
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    if (precision == PREC_F64) {
+        if (recon == 12) transform_identity_kernel<double, 12><<<grid, block, 0, st>>>(static_cast<double*>(gtrans), G);
+        else transform_identity_kernel<double, 18><<<grid, block, 0, st>>>(static_cast<double*>(gtrans), G);
+    } else {
+        if (recon == 12) transform_identity_kernel<float, 12><<<grid, block, 0, st>>>(static_cast<float*>(gtrans), G);
+        else transform_identity_kernel<float, 18><<<grid, block, 0, st>>>(static_cast<float*>(gtrans), G);
+    }
+    return cudaGetLastError();
+}
+
+// PAPER.md:43 (eq. 3): dst_mu(x) = G(x) src_mu(x) G(x+mu)^dagger, formed in fp64 whatever the storage
+// types.  A transformation accumulated in fp32 has drifted from SU(3) by its rounding; it is
+// re-projected (Gram-Schmidt) in fp64 before use, so that the result is gauge equivalent to src to
+// fp64 accuracy.  Every link is read and written by the same thread: src may alias dst.
+template <typename TG, int RECON>
+__device__ __forceinline__ void load_transform_d(const TG* gtrans, const Geom& G, uint32_t parity, uint32_t h, double (&m)[18])
+{
+    TG u[18];
+    load_link<RECON>(gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, u);
+    if (RECON == 12) reconstruct_row2(u);
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m[k] = (double)u[k];
+    if (sizeof(TG) == 4) project_su3(m);
+}
+
+template <typename TG, typename TS, typename TD, int RECON>
+__global__ void apply_transform_kernel(const TG* __restrict__ gtrans, const TS* src, TD* dst, const Geom G)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    const Site s = decode_site(G, h, parity);
+    double Gx[18];
+    load_transform_d<TG, RECON>(gtrans, G, parity, h, Gx);
+    for (int mu = 0; mu < 4; ++mu) {
+        double U[18], Gf[18], tmp[18], out[18];
+        load_full_d<TS, RECON>(src, G, parity, mu, h, U);
+        load_transform_d<TG, RECON>(gtrans, G, parity ^ 1u, forward_index(G, s, mu), Gf);
+        mul_full(Gx, U, tmp, false);
+        mul_full(tmp, Gf, out, true);
+        TD o[18];
+#pragma unroll
+        for (int k = 0; k < 18; ++k) o[k] = (TD)out[k];
+        store_link<RECON>(dst + block_offset<TD>(parity, mu, RECON, G.Vh), G.Vh, h, o);
+    }
+}
+
+template <typename TG, typename TS, typename TD>
+static cudaError_t apply_run(int recon, const void* gtrans, const void* src, void* dst, const Geom& G, cudaStream_t st)
+{
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    if (recon == 12)
+        apply_transform_kernel<TG, TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G);
+    else
+        apply_transform_kernel<TG, TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G);
+    return cudaGetLastError();
+}
+
+template <typename TG>
+static cudaError_t apply_prec(int src_precision, int dst_precision, int recon, const void* gtrans, const void* src, void* dst,
+                              const Geom& G, cudaStream_t st)
+{
+    if (src_precision == PREC_F64)
+        return dst_precision == PREC_F64 ? apply_run<TG, double, double>(recon, gtrans, src, dst, G, st)
+                                         : apply_run<TG, double, float>(recon, gtrans, src, dst, G, st);
+    return dst_precision == PREC_F64 ? apply_run<TG, float, double>(recon, gtrans, src, dst, G, st)
+                                     : apply_run<TG, float, float>(recon, gtrans, src, dst, G, st);
+}
+
+cudaError_t launch_apply_transform(int g_precision, int src_precision, int dst_precision, int recon,
+                                   const void* gtrans, const void* src, void* dst, const Geom& G, cudaStream_t st)
+{
+    return g_precision == PREC_F64 ? apply_prec<double>(src_precision, dst_precision, recon, gtrans, src, dst, G, st)
+                                   : apply_prec<float>(src_precision, dst_precision, recon, gtrans, src, dst, G, st);
 }
 
 // ------------------------------------------------------------------------------- Philox KAT

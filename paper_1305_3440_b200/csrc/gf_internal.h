@@ -12,6 +12,7 @@ enum { PREC_F32 = 0, PREC_F64 = 1 };
 
 struct SweepArgs {
     void* links;            // internal field of the chosen precision
+    void* gtrans;           // accumulated transformation of the same precision, or NULL
     Geom G;
     uint32_t parity;        // active parity
     int mu0;                // first direction entering K: 0 Landau, 1 Coulomb
@@ -43,8 +44,18 @@ cudaError_t launch_pack(int precision, int recon, void* links, const Geom& G, co
                         int canonical_is_f64, cudaStream_t st);
 cudaError_t launch_unpack(int precision, int recon, const void* links, const Geom& G, void* canonical,
                           int canonical_is_f64, cudaStream_t st);
+// nblocks: 8 for a link field (parity x mu), 2 for a transformation field (parity)
 cudaError_t launch_cast(int from_precision, int to_precision, int recon, const void* src, void* dst,
-                        const Geom& G, int reproject, cudaStream_t st);
+                        const Geom& G, int reproject, int nblocks, cudaStream_t st);
+// transformation field G[parity][chunk][h] <-> canonical (V,3,3) complex; identity fill
+cudaError_t launch_transform_pack(int precision, int recon, void* gtrans, const Geom& G, const void* canonical,
+                                  int canonical_is_f64, cudaStream_t st);
+cudaError_t launch_transform_unpack(int precision, int recon, const void* gtrans, const Geom& G, void* canonical,
+                                    int canonical_is_f64, cudaStream_t st);
+cudaError_t launch_transform_identity(int precision, int recon, void* gtrans, const Geom& G, cudaStream_t st);
+// dst_mu(x) = G(x) src_mu(x) G(x+mu)^dagger in fp64 (eq. 3); src may alias dst
+cudaError_t launch_apply_transform(int g_precision, int src_precision, int dst_precision, int recon,
+                                   const void* gtrans, const void* src, void* dst, const Geom& G, cudaStream_t st);
 cudaError_t launch_philox(int n, const uint32_t* ctr, const uint32_t* key, uint32_t* out, cudaStream_t st);
 
 }  // namespace gf

@@ -104,6 +104,45 @@ class GaugeField:
     def unitarity(self, precision):
         return B.gf_unitarity(self.ctx, precision)
 
+    # ---- the accumulated transformation G(x)
+    def attach_transform(self, precisions=("f64",)):
+        """Allocates G(x) for the given precisions, sets it to the identity and attaches it: sweeps of
+        those precisions then record G(x) <- g(x) G(x).  attach_transform(()) detaches."""
+        self._gbufs = {}
+        for name, prec in (("f32", B.GF_F32), ("f64", B.GF_F64)):
+            if name in precisions:
+                n = B.gf_transform_bytes(self.dims, prec, self.recon)
+                self._gbufs[prec] = torch.empty(n, dtype=torch.uint8, device=self.device)
+        B.gf_set_transform(self.ctx,
+                           self._gbufs[B.GF_F64].data_ptr() if B.GF_F64 in self._gbufs else 0,
+                           self._gbufs[B.GF_F32].data_ptr() if B.GF_F32 in self._gbufs else 0)
+        for prec in self._gbufs:
+            B.gf_transform_identity(self.ctx, prec)
+
+    def transform(self, precision, dtype=torch.complex128):
+        """G(x) as a canonical tensor (Nt, Nz, Ny, Nx, 3, 3)."""
+        out = torch.empty(self.shape[:4] + (3, 3), dtype=dtype, device=self.device)
+        B.gf_transform_unpack(self.ctx, out.data_ptr(), dtype == torch.complex128, precision)
+        return out
+
+    def set_transform(self, canonical, precision):
+        if canonical.dtype not in (torch.complex128, torch.complex64) or tuple(canonical.shape) != self.shape[:4] + (3, 3) \
+                or not canonical.is_contiguous() or canonical.device != self.device:
+            raise ValueError("transformation must be contiguous complex %r on %s" % (self.shape[:4] + (3, 3), self.device))
+        B.gf_transform_pack(self.ctx, canonical.data_ptr(), canonical.dtype == torch.complex128, precision)
+
+    def transform_identity(self, precision):
+        B.gf_transform_identity(self.ctx, precision)
+
+    def transform_cast(self, from_precision, to_precision):
+        B.gf_transform_cast(self.ctx, from_precision, to_precision)
+
+    def apply_transform(self, g_precision, src_precision, dst_precision):
+        B.gf_apply_transform(self.ctx, g_precision, src_precision, dst_precision)
+
+    def cast(self, from_precision, to_precision):
+        B.gf_cast(self.ctx, from_precision, to_precision)
+
     def set_tuning(self, precision, lanes, block):
         B.gf_set_tuning(self.ctx, precision, lanes, block)
 
