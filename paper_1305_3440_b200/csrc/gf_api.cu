@@ -232,11 +232,12 @@ static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
 
 // Launch configuration chosen by measurement on B200 at 32^4 (profiles/r1_tune_32x32x32x32.txt,
 // DESIGN.md "Kernels"): two lanes per site everywhere except fp64 / 12-real (four).
-static void default_tuning(int precision, int recon, int solver_f64, int* lanes, int* block)
+static void default_tuning(int precision, int recon, int solver_f64, int accumulate, int* lanes, int* block)
 {
     if (precision == GF_F64) {
         *lanes = recon == GF_RECON12 ? 4 : 2;
         *block = recon == GF_RECON12 ? 64 : 128;
+        if (accumulate && recon == GF_RECON12) *lanes = 1;      // one lane does the G(x) update: no imbalance with one lane per site
     } else {
         *lanes = 2;
         *block = (recon == GF_RECON18 && !solver_f64) ? 128 : 64;
@@ -260,7 +261,7 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.reverse = ctx->zigzag ? (uint32_t)(ctx->sweeps & 1u) : 0u;
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
     int lanes, block;
-    default_tuning(precision, ctx->recon, solver_f64, &lanes, &block);
+    default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, &lanes, &block);
     if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
     if (ctx->block[precision]) block = ctx->block[precision];
     cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, lanes, block, a, ctx->stream);

@@ -60,6 +60,15 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     if (!live) h = G.Vh - 1u;                           // keeps the lane in the shuffles; no store
     const Site s = decode_site(G, h, P.parity);
 
+    if (ACC && j == 0) {
+        // G(x) is only needed after the links have been written back: start moving it towards L2 now
+        const T* gp = P.gtrans + (size_t)P.parity * RECON * G.Vh;
+        constexpr int CH = (RECON * (int)sizeof(T)) / 16;      // whole 16-byte chunks (the fp32/18 tail rides along)
+#pragma unroll
+        for (int c = 0; c < CH; ++c)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(gp) + ((size_t)c * G.Vh + h) * 16));
+    }
+
     // a2: gather this lane's links
     T Uf[ND][18], Ub[ND][18];
     uint32_t hb[ND];

@@ -174,6 +174,48 @@ def test_philox_known_answers_on_device(cuda_device):
         assert tuple(out[i]) == oracle.philox4x32_10(ctr[i].tolist(), key[i].tolist())
 
 
+def test_philox_agrees_with_curand_on_device(cuda_device):
+    """Pin 13: a library routine as third opinion.  cuRAND's Philox4_32_10 device
+    generator (tests/curand_philox_ref.cu, test-only) initialised with (seed, subsequence = half-sweep
+    counter, offset = 4 * site) returns, as its first block, Philox4x32-10 of the counter
+    (site lo, site hi, counter, 0) under the key (seed lo, seed hi) -- the sweep kernel's draw.  The
+    oracle's and the library's device implementations must both reproduce it bit for bit."""
+    import ctypes
+    import os
+    import subprocess
+    here = os.path.dirname(os.path.abspath(__file__))
+    so, src = os.path.join(here, "libcurand_philox_ref.so"), os.path.join(here, "curand_philox_ref.cu")
+    if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
+        subprocess.run(["/usr/local/cuda/bin/nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared",
+                        "-Xcompiler", "-fPIC", src, "-o", so], check=True)
+    ref = ctypes.CDLL(so)
+    ref.curand_philox_ref.argtypes = [ctypes.c_int] + [ctypes.c_void_p] * 5
+    rng = np.random.default_rng(17)
+    n = 2000
+    seed = rng.integers(0, 2 ** 63, n, dtype=np.int64)
+    site = rng.integers(0, 2 ** 40, n, dtype=np.int64)           # beyond 2^32: exercises the high word
+    site[:4] = [0, 1, 2 ** 32 - 1, 2 ** 32]
+    counter = rng.integers(0, 2 ** 32, n, dtype=np.int64)
+    d_seed, d_sub, d_off = (torch.from_numpy(a).to(cuda_device) for a in (seed, counter, 4 * site))
+    d_ref = torch.zeros(n * 4, dtype=torch.int32, device=cuda_device)
+    assert ref.curand_philox_ref(n, d_seed.data_ptr(), d_sub.data_ptr(), d_off.data_ptr(), d_ref.data_ptr(),
+                                 torch.cuda.current_stream().cuda_stream) == 0
+    ctr = np.stack([site & 0xffffffff, site >> 32, counter, np.zeros(n, np.int64)], axis=1).astype(np.uint32)
+    key = np.stack([seed & 0xffffffff, seed >> 32], axis=1).astype(np.uint32)
+    fld = make_field((4, 4, 4, 4), "f64", cuda_device)
+    d_c = torch.from_numpy(ctr.view(np.int32)).to(cuda_device)
+    d_k = torch.from_numpy(key.view(np.int32)).to(cuda_device)
+    d_o = torch.zeros_like(d_c)
+    gf.gf_debug_philox(fld.ctx, n, d_c.data_ptr(), d_k.data_ptr(), d_o.data_ptr())
+    torch.cuda.synchronize()
+    want = d_ref.cpu().numpy().view(np.uint32).reshape(n, 4)
+    assert np.array_equal(d_o.cpu().numpy().view(np.uint32), want)
+    for i in range(0, n, 10):
+        assert oracle.philox4x32_10(ctr[i].tolist(), key[i].tolist()) == tuple(want[i])
+        u = oracle.site_uniforms(int(seed[i]), int(counter[i]), int(site[i]))
+        assert all(u[k] == (int(want[i][k]) >> 8) / 2.0 ** 24 for k in range(3))
+
+
 # ---------------------------------------------------------------------------------- the fix loop
 
 @pytest.mark.parametrize("seed", [0, 1, 2, 3, 4])
