@@ -49,6 +49,11 @@ def load():
     lib.oracle_sweep_accumulate.argtypes = [cd_p, cd_p, i4, C.c_int, C.c_int, C.c_int, C.c_double,
                                             C.c_double, C.c_uint64, C.c_uint32]
     lib.oracle_apply_transform.argtypes = [cd_p, cd_p, i4, cd_p]
+    lib.oracle_sweep_masked.argtypes = [cd_p, cd_p, i4, i4, C.c_int, C.c_int, C.c_int, C.c_double,
+                                        C.c_double, C.c_uint64, C.c_uint32]
+    lib.oracle_fix_until_freeze.argtypes = [cd_p, i4, C.c_int, C.c_double, C.c_double, C.c_uint64, C.c_uint32,
+                                            C.c_double, C.c_int, C.c_int, dbl_p, i4, C.POINTER(C.c_int)]
+    lib.oracle_fix_until_freeze.restype = C.c_int
     lib.oracle_fix_until.argtypes = [cd_p, i4, C.c_int, C.c_int, C.c_double, C.c_double,
                                      C.c_uint64, C.c_uint32, C.c_double, C.c_int, C.c_int,
                                      dbl_p, C.POINTER(C.c_int)]
@@ -197,6 +202,25 @@ def apply_transform(U, G, dims):
     out = np.empty_like(U)
     load().oracle_apply_transform(_field(U, dims), _transform(G, dims), _dims(dims), _field(out, dims))
     return out
+
+
+def sweep_masked(U, dims, parity, slice_active, G=None, gauge=COULOMB, algo=OVERRELAX, omega=1.0, p=0.0, seed=0,
+                 half_sweep_counter=0):
+    """Half-sweep that skips the sites of time slices with slice_active[t] == 0 (reading A17b)."""
+    act = (C.c_int * dims[0])(*[int(bool(a)) for a in slice_active])
+    load().oracle_sweep_masked(_field(U, dims), _transform(G, dims) if G is not None else None, act, _dims(dims),
+                               gauge, parity, algo, omega, p, int(seed), int(half_sweep_counter))
+
+
+def fix_until_freeze(U, dims, algo=OVERRELAX, omega=1.0, p=0.0, seed=0, first_counter=0, theta_target=1e-12,
+                     max_iter=2000, check_every=1):
+    """Coulomb gauge with slice freezing.  Returns (iterations, theta_t array, frozen_at array, converged)."""
+    th = np.zeros(dims[0])
+    fr = (C.c_int * dims[0])()
+    conv = C.c_int()
+    it = load().oracle_fix_until_freeze(_field(U, dims), _dims(dims), algo, omega, p, int(seed), int(first_counter),
+                                        theta_target, max_iter, check_every, _dbl(th), fr, C.byref(conv))
+    return it, th, np.array(list(fr)), bool(conv.value)
 
 
 def fix_until(U, dims, gauge=LANDAU, algo=OVERRELAX, omega=1.0, p=0.0, seed=0, first_counter=0,

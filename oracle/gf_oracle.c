@@ -381,12 +381,13 @@ void oracle_update_links8(cd fwd[4][9], cd bwd[4][9], int gauge, int algo,
 /* Gtot (may be NULL): the accumulated transformation, one 3x3 matrix per site,
  * Gtot[s][a][b].  A site visit applies g(x) on top of what was applied before,
  * so by PAPER.md:43 (eq. 3) the total transformation becomes g(x) Gtot(x). */
-static void visit_site(cd *U, cd *Gtot, const int dims[4], int gauge, int parity, int algo,
+static void visit_site(cd *U, cd *Gtot, const int *slice_active, const int dims[4], int gauge, int parity, int algo,
                        double omega, double p, uint64_t seed, uint32_t half_sweep_counter, size_t s)
 {
     int c[4];
     site_coords(dims, s, c);
     if (site_parity(c) != parity) return;
+    if (slice_active && !slice_active[c[0]]) return;   /* frozen time slice (Coulomb, reading A17b) */
     cd *fwd[4], *bwd[4];
     for (int mu = 0; mu < 4; ++mu) {
         fwd[mu] = link_ptr(U, s, mu);
@@ -406,26 +407,26 @@ static void visit_site(cd *U, cd *Gtot, const int dims[4], int gauge, int parity
  * time; the sites are visited in lexicographic order (reverse_order != 0: in
  * the opposite order -- same-parity sites share no link, so the result must be
  * bitwise the same; that is one of the pins). */
-static void sweep_impl(cd *U, cd *Gtot, const int dims[4], int gauge, int parity, int algo, double omega,
+static void sweep_impl(cd *U, cd *Gtot, const int *slice_active, const int dims[4], int gauge, int parity, int algo, double omega,
                        double p, uint64_t seed, uint32_t half_sweep_counter, int reverse_order)
 {
     const size_t V = volume(dims);
     if (reverse_order) {
         for (size_t k = V; k-- > 0;)
-            visit_site(U, Gtot, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, k);
+            visit_site(U, Gtot, slice_active, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, k);
         return;
     }
 #ifdef _OPENMP
 #pragma omp parallel for num_threads(g_threads) schedule(static)
 #endif
     for (size_t s = 0; s < V; ++s)
-        visit_site(U, Gtot, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, s);
+        visit_site(U, Gtot, slice_active, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, s);
 }
 
 void oracle_sweep_ordered(cd *U, const int dims[4], int gauge, int parity, int algo, double omega,
                           double p, uint64_t seed, uint32_t half_sweep_counter, int reverse_order)
 {
-    sweep_impl(U, NULL, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, reverse_order);
+    sweep_impl(U, NULL, NULL, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, reverse_order);
 }
 
 /* The same half-sweep, also recording the transformation: Gtot(x) <- g(x) Gtot(x)
@@ -435,7 +436,18 @@ void oracle_sweep_ordered(cd *U, const int dims[4], int gauge, int parity, int a
 void oracle_sweep_accumulate(cd *U, cd *Gtot, const int dims[4], int gauge, int parity, int algo,
                              double omega, double p, uint64_t seed, uint32_t half_sweep_counter)
 {
-    sweep_impl(U, Gtot, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, 0);
+    sweep_impl(U, Gtot, NULL, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, 0);
+}
+
+/* Reading A17b (an option beside A17; PAPER.md:11, :29 only name Coulomb gauge): time slices
+ * are fixed independently -- in Coulomb gauge K, F_t and theta_t of slice t involve only the
+ * spatial links of slice t, which only the sites of slice t change -- so a slice whose theta_t
+ * has reached the target may stop being swept ("frozen").  slice_active[t] != 0: the sites of
+ * slice t are visited; 0: skipped.  Gtot may be NULL. */
+void oracle_sweep_masked(cd *U, cd *Gtot, const int *slice_active, const int dims[4], int gauge, int parity,
+                         int algo, double omega, double p, uint64_t seed, uint32_t half_sweep_counter)
+{
+    sweep_impl(U, Gtot, slice_active, dims, gauge, parity, algo, omega, p, seed, half_sweep_counter, 0);
 }
 
 /* PAPER.md:43 (eq. 3) written out: U_out_mu(x) = G(x) U_mu(x) G(x + mu_hat)^dagger. */
@@ -493,6 +505,38 @@ int oracle_fix_until(cd *U, const int dims[4], int gauge, int algo, double omega
         }
     }
     *theta_out = theta;
+    return it;
+}
+
+/* The fix loop of oracle_fix_until for Coulomb gauge with slice freezing (A17b): after every
+ * theta evaluation the slices with theta_t < target are frozen for the rest of the run; the
+ * run ends when all are frozen.  theta_slices[t] = theta_t at the last evaluation (a frozen
+ * slice keeps its value: nothing that enters it changes any more); frozen_at[t] = iteration at
+ * which slice t was frozen (0 = never).  Returns the iterations done. */
+int oracle_fix_until_freeze(cd *U, const int dims[4], int algo, double omega, double p, uint64_t seed,
+                            uint32_t first_counter, double theta_target, int max_iter, int check_every,
+                            double *theta_slices, int *frozen_at, int *converged)
+{
+    int active[4096];
+    const int nt = dims[0];
+    for (int t = 0; t < nt; ++t) { active[t] = 1; frozen_at[t] = 0; }
+    *converged = 0;
+    int it = 0;
+    if (check_every < 1) check_every = 1;
+    while (it < max_iter) {
+        oracle_sweep_masked(U, NULL, active, dims, ORACLE_COULOMB, 0, algo, omega, p, seed, first_counter + 2u * (uint32_t)it);
+        oracle_sweep_masked(U, NULL, active, dims, ORACLE_COULOMB, 1, algo, omega, p, seed, first_counter + 2u * (uint32_t)it + 1u);
+        ++it;
+        if (it % check_every == 0 || it == max_iter) {
+            oracle_theta(U, dims, ORACLE_COULOMB, theta_slices);
+            int left = 0;
+            for (int t = 0; t < nt; ++t) {
+                if (active[t] && theta_slices[t] < theta_target) { active[t] = 0; frozen_at[t] = it; }
+                left += active[t];
+            }
+            if (left == 0) { *converged = 1; break; }
+        }
+    }
     return it;
 }
 

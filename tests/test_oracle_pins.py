@@ -474,3 +474,53 @@ def test_accumulated_transformation_reproduces_the_swept_links(gauge, algo):
     GG = np.einsum("...ab,...cb->...ac", G, G.conj())
     assert np.abs(GG - np.eye(3)).max() < 1e-13
     assert np.abs(np.linalg.det(G) - 1).max() < 1e-13
+
+
+# ------------------------------------------------- Coulomb gauge: frozen slices (reading A17b)
+
+def test_masked_sweep_skips_exactly_the_frozen_slices():
+    dims = (6, 4, 4, 4)
+    U0 = gi.smooth_random_gauge(dims, 0.5, 8)
+    kw = dict(gauge=oracle.COULOMB, algo=oracle.STOCHASTIC, p=0.6, seed=3, half_sweep_counter=4)
+    A, B = U0.copy(), U0.copy()
+    oracle.sweep_masked(A, dims, 0, [1] * 6, **kw)
+    oracle.sweep(B, dims, 0, **kw)
+    assert np.array_equal(A, B)                                  # all active = the plain sweep
+    C = U0.copy()
+    oracle.sweep_masked(C, dims, 0, [1, 0, 1, 1, 0, 1], **kw)
+    oracle.sweep_masked(C, dims, 1, [1, 0, 1, 1, 0, 1], **dict(kw, half_sweep_counter=5))
+    oracle.sweep(B, dims, 1, **dict(kw, half_sweep_counter=5))
+    for t in (1, 4):                                             # frozen: spatial links untouched, theta_t unchanged
+        assert np.array_equal(C[t][..., 1:, :, :], U0[t][..., 1:, :, :])
+    th0, thC, thB = (oracle.theta(X, dims, oracle.COULOMB) for X in (U0, C, B))
+    assert thC[1] == th0[1] and thC[4] == th0[4]
+    for t in (0, 2, 3, 5):                                       # active slices evolve as if nothing were frozen
+        assert np.array_equal(C[t][..., 1:, :, :], B[t][..., 1:, :, :])
+        assert thC[t] == thB[t]
+    # the temporal links leaving a frozen slice are still rotated by the active slice above it
+    assert not np.array_equal(C[1][..., 0, :, :], U0[1][..., 0, :, :])
+    assert abs(oracle.plaquette(C, dims) - oracle.plaquette(U0, dims)) < 1e-14
+
+
+def test_fix_until_freeze_fixes_every_slice_as_the_unfrozen_run_does():
+    """Each slice ends exactly where the unfrozen run had it at the iteration it was frozen (slices are
+    decoupled); every theta_t < target; the run is still a gauge transformation."""
+    dims = (6, 4, 4, 6)
+    U0 = gi.smooth_random_gauge(dims, 0.4, 31)
+    kw = dict(algo=oracle.OVERRELAX, omega=1.6)
+    U = U0.copy()
+    it, th, frozen_at, conv = oracle.fix_until_freeze(U, dims, theta_target=1e-12, max_iter=3000, check_every=1, **kw)
+    assert conv and np.all(th < 1e-12) and np.all(frozen_at > 0) and it == frozen_at.max()
+    assert len(set(frozen_at.tolist())) > 1                      # the slices do converge at different times
+    assert np.array_equal(th, oracle.theta(U, dims, oracle.COULOMB))
+    assert abs(oracle.plaquette(U, dims) - oracle.plaquette(U0, dims)) < 1e-13
+    W = U0.copy()
+    for n in range(1, it + 1):
+        for parity in (0, 1):
+            oracle.sweep(W, dims, parity, gauge=oracle.COULOMB, half_sweep_counter=2 * (n - 1) + parity, **kw)
+        for t in np.nonzero(frozen_at == n)[0]:
+            assert np.array_equal(W[t][..., 1:, :, :], U[t][..., 1:, :, :])
+    # and it stops no later than the unfrozen loop
+    it_plain, _, conv_plain = oracle.fix_until(U0.copy(), dims, gauge=oracle.COULOMB, theta_target=1e-12, max_iter=3000,
+                                               check_every=1, **kw)
+    assert conv_plain and it == it_plain
