@@ -53,6 +53,9 @@ def _load():
         "gf_transform_unpack": (i32, [vp, vp, i32, i32]),
         "gf_transform_cast": (i32, [vp, i32, i32]),
         "gf_apply_transform": (i32, [vp, i32, i32, i32]),
+        "gf_set_coulomb_mode": (i32, [vp, i32, i32]),
+        "gf_coulomb_finish": (i32, [vp, i32]),
+        "gf_set_slice_mask": (i32, [vp, C.c_char_p]),
         "gf_set_rng": (i32, [vp, u64, u32]),
         "gf_get_counter": (i32, [vp, C.POINTER(u32)]),
         "gf_reunitarize": (i32, [vp, i32]),
@@ -77,7 +80,7 @@ lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
            "gf_sweep gf_functional gf_theta gf_measure gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
-           "gf_transform_cast gf_apply_transform gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_debug_philox gf_launch_count gf_last_error "
+           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
 
 
@@ -219,6 +222,20 @@ def gf_transform_cast(ctx, from_precision, to_precision, check=True):
 
 def gf_apply_transform(ctx, g_precision, src_precision, dst_precision, check=True):
     return _rc(ctx, lib.gf_apply_transform(ctx, g_precision, src_precision, dst_precision), check)
+
+
+def gf_set_coulomb_mode(ctx, defer_temporal, freeze_slices, check=True):
+    return _rc(ctx, lib.gf_set_coulomb_mode(ctx, int(defer_temporal), int(freeze_slices)), check)
+
+
+def gf_coulomb_finish(ctx, precision, check=True):
+    return _rc(ctx, lib.gf_coulomb_finish(ctx, precision), check)
+
+
+def gf_set_slice_mask(ctx, active, check=True):
+    """active: sequence of Nt truth values, or None for all slices."""
+    buf = None if active is None else bytes(1 if a else 0 for a in active)
+    return _rc(ctx, lib.gf_set_slice_mask(ctx, buf), check)
 
 
 def gf_plaquette(ctx, precision, check=True):

@@ -11,6 +11,10 @@
 
 using namespace gf;
 
+extern "C" int gf_transform_identity(gf_ctx* ctx, int precision);
+extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision);
+static int upload_mask(gf_ctx* ctx);
+
 namespace {
 constexpr int kMeasureBlock = 128;
 constexpr int kMaxNt = 4096;
@@ -21,6 +25,12 @@ struct gf_ctx {
     int gauge, recon;
     void* links[2];             // [PREC_F32], [PREC_F64]
     void* gtrans[2];            // accumulated transformation per precision (gf_set_transform), or NULL
+    int defer_temporal;         // Coulomb: sweeps record G(x) and leave the temporal links to gf_coulomb_finish
+    int freeze_slices;          // Coulomb: gf_fix_until stops sweeping slices whose theta_t is below the target
+    int pending[2];             // deferred temporal update outstanding for the field of that precision
+    uint8_t* dev_mask;          // workspace: one byte per time slice, 0 = frozen
+    uint8_t* host_mask;         // pinned copy
+    int mask_on;                // the sweeps consult dev_mask
     double* workspace;
     double* partials;           // workspace: per-block partial sums
     double* slice_out;          // workspace: 2 doubles per time slice
@@ -91,7 +101,7 @@ extern "C" size_t gf_workspace_bytes(const int dims[4])
 {
     if (!dims_ok(dims)) return 0;
     const MeasureGrid mg = measure_grid(dims);
-    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double);
+    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt;   // + the slice mask
 }
 
 extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
@@ -127,6 +137,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->mg = measure_grid(dims);
     c->partials = c->workspace;
     c->slice_out = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
+    c->dev_mask = reinterpret_cast<uint8_t*>(c->slice_out + (size_t)dims[0] * 2);
 
     Geom& G = c->G;
     G.nt = dims[0];
@@ -149,11 +160,12 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->solver_mode = GF_SOLVER_AUTO;
     c->zigzag = 1;
 
-    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt) != cudaSuccess) {
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return GF_ENOMEM;
     }
+    c->host_mask = reinterpret_cast<uint8_t*>(c->host_pinned + 2 * kMaxNt);
     *out = c;
     return GF_OK;
 }
@@ -179,6 +191,7 @@ extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_
 {
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
+    ctx->pending[precision] = 0;      // the field is overwritten: nothing left to apply
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
     cudaError_t e = launch_pack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_pack");
@@ -189,6 +202,8 @@ extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_
 extern "C" int gf_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision)
 {
     int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
     cudaError_t e = launch_unpack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
@@ -246,9 +261,20 @@ static void default_tuning(int precision, int recon, int solver_f64, int accumul
 
 static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
 {
+    if (ctx->defer_temporal) {
+        if (!ctx->gtrans[precision])
+            return fail(ctx, GF_ESTATE, "deferred temporal links need a transformation buffer for precision %d (gf_set_transform)", precision);
+        if (!ctx->pending[precision]) {      // G(x) restarts from the identity: it is what gf_coulomb_finish will apply
+            int rc = gf_transform_identity(ctx, precision);
+            if (rc) return rc;
+            ctx->pending[precision] = 1;
+        }
+    }
     SweepArgs a;
     a.links = ctx->links[precision];
     a.gtrans = ctx->gtrans[precision];
+    a.defer_temporal = ctx->defer_temporal;
+    a.slice_active = ctx->mask_on ? ctx->dev_mask : nullptr;
     a.G = ctx->G;
     a.parity = (uint32_t)parity;
     a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
@@ -353,6 +379,15 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
 {
     int it = *it_io;
     int rc = GF_NOT_CONVERGED;
+    const bool freeze = ctx->freeze_slices && ctx->gauge == GF_COULOMB;
+    if (freeze) {                            // every slice starts active (the stream is idle or ordered: pinned copy is free)
+        cudaError_t e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "fix loop");
+        for (int t = 0; t < ctx->dims[0]; ++t) ctx->host_mask[t] = 1;
+        ctx->mask_on = 1;
+        int rc0 = upload_mask(ctx);
+        if (rc0) return rc0;
+    }
     while (it < max_iter) {
         int n = check_every - (it % check_every);
         if (n > max_iter - it) n = max_iter - it;
@@ -366,7 +401,23 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
         if (e != GF_OK) { *it_io = it; return e; }
         *theta_out = finish_measure(ctx, nullptr, nullptr);
         if (*theta_out < target) { rc = GF_OK; break; }
+        if (freeze) {
+            // reading A17b: a slice below the target stops being swept; nothing that enters its F_t and
+            // theta_t changes afterwards, so max_t theta_t above remains the stopping criterion
+            const double Vs = (double)(ctx->V / ctx->dims[0]);
+            bool changed = false;
+            for (int t = 0; t < ctx->dims[0]; ++t)
+                if (ctx->host_mask[t] && ctx->host_pinned[2 * t + 1] / (3.0 * Vs) < target) {
+                    ctx->host_mask[t] = 0;
+                    changed = true;
+                }
+            if (changed) {
+                e = upload_mask(ctx);
+                if (e != GF_OK) { *it_io = it; return e; }
+            }
+        }
     }
+    if (freeze) ctx->mask_on = 0;
     *it_io = it;
     return rc;
 }
@@ -385,6 +436,10 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
     int rc = check_algo(ctx, algo, omega, p);
     if (rc) return rc;
     if (max_iter < 0 || check_every < 1 || !(theta_target >= 0.0)) return fail(ctx, GF_EINVAL, "bad max_iter / check_every / theta_target");
+    if (ctx->defer_temporal && precision == GF_MIXED_EXACT)
+        return fail(ctx, GF_ESTATE, "GF_MIXED_EXACT and deferred temporal links both use the transformation buffers");
+    if (ctx->defer_temporal && ((precision != GF_F64 && !ctx->gtrans[PREC_F32]) || (precision != GF_F32 && !ctx->gtrans[PREC_F64])))
+        return fail(ctx, GF_ESTATE, "deferred temporal links need a transformation buffer for every precision swept (gf_set_transform)");
 
     int it = 0;
     double theta = -1.0;
@@ -431,6 +486,10 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
         }
     }
     if (rc < 0) return rc;
+    for (int prec = 0; prec < 2; ++prec) {          // deferred temporal links: the result is a complete field
+        int e = gf_coulomb_finish(ctx, prec);
+        if (e != GF_OK) return e;
+    }
     if (iters_out) *iters_out = it;
     if (theta_out) *theta_out = theta;
     return rc;
@@ -455,6 +514,8 @@ extern "C" int gf_reunitarize(gf_ctx* ctx, int precision)
 {
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
+    rc = gf_coulomb_finish(ctx, precision);
+    if (rc) return rc;
     cudaError_t e = launch_cast(precision, precision, ctx->recon, ctx->links[precision], ctx->links[precision], ctx->G, 1, 8, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_reunitarize");
     ctx->launches += 1;
@@ -467,6 +528,9 @@ extern "C" int gf_cast(gf_ctx* ctx, int from_precision, int to_precision)
     if (rc) return rc;
     rc = check_prec(ctx, to_precision);
     if (rc) return rc;
+    rc = gf_coulomb_finish(ctx, from_precision);
+    if (rc) return rc;
+    ctx->pending[to_precision] = 0;
     if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_cast needs two different precisions");
     const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
     cudaError_t e = launch_cast(from_precision, to_precision, ctx->recon, ctx->links[from_precision], ctx->links[to_precision],
@@ -549,10 +613,71 @@ extern "C" int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precisio
     if (rc) return rc;
     rc = check_prec(ctx, dst_precision);
     if (rc) return rc;
+    rc = gf_coulomb_finish(ctx, src_precision);
+    if (rc) return rc;
     cudaError_t e = launch_apply_transform(g_precision, src_precision, dst_precision, ctx->recon, ctx->gtrans[g_precision],
-                                           ctx->links[src_precision], ctx->links[dst_precision], ctx->G, ctx->stream);
+                                           ctx->links[src_precision], ctx->links[dst_precision], ctx->G, 0, 4, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_apply_transform");
     ctx->launches += 1;
+    return GF_OK;
+}
+
+// ------------------------------------------------------------------- Coulomb specialisation
+extern "C" int gf_set_coulomb_mode(gf_ctx* ctx, int defer_temporal, int freeze_slices)
+{
+    if (!ctx) return GF_EINVAL;
+    if ((defer_temporal != 0 && defer_temporal != 1) || (freeze_slices != 0 && freeze_slices != 1))
+        return fail(ctx, GF_EINVAL, "defer_temporal and freeze_slices must be 0 or 1");
+    if (ctx->gauge != GF_COULOMB && (defer_temporal || freeze_slices))
+        return fail(ctx, GF_EINVAL, "deferred temporal links and slice freezing exist in Coulomb gauge only");
+    if (!defer_temporal) {
+        for (int prec = 0; prec < 2; ++prec) {
+            int rc = gf_coulomb_finish(ctx, prec);
+            if (rc) return rc;
+        }
+    }
+    ctx->defer_temporal = defer_temporal;
+    ctx->freeze_slices = freeze_slices;
+    return GF_OK;
+}
+
+// uploads ctx->host_mask (pinned) to the device; the copy is ordered on the stream between the sweeps
+static int upload_mask(gf_ctx* ctx)
+{
+    cudaError_t e = cudaMemcpyAsync(ctx->dev_mask, ctx->host_mask, (size_t)ctx->dims[0], cudaMemcpyHostToDevice, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "slice mask copy");
+    return GF_OK;
+}
+
+extern "C" int gf_set_slice_mask(gf_ctx* ctx, const uint8_t* host_active)
+{
+    if (!ctx) return GF_EINVAL;
+    if (ctx->gauge != GF_COULOMB && host_active) return fail(ctx, GF_EINVAL, "slice masks exist in Coulomb gauge only");
+    if (!host_active) {
+        ctx->mask_on = 0;
+        return GF_OK;
+    }
+    // the pinned staging copy may still be in flight from an earlier call
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_set_slice_mask");
+    for (int t = 0; t < ctx->dims[0]; ++t) ctx->host_mask[t] = host_active[t] ? 1 : 0;
+    ctx->mask_on = 1;
+    return upload_mask(ctx);
+}
+
+extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision)
+{
+    if (!ctx) return GF_EINVAL;
+    if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
+    if (!ctx->pending[precision]) return GF_OK;
+    if (!ctx->gtrans[precision] || !ctx->links[precision])
+        return fail(ctx, GF_ESTATE, "deferred temporal update pending but the transformation buffer was detached");
+    // U_0(x) <- G(x) U_0(x) G(x+0)^dagger (eq. 3): the spatial links already carry G
+    cudaError_t e = launch_apply_transform(precision, precision, precision, ctx->recon, ctx->gtrans[precision],
+                                           ctx->links[precision], ctx->links[precision], ctx->G, 0, 1, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_coulomb_finish");
+    ctx->launches += 1;
+    ctx->pending[precision] = 0;
     return GF_OK;
 }
 
@@ -569,6 +694,8 @@ extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)
 {
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
+    rc = gf_coulomb_finish(ctx, precision);
+    if (rc) return rc;
     if (!host_out) return fail(ctx, GF_EINVAL, "null output");
     cudaError_t e = launch_plaquette(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_plaquette launch");
@@ -583,6 +710,8 @@ extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)
 extern "C" int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2)
 {
     int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!host_out2) return fail(ctx, GF_EINVAL, "null output");
     cudaError_t e = launch_unitarity(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);

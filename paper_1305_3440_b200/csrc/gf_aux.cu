@@ -525,7 +525,8 @@ __device__ __forceinline__ void load_transform_d(const TG* gtrans, const Geom& G
 }
 
 template <typename TG, typename TS, typename TD, int RECON>
-__global__ void apply_transform_kernel(const TG* __restrict__ gtrans, const TS* src, TD* dst, const Geom G)
+__global__ void apply_transform_kernel(const TG* __restrict__ gtrans, const TS* src, TD* dst, const Geom G,
+                                       const int mu_begin, const int mu_end)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 2u * G.Vh) return;
@@ -533,7 +534,7 @@ __global__ void apply_transform_kernel(const TG* __restrict__ gtrans, const TS* 
     const Site s = decode_site(G, h, parity);
     double Gx[18];
     load_transform_d<TG, RECON>(gtrans, G, parity, h, Gx);
-    for (int mu = 0; mu < 4; ++mu) {
+    for (int mu = mu_begin; mu < mu_end; ++mu) {
         double U[18], Gf[18], tmp[18], out[18];
         load_full_d<TS, RECON>(src, G, parity, mu, h, U);
         load_transform_d<TG, RECON>(gtrans, G, parity ^ 1u, forward_index(G, s, mu), Gf);
@@ -547,32 +548,34 @@ __global__ void apply_transform_kernel(const TG* __restrict__ gtrans, const TS* 
 }
 
 template <typename TG, typename TS, typename TD>
-static cudaError_t apply_run(int recon, const void* gtrans, const void* src, void* dst, const Geom& G, cudaStream_t st)
+static cudaError_t apply_run(int recon, const void* gtrans, const void* src, void* dst, const Geom& G, int mu_begin, int mu_end,
+                             cudaStream_t st)
 {
     const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
     if (recon == 12)
-        apply_transform_kernel<TG, TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G);
+        apply_transform_kernel<TG, TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G, mu_begin, mu_end);
     else
-        apply_transform_kernel<TG, TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G);
+        apply_transform_kernel<TG, TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G, mu_begin, mu_end);
     return cudaGetLastError();
 }
 
 template <typename TG>
 static cudaError_t apply_prec(int src_precision, int dst_precision, int recon, const void* gtrans, const void* src, void* dst,
-                              const Geom& G, cudaStream_t st)
+                              const Geom& G, int mu_begin, int mu_end, cudaStream_t st)
 {
     if (src_precision == PREC_F64)
-        return dst_precision == PREC_F64 ? apply_run<TG, double, double>(recon, gtrans, src, dst, G, st)
-                                         : apply_run<TG, double, float>(recon, gtrans, src, dst, G, st);
-    return dst_precision == PREC_F64 ? apply_run<TG, float, double>(recon, gtrans, src, dst, G, st)
-                                     : apply_run<TG, float, float>(recon, gtrans, src, dst, G, st);
+        return dst_precision == PREC_F64 ? apply_run<TG, double, double>(recon, gtrans, src, dst, G, mu_begin, mu_end, st)
+                                         : apply_run<TG, double, float>(recon, gtrans, src, dst, G, mu_begin, mu_end, st);
+    return dst_precision == PREC_F64 ? apply_run<TG, float, double>(recon, gtrans, src, dst, G, mu_begin, mu_end, st)
+                                     : apply_run<TG, float, float>(recon, gtrans, src, dst, G, mu_begin, mu_end, st);
 }
 
 cudaError_t launch_apply_transform(int g_precision, int src_precision, int dst_precision, int recon,
-                                   const void* gtrans, const void* src, void* dst, const Geom& G, cudaStream_t st)
+                                   const void* gtrans, const void* src, void* dst, const Geom& G,
+                                   int mu_begin, int mu_end, cudaStream_t st)
 {
-    return g_precision == PREC_F64 ? apply_prec<double>(src_precision, dst_precision, recon, gtrans, src, dst, G, st)
-                                   : apply_prec<float>(src_precision, dst_precision, recon, gtrans, src, dst, G, st);
+    return g_precision == PREC_F64 ? apply_prec<double>(src_precision, dst_precision, recon, gtrans, src, dst, G, mu_begin, mu_end, st)
+                                   : apply_prec<float>(src_precision, dst_precision, recon, gtrans, src, dst, G, mu_begin, mu_end, st);
 }
 
 // ------------------------------------------------------------------------------- Philox KAT

@@ -13,6 +13,8 @@ enum { PREC_F32 = 0, PREC_F64 = 1 };
 struct SweepArgs {
     void* links;            // internal field of the chosen precision
     void* gtrans;           // accumulated transformation of the same precision, or NULL
+    int defer_temporal;     // Coulomb: with gtrans, leave the temporal links to gf_coulomb_finish
+    const uint8_t* slice_active;   // per time slice, 0 = frozen; NULL = all active
     Geom G;
     uint32_t parity;        // active parity
     int mu0;                // first direction entering K: 0 Landau, 1 Coulomb
@@ -54,8 +56,10 @@ cudaError_t launch_transform_unpack(int precision, int recon, const void* gtrans
                                     int canonical_is_f64, cudaStream_t st);
 cudaError_t launch_transform_identity(int precision, int recon, void* gtrans, const Geom& G, cudaStream_t st);
 // dst_mu(x) = G(x) src_mu(x) G(x+mu)^dagger in fp64 (eq. 3); src may alias dst
+// only the directions mu_begin <= mu < mu_end are transformed
 cudaError_t launch_apply_transform(int g_precision, int src_precision, int dst_precision, int recon,
-                                   const void* gtrans, const void* src, void* dst, const Geom& G, cudaStream_t st);
+                                   const void* gtrans, const void* src, void* dst, const Geom& G,
+                                   int mu_begin, int mu_end, cudaStream_t st);
 cudaError_t launch_philox(int n, const uint32_t* ctr, const uint32_t* key, uint32_t* out, cudaStream_t st);
 
 }  // namespace gf

@@ -140,6 +140,16 @@ class GaugeField:
     def apply_transform(self, g_precision, src_precision, dst_precision):
         B.gf_apply_transform(self.ctx, g_precision, src_precision, dst_precision)
 
+    # ---- Coulomb specialisation
+    def set_coulomb_mode(self, defer_temporal=False, freeze_slices=False):
+        B.gf_set_coulomb_mode(self.ctx, defer_temporal, freeze_slices)
+
+    def coulomb_finish(self, precision):
+        B.gf_coulomb_finish(self.ctx, precision)
+
+    def set_slice_mask(self, active):
+        B.gf_set_slice_mask(self.ctx, active)
+
     def cast(self, from_precision, to_precision):
         B.gf_cast(self.ctx, from_precision, to_precision)
 
