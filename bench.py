@@ -224,6 +224,35 @@ def run_ours(args):
             variants[name] = {"site_updates_per_s": r["value"], "gflops_nominal": r["value"] * FLOP_PER_SITE_UPDATE / 1e9,
                               "roofline_GBs": r["roofline"]["achieved"], "roofline_frac": r["roofline"]["frac"]}
 
+    # Time to solution (BASELINE.json configs[2]: "fp32, mixed and fp64"): gf_fix_until to theta < 1e-12 on the
+    # same 32^4 input, theta every 10 iterations.  Context for the SP/MP/DP reading of the metric, not the headline.
+    fixes = {}
+    if not args.no_fix:
+        runs = [("f64", gf.GF_F64, None, 18), ("mixed_handoff_1e-6", gf.GF_MIXED, 1e-6, 18),
+                ("mixed_exact_handoff_1e-10", gf.GF_MIXED_EXACT, 1e-10, 18), ("f64_recon12", gf.GF_F64, None, 12),
+                ("mixed_exact_handoff_1e-10_recon12", gf.GF_MIXED_EXACT, 1e-10, 12)]
+        for name, mode, handoff, recon in runs:
+            fld = gf.GaugeField(DIMS, recon=recon, precisions=("f64",) if mode == gf.GF_F64 else ("f64", "f32"), device=dev)
+            fld.pack(U64, gf.GF_F64)
+            if mode == gf.GF_MIXED:
+                fld.pack(U64.to(torch.complex64), gf.GF_F32)
+            if mode == gf.GF_MIXED_EXACT:
+                fld.attach_transform(("f64", "f32"))
+            if handoff:
+                fld.set_mixed_handoff(handoff)
+            P0 = fld.plaquette(gf.GF_F64)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            rc, it, th = fld.fix_until(gf.GF_OVERRELAX, OMEGA, 0.0, mode, 1e-12, 50000, 10)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            fixes[name] = {"converged": rc == gf.GF_OK, "iterations": it, "theta": th, "seconds": ms * 1e-3,
+                           "site_updates_per_s": V * it / (ms * 1e-3), "plaquette_drift": fld.plaquette(gf.GF_F64) - P0}
+            fld.close()
+            del fld
+            torch.cuda.empty_cache()
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(U64.cpu().numpy(), budget_s=12.0)
@@ -241,7 +270,7 @@ def run_ours(args):
                        "parallelism": "replicas only (one lattice per GPU)" if world > 1 else "single GPU"},
             "gflops_nominal": main["value"] * FLOP_PER_SITE_UPDATE / 1e9,
             "gpu_launches": main["gpu_launches"], "clocks": main["clocks"], "e2e": main["e2e"],
-            "roofline": main["roofline"], "cpu_baseline": cpu, "variants": variants,
+            "roofline": main["roofline"], "cpu_baseline": cpu, "variants": variants, "fix_until_theta_1e-12": fixes,
             "final_F": main["final_F"], "final_theta": main["final_theta"],
         }
         print(json.dumps(line), flush=True)
@@ -317,6 +346,7 @@ def main():
     ap.add_argument("--check", type=int, default=10, help="F/theta reduction every CHECK iterations")
     ap.add_argument("--e2e-lanes", type=int, default=4, help="lattices in flight in the end-to-end pipeline")
     ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--no-fix", action="store_true", help="skip the time-to-solution runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -203,6 +203,13 @@ int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2);
  * precision), measured on B200.  Results do not depend on it beyond the summation order inside K. */
 int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_threads);
 
+/* Mixed precision (GF_MIXED, GF_MIXED_EXACT): the fp32 phase of gf_fix_until runs until
+ * theta < max(theta_target, theta_handoff).  Default 1e-6 (BASELINE.json configs[2]).  fp32 sweeps
+ * keep lowering theta down to about 1e-11 (measured at 32^4), so with GF_MIXED_EXACT, whose result
+ * does not inherit the fp32 rounding, a later hand-off moves most of the run to the cheaper sweeps.
+ * A hand-off below what fp32 can reach makes the fp32 phase run to max_iter. */
+int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff);
+
 /* Order in which the blocks of consecutive gf_sweep launches walk the lattice: 1 (default) =
  * zigzag, every other half-sweep runs from the last site to the first, so that a launch starts on
  * the links the previous one touched last and finds them in the L2 cache; 0 = always ascending.

@@ -31,6 +31,7 @@ struct gf_ctx {
     uint8_t* dev_mask;          // workspace: one byte per time slice, 0 = frozen
     uint8_t* host_mask;         // pinned copy
     int mask_on;                // the sweeps consult dev_mask
+    double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
     double* workspace;
     double* partials;           // workspace: per-block partial sums
     double* slice_out;          // workspace: 2 doubles per time slice
@@ -159,6 +160,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->block[PREC_F32] = c->block[PREC_F64] = 0;
     c->solver_mode = GF_SOLVER_AUTO;
     c->zigzag = 1;
+    c->handoff = 1e-6;
 
     if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt) != cudaSuccess) {
         cudaGetLastError();
@@ -444,7 +446,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
     int it = 0;
     double theta = -1.0;
     if (precision == GF_MIXED) {
-        const double t32 = theta_target > 1e-6 ? theta_target : 1e-6;
+        const double t32 = theta_target > ctx->handoff ? theta_target : ctx->handoff;
         rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta);
         if (rc < 0) return rc;
         int e = gf_cast(ctx, GF_F32, GF_F64);
@@ -462,7 +464,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
         int e = gf_cast(ctx, GF_F64, GF_F32);
         if (e == GF_OK) e = gf_transform_identity(ctx, GF_F32);
         if (e != GF_OK) return e;
-        const double t32 = theta_target > 1e-6 ? theta_target : 1e-6;
+        const double t32 = theta_target > ctx->handoff ? theta_target : ctx->handoff;
         rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta);
         if (rc < 0) return rc;
         e = gf_transform_cast(ctx, GF_F32, GF_F64);
@@ -734,6 +736,14 @@ extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int
         return fail(ctx, GF_EINVAL, "lanes must be 0,1,2,4 and block 0 or 64..512 (power of two)");
     ctx->lanes[precision] = lanes_per_site;
     ctx->block[precision] = block_threads;
+    return GF_OK;
+}
+
+extern "C" int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff)
+{
+    if (!ctx) return GF_EINVAL;
+    if (!(theta_handoff > 0.0)) return fail(ctx, GF_EINVAL, "the hand-off theta must be positive");
+    ctx->handoff = theta_handoff;
     return GF_OK;
 }
 

@@ -159,5 +159,8 @@ class GaugeField:
     def set_solver_precision(self, solver_precision):
         B.gf_set_solver_precision(self.ctx, solver_precision)
 
+    def set_mixed_handoff(self, theta_handoff):
+        B.gf_set_mixed_handoff(self.ctx, theta_handoff)
+
     def set_traversal(self, zigzag):
         B.gf_set_traversal(self.ctx, zigzag)

@@ -164,3 +164,25 @@ def test_mixed_exact_fix_is_gauge_equivalent_to_the_input_at_fp64_accuracy(cuda_
     assert rc2 == gf.GF_OK and abs(it - it2) <= 0.2 * it2 + 20
     fld.close()
     fld2.close()
+
+
+def test_mixed_handoff_knob(cuda_device):
+    """gf_set_mixed_handoff: a later hand-off moves iterations into the fp32 phase; GF_MIXED_EXACT still
+    returns a field gauge equivalent to the input at fp64 accuracy."""
+    dims = (8, 8, 8, 8)
+    U = gi.smooth_random_gauge(dims, 0.5, 1234)
+    fld = gf.GaugeField(dims, precisions=("f32", "f64"), device=cuda_device)
+    fld.attach_transform(("f64", "f32"))
+    assert gf.binding.lib.gf_set_mixed_handoff(fld.ctx, 0.0) == gf.GF_EINVAL
+    fld.set_mixed_handoff(1e-10)
+    fld.pack(to_device(U, "f64", cuda_device), gf.GF_F64)
+    P0 = fld.plaquette(gf.GF_F64)
+    c0 = gf.gf_launch_count(fld.ctx)
+    rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_MIXED_EXACT, 1e-12, 20000, 10)
+    assert rc == gf.GF_OK and th < 1e-12
+    assert abs(fld.plaquette(gf.GF_F64) - P0) < 1e-13
+    Ug = fld.unpack(gf.GF_F64, torch.complex128).cpu().numpy()
+    G = fld.transform(gf.GF_F64).cpu().numpy()
+    assert np.abs(oracle.apply_transform(U, np.ascontiguousarray(G), dims) - Ug).max() < 1e-11
+    assert oracle.theta(np.ascontiguousarray(Ug), dims) < 1.1e-12
+    fld.close()
