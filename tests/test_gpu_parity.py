@@ -352,3 +352,50 @@ def _sampled_site_check(dev, dims, prec, recon, seed, nsamples):
     du, dd = fld.unitarity(PREC[prec])
     assert du < (1e-12 if prec == "f64" else 1e-5)
     fld.close()
+
+
+# ------------------------------------------------------------------------- out-of-bounds writes
+
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 6, 6, 6), (6, 2, 4, 2), (4, 6, 8, 10)])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_no_writes_outside_the_lent_buffers(cuda_device, dims, prec, recon):
+    """compute-sanitizer is closed on this pool: the link, transformation and workspace buffers are
+    carved out of larger allocations with 0xA5 guard zones on both sides; every kernel family runs on
+    ragged lattices with every lane count and the guards must come back untouched."""
+    from paper_1305_3440_b200 import binding as B
+    guard = 1 << 16
+    nbytes = [B.gf_storage_bytes(dims, PREC[prec], recon), B.gf_transform_bytes(dims, PREC[prec], recon),
+              B.gf_workspace_bytes(dims)]
+    bufs = [torch.full((n + 2 * guard,), 0xA5, dtype=torch.uint8, device=cuda_device) for n in nbytes]
+    ptrs = [b.data_ptr() + guard for b in bufs]
+    assert all(p % 16 == 0 for p in ptrs)
+    links = (ptrs[0], 0) if prec == "f64" else (0, ptrs[0])
+    ctx = B.gf_init_lattice(dims, gf.GF_COULOMB, recon, links[0], links[1], ptrs[2],
+                            torch.cuda.current_stream().cuda_stream, 3)
+    U = to_device(gi.smooth_random_gauge(dims, 0.5, 2), prec, cuda_device)
+    out = torch.empty_like(U)
+    B.gf_pack(ctx, U.data_ptr(), prec == "f64", PREC[prec])
+    B.gf_set_transform(ctx, ptrs[1] if prec == "f64" else 0, 0 if prec == "f64" else ptrs[1])
+    B.gf_transform_identity(ctx, PREC[prec])
+    for defer in (0, 1):
+        B.gf_set_coulomb_mode(ctx, defer, 0)
+        for lanes in (1, 2, 4):
+            B.gf_set_tuning(ctx, PREC[prec], lanes, 64)
+            for parity in (0, 1):
+                B.gf_sweep(ctx, parity, gf.GF_STOCHASTIC, 1.0, 0.5, PREC[prec])
+        B.gf_set_slice_mask(ctx, [1, 0] * (dims[0] // 2))
+        B.gf_sweep(ctx, 0, gf.GF_OVERRELAX, 1.5, 0.0, PREC[prec])
+        B.gf_set_slice_mask(ctx, None)
+        B.gf_measure(ctx, PREC[prec], dims[0])
+    B.gf_coulomb_finish(ctx, PREC[prec])
+    B.gf_apply_transform(ctx, PREC[prec], PREC[prec], PREC[prec])
+    B.gf_reunitarize(ctx, PREC[prec])
+    B.gf_plaquette(ctx, PREC[prec])
+    B.gf_unitarity(ctx, PREC[prec])
+    B.gf_unpack(ctx, out.data_ptr(), prec == "f64", PREC[prec])
+    torch.cuda.synchronize()
+    B.gf_destroy(ctx)
+    assert torch.isfinite(torch.view_as_real(out)).all()
+    for b, n in zip(bufs, nbytes):
+        assert bool((b[:guard] == 0xA5).all()) and bool((b[guard + n:] == 0xA5).all())
