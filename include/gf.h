@@ -181,6 +181,34 @@ int gf_set_coulomb_mode(gf_ctx* ctx, int defer_temporal, int freeze_slices);
 int gf_coulomb_finish(gf_ctx* ctx, int precision);
 int gf_set_slice_mask(gf_ctx* ctx, const uint8_t* host_active);
 
+/* ---- Slab decomposition along t (the paper's multi-GPU scheme, PAPER.md:98-117,
+ * re-done over peer memory).  A lattice of nranks * N_t time slices is cut into nranks slabs of N_t
+ * slices, one context (one GPU) each; dims given to gf_init_lattice are the LOCAL ones.  The only
+ * data a slab shares with a neighbour are the temporal links U_0 of its last slice: the sites of the
+ * first slice of the slab above read and write them IN PLACE through dev_prev_links_* (a pointer
+ * into the neighbour's link field: a peer mapping over NVLink, CUDA IPC between processes, or plain
+ * device memory when several slabs live on one GPU) -- no halo buffers, no exchange step, no
+ * collective.  dev_next_links_* is read by gf_plaquette only.
+ *
+ * Ordering: every link operation (gf_pack, gf_unpack, gf_sweep, gf_measure/gf_functional/gf_theta,
+ * gf_plaquette, gf_unitarity, gf_reunitarize, gf_cast) is numbered per slab; operation n of a slab
+ * starts when both neighbours have completed their operation n-1.  Completion counts live in one
+ * 32-bit device word per slab (dev_flag_*, zero-initialised by the caller, 4-byte aligned, the
+ * neighbours' words mapped like their fields) and are written and awaited with stream memory
+ * operations (cuStreamWriteValue32 / cuStreamWaitValue32): no kernel spins, the host never blocks.
+ * ALL SLABS MUST ISSUE THE SAME SEQUENCE OF OPERATIONS.
+ *
+ * Results: links are those of the undivided lattice (sweep-by-sweep parity with the oracle; Philox
+ * uses the global site index).  Landau gf_measure / gf_functional / gf_theta / gf_plaquette return
+ * this slab's SHARE of the global value (local sum over the global normalisation): the caller adds
+ * the slabs up (one scalar all-reduce).  Coulomb values are per local time slice.  Not available on
+ * slabs (GF_ESTATE): gf_fix_until (the caller iterates and reduces theta), the transformation field,
+ * deferred temporal links.  nranks = 1 restores the single-lattice behaviour.
+ * Errors: GF_EINVAL (rank, missing pointers, alignment, global volume >= 2^32), GF_ESTATE, GF_ECUDA. */
+int gf_set_slab(gf_ctx* ctx, int rank, int nranks, void* dev_prev_links_f64, void* dev_prev_links_f32,
+                void* dev_next_links_f64, void* dev_next_links_f32, uint32_t* dev_flag_own,
+                uint32_t* dev_flag_prev, uint32_t* dev_flag_next);
+
 /* Sets the Philox key and the half-sweep counter (checkpoint/resume: the RNG state is just these). */
 int gf_set_rng(gf_ctx* ctx, uint64_t seed, uint32_t half_sweep_counter);
 int gf_get_counter(const gf_ctx* ctx, uint32_t* half_sweep_counter_out);

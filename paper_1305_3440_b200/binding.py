@@ -56,6 +56,7 @@ def _load():
         "gf_set_coulomb_mode": (i32, [vp, i32, i32]),
         "gf_coulomb_finish": (i32, [vp, i32]),
         "gf_set_slice_mask": (i32, [vp, C.c_char_p]),
+        "gf_set_slab": (i32, [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp]),
         "gf_set_rng": (i32, [vp, u64, u32]),
         "gf_get_counter": (i32, [vp, C.POINTER(u32)]),
         "gf_reunitarize": (i32, [vp, i32]),
@@ -81,7 +82,7 @@ lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
            "gf_sweep gf_functional gf_theta gf_measure gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
-           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
+           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
 
 
@@ -237,6 +238,11 @@ def gf_set_slice_mask(ctx, active, check=True):
     """active: sequence of Nt truth values, or None for all slices."""
     buf = None if active is None else bytes(1 if a else 0 for a in active)
     return _rc(ctx, lib.gf_set_slice_mask(ctx, buf), check)
+
+
+def gf_set_slab(ctx, rank, nranks, prev_f64, prev_f32, next_f64, next_f32, flag_own, flag_prev, flag_next, check=True):
+    return _rc(ctx, lib.gf_set_slab(ctx, int(rank), int(nranks), prev_f64 or None, prev_f32 or None, next_f64 or None,
+                                    next_f32 or None, flag_own or None, flag_prev or None, flag_next or None), check)
 
 
 def gf_plaquette(ctx, precision, check=True):

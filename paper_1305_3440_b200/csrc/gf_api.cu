@@ -1,6 +1,8 @@
 // gf_api.cu -- the C ABI of include/gf.h: argument checks, the context, the host-side fix loop
 // and the mixed-precision hand-off.  No arithmetic of the method runs on the
 // host: every step is one of the kernels in gf_sweep.cu / gf_aux.cu.
+#include <cuda.h>
+
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -32,6 +34,14 @@ struct gf_ctx {
     uint8_t* host_mask;         // pinned copy
     int mask_on;                // the sweeps consult dev_mask
     double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
+    // slab decomposition along t (gf_set_slab): this context holds N_t local slices of a lattice nranks times as long
+    int slab_rank, slab_n;
+    void* prev_links[2];        // field of the slab below (per precision); NULL = own (one slab)
+    void* next_links[2];        // field of the slab above
+    uint32_t *flag_own, *flag_prev, *flag_next;   // device words: number of operations completed by that slab
+    uint32_t epoch;             // operations this slab has enqueued
+    CUresult (*wait32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+    CUresult (*write32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
     double* workspace;
     double* partials;           // workspace: per-block partial sums
     double* slice_out;          // workspace: 2 doubles per time slice
@@ -161,6 +171,8 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->solver_mode = GF_SOLVER_AUTO;
     c->zigzag = 1;
     c->handoff = 1e-6;
+    c->slab_rank = 0;
+    c->slab_n = 1;
 
     if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt) != cudaSuccess) {
         cudaGetLastError();
@@ -189,14 +201,92 @@ static int check_prec(gf_ctx* ctx, int precision)
     return GF_OK;
 }
 
+// Slab decomposition: every operation that reads or writes links is numbered; operation n of a slab
+// starts when both neighbouring slabs have completed their operation n-1 (they may still be reading
+// or writing the temporal links across the boundary), and publishes its completion.  The waits and
+// writes are stream memory operations (no kernel spins, no host synchronisation).
+static int slab_begin(gf_ctx* ctx)
+{
+    if (ctx->slab_n <= 1) return GF_OK;
+    CUresult r = ctx->wait32((CUstream)ctx->stream, (CUdeviceptr)ctx->flag_prev, ctx->epoch, CU_STREAM_WAIT_VALUE_GEQ);
+    if (r == CUDA_SUCCESS && ctx->flag_next != ctx->flag_prev)
+        r = ctx->wait32((CUstream)ctx->stream, (CUdeviceptr)ctx->flag_next, ctx->epoch, CU_STREAM_WAIT_VALUE_GEQ);
+    if (r != CUDA_SUCCESS) return fail(ctx, GF_ECUDA, "cuStreamWaitValue32 failed (%d)", (int)r);
+    return GF_OK;
+}
+
+static int slab_end(gf_ctx* ctx)
+{
+    if (ctx->slab_n <= 1) return GF_OK;
+    ctx->epoch += 1;
+    CUresult r = ctx->write32((CUstream)ctx->stream, (CUdeviceptr)ctx->flag_own, ctx->epoch, CU_STREAM_WRITE_VALUE_DEFAULT);
+    if (r != CUDA_SUCCESS) return fail(ctx, GF_ECUDA, "cuStreamWriteValue32 failed (%d)", (int)r);
+    return GF_OK;
+}
+
+#define GF_SLAB_BEGIN(ctx)              \
+    do {                                \
+        int rc_ = slab_begin(ctx);      \
+        if (rc_) return rc_;            \
+    } while (0)
+#define GF_SLAB_END(ctx)                \
+    do {                                \
+        int rc_ = slab_end(ctx);        \
+        if (rc_) return rc_;            \
+    } while (0)
+
+extern "C" int gf_set_slab(gf_ctx* ctx, int rank, int nranks, void* dev_prev_links_f64, void* dev_prev_links_f32,
+                           void* dev_next_links_f64, void* dev_next_links_f32, uint32_t* dev_flag_own,
+                           uint32_t* dev_flag_prev, uint32_t* dev_flag_next)
+{
+    if (!ctx) return GF_EINVAL;
+    if (nranks < 1 || rank < 0 || rank >= nranks) return fail(ctx, GF_EINVAL, "bad slab rank %d of %d", rank, nranks);
+    if ((uint64_t)ctx->V * (uint64_t)nranks >= (uint64_t(1) << 32)) return fail(ctx, GF_EINVAL, "global volume must stay below 2^32 sites");
+    if (nranks > 1) {
+        if (!dev_flag_own || !dev_flag_prev || !dev_flag_next) return fail(ctx, GF_EINVAL, "slab flags missing");
+        for (int prec = 0; prec < 2; ++prec) {
+            void* pv = prec == PREC_F64 ? dev_prev_links_f64 : dev_prev_links_f32;
+            void* nx = prec == PREC_F64 ? dev_next_links_f64 : dev_next_links_f32;
+            if (ctx->links[prec] && (!pv || !nx)) return fail(ctx, GF_EINVAL, "neighbour fields missing for precision %d", prec);
+            if (((uintptr_t)pv | (uintptr_t)nx) & 15u) return fail(ctx, GF_EINVAL, "neighbour fields must be 16-byte aligned");
+        }
+        if (ctx->gtrans[0] || ctx->gtrans[1] || ctx->defer_temporal)
+            return fail(ctx, GF_ESTATE, "the transformation field and deferred temporal links are not available on slabs");
+        if (!ctx->wait32) {
+            cudaDriverEntryPointQueryResult q;
+            void *w = nullptr, *wr = nullptr;
+            if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &w, cudaEnableDefault, &q) != cudaSuccess || !w ||
+                cudaGetDriverEntryPoint("cuStreamWriteValue32", &wr, cudaEnableDefault, &q) != cudaSuccess || !wr) {
+                cudaGetLastError();
+                return fail(ctx, GF_ECUDA, "stream memory operations are not available");
+            }
+            ctx->wait32 = reinterpret_cast<decltype(ctx->wait32)>(w);
+            ctx->write32 = reinterpret_cast<decltype(ctx->write32)>(wr);
+        }
+    }
+    ctx->slab_rank = rank;
+    ctx->slab_n = nranks;
+    ctx->prev_links[PREC_F64] = nranks > 1 ? dev_prev_links_f64 : nullptr;
+    ctx->prev_links[PREC_F32] = nranks > 1 ? dev_prev_links_f32 : nullptr;
+    ctx->next_links[PREC_F64] = nranks > 1 ? dev_next_links_f64 : nullptr;
+    ctx->next_links[PREC_F32] = nranks > 1 ? dev_next_links_f32 : nullptr;
+    ctx->flag_own = dev_flag_own;
+    ctx->flag_prev = dev_flag_prev;
+    ctx->flag_next = dev_flag_next;
+    ctx->epoch = 0;
+    return GF_OK;
+}
+
 extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision)
 {
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     ctx->pending[precision] = 0;      // the field is overwritten: nothing left to apply
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_pack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_pack");
+    GF_SLAB_END(ctx);
     ctx->launches += 1;
     return GF_OK;
 }
@@ -208,8 +298,10 @@ extern "C" int gf_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64,
     rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_unpack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_unpack");
+    GF_SLAB_END(ctx);
     ctx->launches += 1;
     return GF_OK;
 }
@@ -277,6 +369,8 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.gtrans = ctx->gtrans[precision];
     a.defer_temporal = ctx->defer_temporal;
     a.slice_active = ctx->mask_on ? ctx->dev_mask : nullptr;
+    a.prev_links = ctx->prev_links[precision];
+    a.site_offset = (uint32_t)((uint64_t)ctx->slab_rank * ctx->V);
     a.G = ctx->G;
     a.parity = (uint32_t)parity;
     a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
@@ -292,8 +386,10 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, &lanes, &block);
     if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
     if (ctx->block[precision]) block = ctx->block[precision];
+    GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, lanes, block, a, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_sweep launch");
+    GF_SLAB_END(ctx);
     ctx->counter += 1;
     ctx->sweeps += 1;
     ctx->launches += 1;
@@ -314,9 +410,11 @@ extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double 
 static int measure_to_host(gf_ctx* ctx, int precision)
 {
     const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
-    cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->G, mu0, ctx->mg, ctx->partials,
-                                   ctx->slice_out, ctx->stream);
+    GF_SLAB_BEGIN(ctx);
+    cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0, ctx->mg,
+                                   ctx->partials, ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
+    GF_SLAB_END(ctx);
     ctx->launches += 2;
     e = cudaMemcpyAsync(ctx->host_pinned, ctx->slice_out, sizeof(double) * 2 * ctx->dims[0], cudaMemcpyDeviceToHost, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
@@ -346,8 +444,9 @@ static double finish_measure(const gf_ctx* ctx, double* host_F, double* host_the
         F += s[2 * t];
         th += s[2 * t + 1];
     }
-    F /= 3.0 * 4.0 * (double)ctx->V;
-    th /= 3.0 * (double)ctx->V;
+    // on slabs: this slab's share of the global sums (the caller adds the slabs up)
+    F /= 3.0 * 4.0 * (double)ctx->V * ctx->slab_n;
+    th /= 3.0 * (double)ctx->V * ctx->slab_n;
     if (host_F) host_F[0] = F;
     if (host_theta) host_theta[0] = th;
     return th;
@@ -438,6 +537,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
     int rc = check_algo(ctx, algo, omega, p);
     if (rc) return rc;
     if (max_iter < 0 || check_every < 1 || !(theta_target >= 0.0)) return fail(ctx, GF_EINVAL, "bad max_iter / check_every / theta_target");
+    if (ctx->slab_n > 1) return fail(ctx, GF_ESTATE, "gf_fix_until needs the whole lattice: on slabs the caller runs the loop and adds up theta");
     if (ctx->defer_temporal && precision == GF_MIXED_EXACT)
         return fail(ctx, GF_ESTATE, "GF_MIXED_EXACT and deferred temporal links both use the transformation buffers");
     if (ctx->defer_temporal && ((precision != GF_F64 && !ctx->gtrans[PREC_F32]) || (precision != GF_F32 && !ctx->gtrans[PREC_F64])))
@@ -518,8 +618,10 @@ extern "C" int gf_reunitarize(gf_ctx* ctx, int precision)
     if (rc) return rc;
     rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
+    GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_cast(precision, precision, ctx->recon, ctx->links[precision], ctx->links[precision], ctx->G, 1, 8, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_reunitarize");
+    GF_SLAB_END(ctx);
     ctx->launches += 1;
     return GF_OK;
 }
@@ -535,9 +637,11 @@ extern "C" int gf_cast(gf_ctx* ctx, int from_precision, int to_precision)
     ctx->pending[to_precision] = 0;
     if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_cast needs two different precisions");
     const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
+    GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_cast(from_precision, to_precision, ctx->recon, ctx->links[from_precision], ctx->links[to_precision],
                                 ctx->G, reproject, 8, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_cast");
+    GF_SLAB_END(ctx);
     ctx->launches += 1;
     return GF_OK;
 }
@@ -547,6 +651,7 @@ extern "C" int gf_set_transform(gf_ctx* ctx, void* dev_g_f64, void* dev_g_f32)
 {
     if (!ctx) return GF_EINVAL;
     if (((uintptr_t)dev_g_f64 | (uintptr_t)dev_g_f32) & 15u) return fail(ctx, GF_EINVAL, "transformation buffers must be 16-byte aligned");
+    if (ctx->slab_n > 1 && (dev_g_f64 || dev_g_f32)) return fail(ctx, GF_ESTATE, "the transformation field is not available on slabs");
     ctx->gtrans[PREC_F64] = dev_g_f64;
     ctx->gtrans[PREC_F32] = dev_g_f32;
     return GF_OK;
@@ -630,6 +735,7 @@ extern "C" int gf_set_coulomb_mode(gf_ctx* ctx, int defer_temporal, int freeze_s
     if (!ctx) return GF_EINVAL;
     if ((defer_temporal != 0 && defer_temporal != 1) || (freeze_slices != 0 && freeze_slices != 1))
         return fail(ctx, GF_EINVAL, "defer_temporal and freeze_slices must be 0 or 1");
+    if (ctx->slab_n > 1 && defer_temporal) return fail(ctx, GF_ESTATE, "deferred temporal links are not available on slabs");
     if (ctx->gauge != GF_COULOMB && (defer_temporal || freeze_slices))
         return fail(ctx, GF_EINVAL, "deferred temporal links and slice freezing exist in Coulomb gauge only");
     if (!defer_temporal) {
@@ -699,13 +805,16 @@ extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)
     rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!host_out) return fail(ctx, GF_EINVAL, "null output");
-    cudaError_t e = launch_plaquette(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);
+    GF_SLAB_BEGIN(ctx);
+    cudaError_t e = launch_plaquette(precision, ctx->recon, ctx->links[precision], ctx->next_links[precision], ctx->G, ctx->mg,
+                                     ctx->partials, ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_plaquette launch");
+    GF_SLAB_END(ctx);
     rc = slices_to_host(ctx, "gf_plaquette copy");
     if (rc) return rc;
     double sum = 0.0;
     for (int t = 0; t < ctx->dims[0]; ++t) sum += ctx->host_pinned[2 * t];
-    *host_out = sum / (6.0 * 3.0 * (double)ctx->V);
+    *host_out = sum / (6.0 * 3.0 * (double)ctx->V * ctx->slab_n);
     return GF_OK;
 }
 
@@ -716,8 +825,10 @@ extern "C" int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2)
     rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!host_out2) return fail(ctx, GF_EINVAL, "null output");
+    GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_unitarity(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_unitarity launch");
+    GF_SLAB_END(ctx);
     rc = slices_to_host(ctx, "gf_unitarity copy");
     if (rc) return rc;
     host_out2[0] = host_out2[1] = 0.0;

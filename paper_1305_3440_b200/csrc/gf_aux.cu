@@ -82,8 +82,8 @@ __device__ __forceinline__ size_t partial_slot(const MeasureGrid& mg)
 // (eq. 4); as A is linear in U, Delta = traceless[(M - M^dagger)/(2i)] with
 // M = sum_mu (U_mu(x) - U_mu(x-mu)).  Accumulation in fp64 whatever the storage precision.
 template <typename T, int RECON>
-__global__ void measure_kernel(const T* __restrict__ links, const Geom G, const int mu0, const MeasureGrid mg,
-                               double* __restrict__ partials)
+__global__ void measure_kernel(const T* __restrict__ links, const T* __restrict__ prev_links, const Geom G, const int mu0,
+                               const MeasureGrid mg, double* __restrict__ partials)
 {
     uint32_t parity;
     Site s;
@@ -97,7 +97,8 @@ __global__ void measure_kernel(const T* __restrict__ links, const Geom G, const 
         if (mu < mu0) continue;
         T Uf[18], Ub[18];
         load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, s.h, Uf);
-        load_link<RECON>(links + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, backward_index(G, s, mu), Ub);
+        const T* back = (mu == 0 && s.c[0] == 0) ? prev_links : links;     // slab below for the first local slice
+        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, backward_index(G, s, mu), Ub);
         if (RECON == 12) {
             reconstruct_row2(Uf);
             reconstruct_row2(Ub);
@@ -159,8 +160,8 @@ __device__ __forceinline__ void mul_full(const double (&A)[18], const double (&B
 
 // sum_{mu<nu} Re tr[U_mu(x) U_nu(x+mu) U_mu(x+nu)^dagger U_nu(x)^dagger]   (diagnostic)
 template <typename T, int RECON>
-__global__ void plaquette_kernel(const T* __restrict__ links, const Geom G, const MeasureGrid mg,
-                                 double* __restrict__ partials)
+__global__ void plaquette_kernel(const T* __restrict__ links, const T* __restrict__ next_links, const Geom G,
+                                 const MeasureGrid mg, double* __restrict__ partials)
 {
     uint32_t parity;
     Site s;
@@ -170,7 +171,8 @@ __global__ void plaquette_kernel(const T* __restrict__ links, const Geom G, cons
         for (int nu = mu + 1; nu < 4; ++nu) {
             double A[18], B[18], C[18], D[18];
             load_full_d<T, RECON>(links, G, parity, mu, s.h, A);
-            load_full_d<T, RECON>(links, G, parity ^ 1u, nu, forward_index(G, s, mu), B);
+            // x + mu_hat leaves the slab through its last time slice only for mu = 0
+            load_full_d<T, RECON>((mu == 0 && s.c[0] + 1u == G.nt) ? next_links : links, G, parity ^ 1u, nu, forward_index(G, s, mu), B);
             mul_full(A, B, C, false);
             load_full_d<T, RECON>(links, G, parity ^ 1u, mu, forward_index(G, s, nu), A);
             mul_full(C, A, D, true);
@@ -229,20 +231,22 @@ static cudaError_t dispatch(int precision, int recon, Args... args)
 static dim3 measure_dims(const Geom& G, const MeasureGrid& mg) { return dim3(2u * mg.bpp, G.nt, 1); }
 
 template <typename T, int RECON> struct MeasureLauncher {
-    static cudaError_t run(const void* links, const Geom& G, int mu0, const MeasureGrid& mg, double* partials,
+    static cudaError_t run(const void* links, const void* prev_links, const Geom& G, int mu0, const MeasureGrid& mg, double* partials,
                            double* slice_out, cudaStream_t st)
     {
-        measure_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mu0, mg, partials);
+        measure_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
+                                                                           static_cast<const T*>(prev_links ? prev_links : links), G, mu0, mg, partials);
         reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
         return cudaGetLastError();
     }
 };
 
 template <typename T, int RECON> struct PlaquetteLauncher {
-    static cudaError_t run(const void* links, const Geom& G, const MeasureGrid& mg, double* partials,
+    static cudaError_t run(const void* links, const void* next_links, const Geom& G, const MeasureGrid& mg, double* partials,
                            double* slice_out, cudaStream_t st)
     {
-        plaquette_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mg, partials);
+        plaquette_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
+                                                                             static_cast<const T*>(next_links ? next_links : links), G, mg, partials);
         reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
         return cudaGetLastError();
     }
@@ -258,16 +262,16 @@ template <typename T, int RECON> struct UnitarityLauncher {
     }
 };
 
-cudaError_t launch_measure(int precision, int recon, const void* links, const Geom& G, int mu0,
+cudaError_t launch_measure(int precision, int recon, const void* links, const void* prev_links, const Geom& G, int mu0,
                            const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
 {
-    return dispatch<MeasureLauncher>(precision, recon, links, G, mu0, mg, partials, slice_out, st);
+    return dispatch<MeasureLauncher>(precision, recon, links, prev_links, G, mu0, mg, partials, slice_out, st);
 }
 
-cudaError_t launch_plaquette(int precision, int recon, const void* links, const Geom& G,
+cudaError_t launch_plaquette(int precision, int recon, const void* links, const void* next_links, const Geom& G,
                              const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
 {
-    return dispatch<PlaquetteLauncher>(precision, recon, links, G, mg, partials, slice_out, st);
+    return dispatch<PlaquetteLauncher>(precision, recon, links, next_links, G, mg, partials, slice_out, st);
 }
 
 cudaError_t launch_unitarity(int precision, int recon, const void* links, const Geom& G,

@@ -15,6 +15,8 @@ struct SweepArgs {
     void* gtrans;           // accumulated transformation of the same precision, or NULL
     int defer_temporal;     // Coulomb: with gtrans, leave the temporal links to gf_coulomb_finish
     const uint8_t* slice_active;   // per time slice, 0 = frozen; NULL = all active
+    void* prev_links;       // slab below (same precision and layout), or NULL = this field (periodic)
+    uint32_t site_offset;   // global site index of the slab's first site
     Geom G;
     uint32_t parity;        // active parity
     int mu0;                // first direction entering K: 0 Landau, 1 Coulomb
@@ -36,9 +38,10 @@ struct MeasureGrid {
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);
 bool sweep_config_valid(int lanes, int block);
 
-cudaError_t launch_measure(int precision, int recon, const void* links, const Geom& G, int mu0,
+// prev_links / next_links: the fields of the slabs below / above in t (NULL = this field, periodic)
+cudaError_t launch_measure(int precision, int recon, const void* links, const void* prev_links, const Geom& G, int mu0,
                            const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
-cudaError_t launch_plaquette(int precision, int recon, const void* links, const Geom& G,
+cudaError_t launch_plaquette(int precision, int recon, const void* links, const void* next_links, const Geom& G,
                              const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
 cudaError_t launch_unitarity(int precision, int recon, const void* links, const Geom& G,
                              const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);

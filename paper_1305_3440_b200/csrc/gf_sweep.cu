@@ -21,6 +21,9 @@ template <typename T, typename TK> struct SweepConsts {
     T* links;
     T* gtrans;              // MODE > 0: the accumulated transformation G[parity][chunk][h], else unused
     const uint8_t* slice_active;   // Coulomb slice freezing: sites of slices with 0 are skipped; NULL = all active
+    T* prev_links;          // slab decomposition in t: field holding U_0(x-0) of the sites with local t = 0 (the rank
+                            // below; this rank's own field when there is one slab, which is the periodic wrap)
+    uint32_t site_offset;   // global index of this slab's first site (Philox counter word 0)
     Geom G;
     uint32_t parity;
     int mu0, algo;
@@ -93,7 +96,9 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
             continue;
         }
         load_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
-        load_link<RECON>(P.links + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
+        // the temporal link below the first local time slice belongs to the slab below
+        const T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
+        load_link<RECON>(back + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
     }
     if (RECON == 12) {
 #pragma unroll
@@ -130,7 +135,7 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     bool sq0 = false, sq1 = false, sq2 = false;
     if (P.algo == ALGO_STOCHASTIC) {
         uint32_t w[4];
-        philox4x32_10(2u * h + s.xodd, 0u, P.counter, 0u, P.key0, P.key1, w);
+        philox4x32_10(P.site_offset + 2u * h + s.xodd, 0u, P.counter, 0u, P.key0, P.key1, w);
         sq0 = (double)(w[0] >> 8) * (1.0 / 16777216.0) < P.p;
         sq1 = (double)(w[1] >> 8) * (1.0 / 16777216.0) < P.p;
         sq2 = (double)(w[2] >> 8) * (1.0 / 16777216.0) < P.p;
@@ -153,7 +158,8 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
         mul_g_U<ROWS>(g, Uf[d], out);
         store_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, out);
         mul_U_gdag<ROWS>(Ub[d], g, out);
-        store_link<RECON>(P.links + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
+        T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
+        store_link<RECON>(back + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
     }
     if (ACC && j == 0) {
         T* blk = P.gtrans + (size_t)P.parity * RECON * G.Vh;
@@ -172,6 +178,8 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     P.links = static_cast<T*>(a.links);
     P.gtrans = static_cast<T*>(a.gtrans);
     P.slice_active = a.slice_active;
+    P.prev_links = a.prev_links ? static_cast<T*>(a.prev_links) : P.links;
+    P.site_offset = a.site_offset;
     P.G = a.G;
     P.parity = a.parity;
     P.mu0 = a.mu0;
