@@ -116,12 +116,16 @@ class SlabRank:
     """One slab per process (rank r of torch.distributed owns slab r, one GPU each)."""
 
     def __init__(self, global_dims, gauge=B.GF_LANDAU, recon=B.GF_RECON18, precisions=("f64",), seed=0, device=None,
-                 group=None):
+                 group=None, _field=None):
         import torch.distributed as dist
         self.dist, self.group = dist, group
         self.rank, self.nslabs = dist.get_rank(group), dist.get_world_size(group)
         self.gauge = gauge
         self.dims = local_dims(global_dims, self.nslabs)
+        if _field is not None:
+            # host-logic tests (gloo, no GPU): a stand-in with iterate() / measure(); nothing is wired
+            self.field, self.device = _field, torch.device("cpu")
+            return
         self.device = torch.device(device if device is not None else "cuda:%d" % torch.cuda.current_device())
         self.field = GaugeField(self.dims, gauge=gauge, recon=recon, precisions=precisions, seed=seed, device=self.device)
         self.flag = torch.zeros(4, dtype=torch.int32, device=self.device)
