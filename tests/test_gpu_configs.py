@@ -183,3 +183,102 @@ def test_config5_coulomb_32_3x64_stochastic(cuda_device):
     assert du < 1e-12 and dd < 1e-12
     print("config5: %d iterations, max theta_t = %.3e" % (it, th))
     fld.close()
+
+
+# ------------------------------------------- full-size checks of the SURVEY 8(f) features (NEXT-1..3)
+
+def _gauge_transform_torch(U, G):
+    """eq. 3 on the device with torch ops (test side only): G(x) U_mu(x) G(x+mu)^dagger."""
+    out = torch.empty_like(U)
+    for mu, axis in enumerate((0, 3, 2, 1)):          # canonical axes (t, z, y, x); mu = 0,1,2,3 = t,x,y,z
+        Gf = torch.roll(G, -1, dims=axis)
+        out[..., mu, :, :] = G @ U[..., mu, :, :] @ Gf.conj().transpose(-1, -2)
+    return out
+
+
+@pytest.mark.parametrize("prec,recon", [("f64", 18), ("f32", 12)])
+def test_32_4_accumulated_transformation(cuda_device, prec, recon):
+    """configs[2] size, default launch configuration with accumulation: sampled G(x) against the
+    oracle's single-site g(x) after each half-sweep, and U_n = G U_0 G^dagger over the whole lattice
+    (a property that holds at any size; eq. 3 restated with torch ops)."""
+    dims = (32, 32, 32, 32)
+    U0 = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device).to(CDTYPE[prec])
+    fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
+    fld.pack(U0, PREC[prec])
+    fld.attach_transform((prec,))
+    before = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
+    rng = np.random.default_rng(9)
+    V = before.shape[0]
+    for parity in (0, 1):
+        fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+        G = fld.transform(PREC[prec]).reshape(-1, 3, 3)
+        picked = 0
+        while picked < 32:
+            s = int(rng.integers(0, V))
+            par, back = _site_and_backward(dims, s)
+            if par != parity:
+                continue
+            picked += 1
+            fwd = before[s].cpu().numpy().copy()
+            bwd = np.stack([before[back[mu], mu].cpu().numpy() for mu in range(4)])
+            g = oracle.update_links8(fwd, bwd, oracle.LANDAU, oracle.OVERRELAX, 1.7, 0.0, (0.0, 0.0, 0.0))
+            assert np.abs(G[s].cpu().numpy() - g).max() < LINK_TOL[prec]       # G was the identity before this visit
+        before = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
+    fld.iterate(4, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+    Un = fld.unpack(PREC[prec], torch.complex128)
+    G = fld.transform(PREC[prec], torch.complex128)
+    replay = _gauge_transform_torch(U0.to(torch.complex128), G)
+    assert float((replay - Un).abs().max()) < (1e-12 if prec == "f64" else 2e-5)
+    fld.close()
+
+
+def test_config5_size_deferred_temporal_links_and_freezing(cuda_device):
+    """32^3 x 64 Coulomb, fp64, stochastic p = 0.8: ten iterations with deferred temporal links equal
+    ten plain iterations link by link (same Philox draws); the plaquette survives; a frozen slice is
+    left alone."""
+    dims = (64, 32, 32, 32)
+    U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device)
+    plain = gf.GaugeField(dims, gauge=gf.GF_COULOMB, precisions=("f64",), seed=2013, device=cuda_device)
+    plain.pack(U, gf.GF_F64)
+    P0 = plain.plaquette(gf.GF_F64)
+    plain.iterate(10, gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64)
+    want = plain.unpack(gf.GF_F64)
+    plain.close()
+    fld = gf.GaugeField(dims, gauge=gf.GF_COULOMB, precisions=("f64",), seed=2013, device=cuda_device)
+    fld.attach_transform(("f64",))
+    fld.pack(U, gf.GF_F64)
+    fld.set_coulomb_mode(defer_temporal=True)
+    fld.iterate(10, gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64)
+    got = fld.unpack(gf.GF_F64)                        # finishes the temporal links
+    assert float((got - want).abs().max()) < 1e-11
+    assert abs(fld.plaquette(gf.GF_F64) - P0) < 1e-13
+    mask = [1] * 64
+    mask[5] = mask[40] = 0
+    fld.set_slice_mask(mask)
+    fld.iterate(2, gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64)
+    after = fld.unpack(gf.GF_F64)
+    for t in (5, 40):
+        assert torch.equal(after[t][..., 1:, :, :], got[t][..., 1:, :, :])
+    assert not torch.equal(after[6][..., 1:, :, :], got[6][..., 1:, :, :])
+    assert abs(fld.plaquette(gf.GF_F64) - P0) < 1e-13
+    fld.close()
+
+
+def test_32_4_as_two_slabs_equals_the_undivided_lattice(cuda_device):
+    from paper_1305_3440_b200.slabs import SlabSet
+    dims = (32, 32, 32, 32)
+    U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device)
+    one = gf.GaugeField(dims, precisions=("f64",), seed=7, device=cuda_device)
+    one.pack(U, gf.GF_F64)
+    one.iterate(5, gf.GF_STOCHASTIC, 1.0, 0.5, gf.GF_F64)
+    want = one.unpack(gf.GF_F64)
+    Fw, thw = one.measure(gf.GF_F64)
+    one.close()
+    lat = SlabSet(dims, 2, seed=7, devices=(str(cuda_device),))
+    lat.pack(U, gf.GF_F64)
+    lat.iterate(5, gf.GF_STOCHASTIC, 1.0, 0.5, gf.GF_F64)
+    F, th = lat.measure(gf.GF_F64)
+    got = lat.unpack(gf.GF_F64)
+    assert torch.equal(got, want)                     # same kernels, same order of operations per site: bitwise
+    assert abs(F[0] - Fw[0]) < 1e-13 and abs(th[0] / thw[0] - 1) < 1e-12
+    lat.close()
