@@ -341,8 +341,13 @@ static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
 
 // Launch configuration chosen by measurement on B200 at 32^4 (profiles/r1_tune_32x32x32x32.txt,
 // DESIGN.md "Kernels"): two lanes per site everywhere except fp64 / 12-real (four).
-static void default_tuning(int precision, int recon, int solver_f64, int accumulate, int* lanes, int* block)
+static void default_tuning(int precision, int recon, int solver_f64, int accumulate, int defer, int* lanes, int* block)
 {
+    if (defer && precision == GF_F32) {      // 6 links + G: one lane per site is balanced and fits the registers
+        *lanes = 1;
+        *block = 64;
+        return;
+    }
     if (precision == GF_F64) {
         *lanes = recon == GF_RECON12 ? 4 : 2;
         *block = recon == GF_RECON12 ? 64 : 128;
@@ -383,7 +388,7 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.reverse = ctx->zigzag ? (uint32_t)(ctx->sweeps & 1u) : 0u;
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
     int lanes, block;
-    default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, &lanes, &block);
+    default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, a.gtrans != nullptr && a.defer_temporal, &lanes, &block);
     if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
     if (ctx->block[precision]) block = ctx->block[precision];
     GF_SLAB_BEGIN(ctx);
@@ -495,11 +500,11 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
         for (int k = 0; k < n; ++k) {
             int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
             if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
-            if (e != GF_OK) { *it_io = it; return e; }
+            if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         }
         it += n;
         int e = measure_to_host(ctx, precision);
-        if (e != GF_OK) { *it_io = it; return e; }
+        if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         *theta_out = finish_measure(ctx, nullptr, nullptr);
         if (*theta_out < target) { rc = GF_OK; break; }
         if (freeze) {
@@ -514,7 +519,7 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
                 }
             if (changed) {
                 e = upload_mask(ctx);
-                if (e != GF_OK) { *it_io = it; return e; }
+                if (e != GF_OK) { *it_io = it; ctx->mask_on = 0; return e; }
             }
         }
     }

@@ -65,7 +65,6 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     if (warp * S >= G.Vh) return;                       // warp-uniform
     uint32_t h = warp * S + (lane % S);
     const int j = lane / S;
-    constexpr bool ACC = MODE != MODE_PLAIN;
     bool live = h < G.Vh;
     if (!live) h = G.Vh - 1u;                           // keeps the lane in the shuffles; no store
     const Site s = decode_site(G, h, P.parity);
@@ -74,7 +73,7 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
         if (!__any_sync(0xffffffffu, live)) return;     // the whole warp sits in frozen slices
     }
 
-    if (ACC && j == 0) {
+    if (MODE == MODE_ACC && j == 0) {
         // G(x) is only needed after the links have been written back: start moving it towards L2 now
         const T* gp = P.gtrans + (size_t)P.parity * RECON * G.Vh;
         constexpr int CH = (RECON * (int)sizeof(T)) / 16;      // whole 16-byte chunks (the fp32/18 tail rides along)
@@ -90,9 +89,12 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
         hb[d] = backward_index(G, s, mu);
-        if (MODE == MODE_DEFER && d == 0 && j == 0) {   // mu = 0: the temporal links stay where they are
+        if (MODE == MODE_DEFER && d == 0 && j == 0) {
+            // mu = 0: the temporal links stay where they are; their register slot carries G(x) instead,
+            // loaded up front with the links (mu = 0 does not enter K in Coulomb gauge: mu0 = 1)
+            load_link<RECON>(P.gtrans + (size_t)P.parity * RECON * G.Vh, G.Vh, h, Uf[d]);
 #pragma unroll
-            for (int k = 0; k < 18; ++k) Uf[d][k] = Ub[d][k] = T(0);
+            for (int k = 0; k < 18; ++k) Ub[d][k] = T(0);
             continue;
         }
         load_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
@@ -153,7 +155,12 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
-        if (MODE == MODE_DEFER && d == 0 && j == 0) continue;
+        if (MODE == MODE_DEFER && d == 0 && j == 0) {   // G(x) <- g(x) G(x)
+            T out[18];
+            mul_g_U<ROWS>(g, Uf[d], out);
+            store_link<RECON>(P.gtrans + (size_t)P.parity * RECON * G.Vh, G.Vh, h, out);
+            continue;
+        }
         T out[18];
         mul_g_U<ROWS>(g, Uf[d], out);
         store_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, out);
@@ -161,7 +168,7 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
         T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
         store_link<RECON>(back + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
     }
-    if (ACC && j == 0) {
+    if (MODE == MODE_ACC && j == 0) {
         T* blk = P.gtrans + (size_t)P.parity * RECON * G.Vh;
         T Gt[18], out[18];
         load_link<RECON>(blk, G.Vh, h, Gt);
