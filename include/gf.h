@@ -99,6 +99,24 @@ int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is_f64, int p
  * GF_ESTATE (no storage for that precision), GF_ECUDA. */
 int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision);
 
+/* n iterations = n x {parity 0, parity 1}, asynchronous; the Philox counter advances by 2 per
+ * iteration exactly as 2n gf_sweep calls would, and the links produced are bitwise the same.
+ * When the context is eligible (one lattice, no transformation buffer attached for `precision`,
+ * N_t >= 4, block_threads / lanes_per_site divides the sites of a time slice and parity) each
+ * iteration is ONE fused launch: the tiles of both parities are handed out in a t-wavefront order
+ * (parity-1 sites of slice t right after the parity-0 sites of slice t+2) and every parity-1 tile
+ * waits, inside the kernel, for the completion counters of the three time slices it depends on.
+ * The second touch of every link then hits the L2 cache: DRAM traffic per iteration is the field
+ * read once and written once instead of twice each (measured at 32^4 fp32/18: 657 MB instead of
+ * 1150 MB per iteration).  gf_set_wavefront: 0 (default) = never fuse, 1 = fuse when a time slice of
+ * links is at most 24 MB (so that ~3 slices stay in the 126 MB L2), 2 = fuse whenever eligible.
+ * Off by default: the sweep kernel is latency-bound once DRAM is relieved, so the fused launch is
+ * not faster yet.  gf_fix_until iterates through the same path.
+ * Errors: as gf_sweep; a later gf_measure / gf_fix_until reports GF_ECUDA if a tile ever gave up
+ * waiting (never expected; the wait is bounded so that a fault cannot hang the GPU). */
+int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, int precision);
+int gf_set_wavefront(gf_ctx* ctx, int mode);
+
 /* F (eq. 2) and theta (eq. 4-5, with A_mu the traceless
  * anti-Hermitian part of U_mu) of the field of `precision`, accumulated in fp64 with a fixed
  * reduction order.  host_out receives 1 double (Landau) or N_t doubles (Coulomb: per time slice,

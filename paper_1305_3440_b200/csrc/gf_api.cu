@@ -34,6 +34,12 @@ struct gf_ctx {
     uint8_t* host_mask;         // pinned copy
     int mask_on;                // the sweeps consult dev_mask
     double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
+    // fused iteration (t-wavefront, gf_sweep.cu): device state in the workspace, running totals on the host
+    int wave_mode;              // 0 never, 1 when eligible and a time slice is small enough for the L2, 2 whenever eligible
+    unsigned long long* wave_ticket;
+    uint32_t *wave_done, *wave_error;
+    unsigned long long wave_ticket_total;
+    uint32_t wave_done_total;
     // slab decomposition along t (gf_set_slab): this context holds N_t local slices of a lattice nranks times as long
     int slab_rank, slab_n;
     void* prev_links[2];        // field of the slab below (per precision); NULL = own (one slab)
@@ -112,7 +118,8 @@ extern "C" size_t gf_workspace_bytes(const int dims[4])
 {
     if (!dims_ok(dims)) return 0;
     const MeasureGrid mg = measure_grid(dims);
-    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt;   // + the slice mask
+    // + the slice mask + the wavefront state (ticket, error word, one completion counter per time slice)
+    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt + 16 + sizeof(uint32_t) * kMaxNt;
 }
 
 extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
@@ -149,6 +156,10 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->partials = c->workspace;
     c->slice_out = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
     c->dev_mask = reinterpret_cast<uint8_t*>(c->slice_out + (size_t)dims[0] * 2);
+    c->wave_ticket = reinterpret_cast<unsigned long long*>(c->dev_mask + kMaxNt);
+    c->wave_error = reinterpret_cast<uint32_t*>(c->wave_ticket + 1);
+    c->wave_done = c->wave_error + 2;
+    c->wave_mode = 0;         // opt-in: see gf_set_wavefront
 
     Geom& G = c->G;
     G.nt = dims[0];
@@ -174,7 +185,12 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->slab_rank = 0;
     c->slab_n = 1;
 
-    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt) != cudaSuccess) {
+    if (cudaMemsetAsync(c->wave_ticket, 0, 16 + sizeof(uint32_t) * kMaxNt, c->stream) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return GF_ECUDA;
+    }
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt + 16) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return GF_ENOMEM;
@@ -370,6 +386,7 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
         }
     }
     SweepArgs a;
+    memset(&a, 0, sizeof(a));
     a.links = ctx->links[precision];
     a.gtrans = ctx->gtrans[precision];
     a.defer_temporal = ctx->defer_temporal;
@@ -401,6 +418,89 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     return GF_OK;
 }
 
+// Largest time slice (bytes of link storage) for which the fused iteration is chosen automatically: the
+// second touch of a link comes about 2.5 slices after the first and has to find it in the L2
+// (126 MB L2, read-modify-write hits up to a reuse distance of ~75 MB).
+static const size_t kWaveMaxSliceBytes = (size_t)24 << 20;
+
+static bool wave_eligible(const gf_ctx* ctx, int precision, int lanes, int block, uint32_t* tiles)
+{
+    if (ctx->wave_mode == 0 || ctx->slab_n > 1 || ctx->gtrans[precision] || ctx->dims[0] < 4) return false;
+    const uint32_t sites_per_block = (uint32_t)(block / lanes);
+    if (ctx->mg.Sh % sites_per_block) return false;             // the tiles must cover a slice exactly
+    if (ctx->wave_mode == 1) {
+        const size_t slice = (size_t)ctx->mg.Sh * 2 * 4 * (size_t)ctx->recon * (precision == GF_F64 ? 8 : 4);
+        if (slice > kWaveMaxSliceBytes) return false;
+    }
+    *tiles = ctx->mg.Sh / sites_per_block;
+    return true;
+}
+
+// One iteration = parity 0 then parity 1: a single fused launch when eligible, else two half-sweeps.
+static int enqueue_iteration(gf_ctx* ctx, int algo, double omega, double p, int precision)
+{
+    const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
+    int lanes, block;
+    default_tuning(precision, ctx->recon, solver_f64, 0, 0, &lanes, &block);
+    if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
+    if (ctx->block[precision]) block = ctx->block[precision];
+    uint32_t tiles = 0;
+    if (!wave_eligible(ctx, precision, lanes, block, &tiles)) {
+        int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
+        if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
+        return e;
+    }
+    SweepArgs a;
+    memset(&a, 0, sizeof(a));
+    a.links = ctx->links[precision];
+    a.slice_active = ctx->mask_on ? ctx->dev_mask : nullptr;
+    a.G = ctx->G;
+    a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
+    a.algo = algo;
+    a.omega = omega;
+    a.p = p;
+    a.key0 = (uint32_t)ctx->seed;
+    a.key1 = (uint32_t)(ctx->seed >> 32);
+    a.counter = ctx->counter;
+    a.wave = 1;
+    a.wave_ticket = ctx->wave_ticket;
+    a.wave_ticket_base = ctx->wave_ticket_total;
+    a.wave_done = ctx->wave_done;
+    a.wave_done_target = ctx->wave_done_total + tiles;
+    a.wave_tiles = tiles;
+    a.wave_error = ctx->wave_error;
+    cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, lanes, block, a, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_iterate launch");
+    ctx->wave_ticket_total += 2ull * (unsigned long long)ctx->dims[0] * tiles;
+    ctx->wave_done_total += tiles;
+    ctx->counter += 2;
+    ctx->sweeps += 2;
+    ctx->launches += 1;
+    return GF_OK;
+}
+
+extern "C" int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, int precision)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (n < 0) return fail(ctx, GF_EINVAL, "negative iteration count");
+    rc = check_algo(ctx, algo, omega, p);
+    if (rc) return rc;
+    for (int k = 0; k < n; ++k) {
+        rc = enqueue_iteration(ctx, algo, omega, p, precision);
+        if (rc) return rc;
+    }
+    return GF_OK;
+}
+
+extern "C" int gf_set_wavefront(gf_ctx* ctx, int mode)
+{
+    if (!ctx) return GF_EINVAL;
+    if (mode < 0 || mode > 2) return fail(ctx, GF_EINVAL, "wavefront mode must be 0 (off), 1 (automatic) or 2 (whenever eligible)");
+    ctx->wave_mode = mode;
+    return GF_OK;
+}
+
 extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
 {
     int rc = check_prec(ctx, precision);
@@ -422,8 +522,12 @@ static int measure_to_host(gf_ctx* ctx, int precision)
     GF_SLAB_END(ctx);
     ctx->launches += 2;
     e = cudaMemcpyAsync(ctx->host_pinned, ctx->slice_out, sizeof(double) * 2 * ctx->dims[0], cudaMemcpyDeviceToHost, ctx->stream);
+    uint32_t* wave_err = reinterpret_cast<uint32_t*>(ctx->host_mask + kMaxNt);
+    if (e == cudaSuccess && ctx->wave_ticket_total)
+        e = cudaMemcpyAsync(wave_err, ctx->wave_error, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure copy");
+    if (ctx->wave_ticket_total && *wave_err) return fail(ctx, GF_ECUDA, "a fused iteration gave up waiting for a dependency (field invalid)");
     return GF_OK;
 }
 
@@ -498,8 +602,7 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
         int n = check_every - (it % check_every);
         if (n > max_iter - it) n = max_iter - it;
         for (int k = 0; k < n; ++k) {
-            int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
-            if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
+            int e = enqueue_iteration(ctx, algo, omega, p, precision);
             if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         }
         it += n;

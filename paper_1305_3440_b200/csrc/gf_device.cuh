@@ -111,32 +111,35 @@ __host__ __device__ __forceinline__ size_t block_offset(uint32_t parity, int mu,
     return (size_t)(parity * 4u + (uint32_t)mu) * (size_t)recon * (size_t)Vh;   // in reals
 }
 
-template <int RECON>
+// CG: load through L2 only (ld.global.cg).  Needed where another block of the SAME launch may have
+// written the link (the fused wavefront iteration): an L1 line could be stale.
+template <int RECON, bool CG = false>
 __device__ __forceinline__ void load_link(const double* __restrict__ blk, uint32_t Vh, uint32_t h, double (&m)[18])
 {
     const double2* p = reinterpret_cast<const double2*>(blk) + h;
 #pragma unroll
     for (int c = 0; c < RECON / 2; ++c) {
-        const double2 v = p[(size_t)c * Vh];
+        const double2 v = CG ? __ldcg(p + (size_t)c * Vh) : p[(size_t)c * Vh];
         m[2 * c] = v.x;
         m[2 * c + 1] = v.y;
     }
 }
 
-template <int RECON>
+template <int RECON, bool CG = false>
 __device__ __forceinline__ void load_link(const float* __restrict__ blk, uint32_t Vh, uint32_t h, float (&m)[18])
 {
     const float4* p = reinterpret_cast<const float4*>(blk) + h;
 #pragma unroll
     for (int c = 0; c < RECON / 4; ++c) {
-        const float4 v = p[(size_t)c * Vh];
+        const float4 v = CG ? __ldcg(p + (size_t)c * Vh) : p[(size_t)c * Vh];
         m[4 * c] = v.x;
         m[4 * c + 1] = v.y;
         m[4 * c + 2] = v.z;
         m[4 * c + 3] = v.w;
     }
     if (RECON == 18) {
-        const float2 v = reinterpret_cast<const float2*>(blk + (size_t)16 * Vh)[h];
+        const float2* t = reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + h;
+        const float2 v = CG ? __ldcg(t) : *t;
         m[16] = v.x;
         m[17] = v.y;
     }

@@ -17,6 +17,15 @@ struct SweepArgs {
     const uint8_t* slice_active;   // per time slice, 0 = frozen; NULL = all active
     void* prev_links;       // slab below (same precision and layout), or NULL = this field (periodic)
     uint32_t site_offset;   // global site index of the slab's first site
+    // fused iteration (both parities in one launch, t-wavefront order; gf_sweep.cu): parity, reverse unused;
+    // the Philox counter is `counter` for parity 0 and counter + 1 for parity 1
+    int wave;
+    unsigned long long* wave_ticket;
+    unsigned long long wave_ticket_base;
+    uint32_t* wave_done;
+    uint32_t wave_done_target;
+    uint32_t wave_tiles;     // blocks per (time slice, parity) = Sh * lanes / block, must divide exactly
+    uint32_t* wave_error;
     Geom G;
     uint32_t parity;        // active parity
     int mu0;                // first direction entering K: 0 Landau, 1 Coulomb

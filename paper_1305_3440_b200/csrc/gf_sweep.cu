@@ -31,7 +31,79 @@ template <typename T, typename TK> struct SweepConsts {
     double p;
     uint32_t key0, key1, counter;
     uint32_t reverse;       // 1: blocks walk the lattice from the last site to the first
+    // WAVE (fused iteration, see wave_schedule): work is handed out by ticket, not by blockIdx
+    unsigned long long* ticket;     // device counter, never reset: ticket = old value - ticket_base
+    unsigned long long ticket_base;
+    uint32_t* done;                 // per time slice: parity-0 tiles completed, monotonic over launches
+    uint32_t done_target;           // value of done[t] once all parity-0 tiles of slice t of THIS launch are complete
+    uint32_t tiles;                 // tiles (blocks) per time slice and parity
+    uint32_t* error;                // set to 1 if a dependency wait gave up (never expected)
 };
+
+// ---------------------------------------------------------------------------------------------
+// Fused iteration ("t-wavefront"): ONE launch does the parity-0 half-sweep and the parity-1
+// half-sweep of an iteration, ordered so that the second touch of every link finds
+// it in the 126 MB L2: the tiles are handed out in the order
+//     E(0) .. E(LAG) | E(s) then O(s-LAG) for s = LAG+1 .. Nt-1 | O(Nt-LAG) .. O(Nt-1), O(0)
+// (E(t) / O(t): the parity-0 / parity-1 sites of time slice t).  O(t) needs the parity-0 updates of
+// all its neighbours, i.e. E(t-1), E(t), E(t+1) complete (periodic in t): its block waits for the
+// three per-slice completion counters.  Tickets are taken when a block STARTS, so everything a
+// block waits for is held by blocks that are already running: no deadlock, whatever the hardware's
+// dispatch order.  E(a) and a concurrently running O(b) never touch the same link: E(a) touches
+// slices a, a-1, O(b) slices b, b-1, and O(b) only starts after E(b-1), E(b), E(b+1).  The links are
+// bitwise those of the two separate half-sweeps.  DRAM traffic per iteration: the field is read once
+// and written once instead of twice each.
+constexpr uint32_t WAVE_LAG = 2;
+
+struct WaveTile {
+    uint32_t parity, t, tile;
+};
+
+__device__ __forceinline__ WaveTile wave_schedule(unsigned long long ticket, uint32_t nt, uint32_t tiles)
+{
+    WaveTile w;
+    const unsigned long long headE = (unsigned long long)(WAVE_LAG + 1) * tiles;          // E(0..LAG)
+    const unsigned long long mid = (unsigned long long)(nt - WAVE_LAG - 1) * 2ull * tiles;  // steps LAG+1..Nt-1
+    if (ticket < headE) {
+        w.parity = 0;
+        w.t = (uint32_t)(ticket / tiles);
+        w.tile = (uint32_t)(ticket % tiles);
+    } else if (ticket < headE + mid) {
+        const unsigned long long k = ticket - headE;
+        const uint32_t s = WAVE_LAG + 1 + (uint32_t)(k / (2ull * tiles));
+        const uint32_t r = (uint32_t)(k % (2ull * tiles));
+        // all of E(s), then all of O(s-LAG): by the time an O tile starts, E(s-LAG+1) was handed out more
+        // than a slice of tiles earlier and is complete, so the dependency waits almost never spin
+        w.parity = r >= tiles ? 1u : 0u;
+        w.tile = w.parity ? r - tiles : r;
+        w.t = w.parity ? s - WAVE_LAG : s;                  // O(1) .. O(Nt-1-LAG)
+    } else {
+        const unsigned long long k = ticket - headE - mid;  // O(Nt-LAG) .. O(Nt-1), O(0)
+        w.parity = 1;
+        w.t = (nt - WAVE_LAG + (uint32_t)(k / tiles)) % nt;
+        w.tile = (uint32_t)(k % tiles);
+    }
+    return w;
+}
+
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p)
+{
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// waits until done[t] has reached target (wrap-safe); gives up after ~seconds and reports
+__device__ __forceinline__ void wave_wait(const uint32_t* done, uint32_t t, uint32_t target, uint32_t* error)
+{
+    for (uint32_t spins = 0; (int32_t)(ld_acquire_u32(done + t) - target) < 0; ++spins) {
+        __nanosleep(100);
+        if (spins > (1u << 24)) {
+            *error = 1u;
+            break;
+        }
+    }
+}
 
 template <typename T>
 __device__ __forceinline__ T shfl_xor_T(T v, int mask)
@@ -49,7 +121,7 @@ __device__ __forceinline__ T shfl_xor_T(T v, int mask)
 // traffic; U_0(x) <- G(x) U_0(x) G(x+0)^dagger is applied once at the end (gf_coulomb_finish).
 enum { MODE_PLAIN = 0, MODE_ACC = 1, MODE_DEFER = 2 };
 
-template <typename T, typename TK, int RECON, int L, int MODE>
+template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
 __global__ void sweep_kernel(const SweepConsts<T, TK> P)
 {
     constexpr int S = 32 / L;    // sites per warp
@@ -60,22 +132,47 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     // Alternate half-sweeps walk the lattice in opposite directions (blocks are dispatched in
     // ascending blockIdx order): the launch starts on the sites the previous one finished with,
     // whose links are still in the 126 MB L2.  The result does not depend on the order.
-    const uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+    uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+    uint32_t parity = P.parity, counter = P.counter, wave_t = 0;
+    if (WAVE) {
+        __shared__ uint32_t sh_tile[3];
+        if (threadIdx.x == 0) {
+#ifdef GF_WAVE_BLOCKIDX
+            const WaveTile w = wave_schedule(blockIdx.x, G.nt, P.tiles);
+#else
+            const WaveTile w = wave_schedule(atomicAdd(P.ticket, 1ull) - P.ticket_base, G.nt, P.tiles);
+#endif
+            if (w.parity) {
+                wave_wait(P.done, w.t == 0 ? G.nt - 1u : w.t - 1u, P.done_target, P.error);
+                wave_wait(P.done, w.t, P.done_target, P.error);
+                wave_wait(P.done, w.t + 1u == G.nt ? 0u : w.t + 1u, P.done_target, P.error);
+            }
+            __threadfence();
+            sh_tile[0] = w.parity;
+            sh_tile[1] = w.t;
+            sh_tile[2] = w.t * P.tiles + w.tile;
+        }
+        __syncthreads();
+        parity = sh_tile[0];
+        wave_t = sh_tile[1];
+        bid = sh_tile[2];
+        counter += parity;
+    }
     const uint32_t warp = (bid * blockDim.x + threadIdx.x) >> 5;
-    if (warp * S >= G.Vh) return;                       // warp-uniform
+    if (!WAVE && warp * S >= G.Vh) return;              // warp-uniform (WAVE: the tiles cover the slices exactly)
     uint32_t h = warp * S + (lane % S);
     const int j = lane / S;
     bool live = h < G.Vh;
     if (!live) h = G.Vh - 1u;                           // keeps the lane in the shuffles; no store
-    const Site s = decode_site(G, h, P.parity);
+    const Site s = decode_site(G, h, parity);
     if (P.slice_active != nullptr) {                    // warp-uniform branch
         live = live && P.slice_active[s.c[0]] != 0;
-        if (!__any_sync(0xffffffffu, live)) return;     // the whole warp sits in frozen slices
+        if (!WAVE && !__any_sync(0xffffffffu, live)) return;     // the whole warp sits in frozen slices
     }
 
     if (MODE == MODE_ACC && j == 0) {
         // G(x) is only needed after the links have been written back: start moving it towards L2 now
-        const T* gp = P.gtrans + (size_t)P.parity * RECON * G.Vh;
+        const T* gp = P.gtrans + (size_t)parity * RECON * G.Vh;
         constexpr int CH = (RECON * (int)sizeof(T)) / 16;      // whole 16-byte chunks (the fp32/18 tail rides along)
 #pragma unroll
         for (int c = 0; c < CH; ++c)
@@ -92,15 +189,15 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
         if (MODE == MODE_DEFER && d == 0 && j == 0) {
             // mu = 0: the temporal links stay where they are; their register slot carries G(x) instead,
             // loaded up front with the links (mu = 0 does not enter K in Coulomb gauge: mu0 = 1)
-            load_link<RECON>(P.gtrans + (size_t)P.parity * RECON * G.Vh, G.Vh, h, Uf[d]);
+            load_link<RECON, WAVE>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, Uf[d]);
 #pragma unroll
             for (int k = 0; k < 18; ++k) Ub[d][k] = T(0);
             continue;
         }
-        load_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
+        load_link<RECON, WAVE>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
         // the temporal link below the first local time slice belongs to the slab below
         const T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        load_link<RECON>(back + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
+        load_link<RECON, WAVE>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
     }
     if (RECON == 12) {
 #pragma unroll
@@ -137,7 +234,7 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     bool sq0 = false, sq1 = false, sq2 = false;
     if (P.algo == ALGO_STOCHASTIC) {
         uint32_t w[4];
-        philox4x32_10(P.site_offset + 2u * h + s.xodd, 0u, P.counter, 0u, P.key0, P.key1, w);
+        philox4x32_10(P.site_offset + 2u * h + s.xodd, 0u, counter, 0u, P.key0, P.key1, w);
         sq0 = (double)(w[0] >> 8) * (1.0 / 16777216.0) < P.p;
         sq1 = (double)(w[1] >> 8) * (1.0 / 16777216.0) < P.p;
         sq2 = (double)(w[2] >> 8) * (1.0 / 16777216.0) < P.p;
@@ -151,30 +248,40 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     for (int k = 0; k < 18; ++k) g[k] = (T)gk[k];
 
     // a6: U_mu(x) <- g U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) g^dagger  (eq. 3)
-    if (!live) return;
+    if (!WAVE && !live) return;
+    if (live) {
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
         if (MODE == MODE_DEFER && d == 0 && j == 0) {   // G(x) <- g(x) G(x)
             T out[18];
             mul_g_U<ROWS>(g, Uf[d], out);
-            store_link<RECON>(P.gtrans + (size_t)P.parity * RECON * G.Vh, G.Vh, h, out);
+            store_link<RECON>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, out);
             continue;
         }
         T out[18];
         mul_g_U<ROWS>(g, Uf[d], out);
-        store_link<RECON>(P.links + block_offset<T>(P.parity, mu, RECON, G.Vh), G.Vh, h, out);
+        store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, out);
         mul_U_gdag<ROWS>(Ub[d], g, out);
         T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        store_link<RECON>(back + block_offset<T>(P.parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
+        store_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
     }
     if (MODE == MODE_ACC && j == 0) {
-        T* blk = P.gtrans + (size_t)P.parity * RECON * G.Vh;
+        T* blk = P.gtrans + (size_t)parity * RECON * G.Vh;
         T Gt[18], out[18];
-        load_link<RECON>(blk, G.Vh, h, Gt);
+        load_link<RECON, WAVE>(blk, G.Vh, h, Gt);
         if (RECON == 12) reconstruct_row2(Gt);
         mul_g_U<ROWS>(g, Gt, out);
         store_link<RECON>(blk, G.Vh, h, out);
+    }
+    }
+    if (WAVE && parity == 0u) {
+        // publish: all of this tile's stores, then one count on its time slice
+#ifndef GF_WAVE_NOFENCE
+        __threadfence();
+#endif
+        __syncthreads();
+        if (threadIdx.x == 0) atomicAdd(P.done + wave_t, 1u);
     }
 }
 
@@ -197,6 +304,20 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     P.key1 = a.key1;
     P.counter = a.counter;
     P.reverse = a.reverse;
+    if (a.wave) {
+        // one launch = one iteration: 2 * Nt * tiles blocks, work handed out by ticket
+        P.ticket = a.wave_ticket;
+        P.ticket_base = a.wave_ticket_base;
+        P.done = a.wave_done;
+        P.done_target = a.wave_done_target;
+        P.tiles = a.wave_tiles;
+        P.error = a.wave_error;
+        P.parity = 0;
+        P.reverse = 0;
+        const uint32_t wgrid = 2u * a.G.nt * a.wave_tiles;
+        sweep_kernel<T, TK, RECON, L, MODE_PLAIN, true><<<wgrid, block, 0, st>>>(P);
+        return cudaGetLastError();
+    }
     const uint64_t threads = (uint64_t)a.G.Vh * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);
     if (a.gtrans && a.defer_temporal)

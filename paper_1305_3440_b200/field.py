@@ -82,9 +82,10 @@ class GaugeField:
         B.gf_sweep(self.ctx, parity, algo, omega, p, precision)
 
     def iterate(self, n, algo, omega, p, precision):
-        for _ in range(n):
-            B.gf_sweep(self.ctx, 0, algo, omega, p, precision)
-            B.gf_sweep(self.ctx, 1, algo, omega, p, precision)
+        B.gf_iterate(self.ctx, n, algo, omega, p, precision)
+
+    def set_wavefront(self, mode):
+        B.gf_set_wavefront(self.ctx, mode)
 
     def functional(self, precision):
         return B.gf_functional(self.ctx, precision, self.n_out)

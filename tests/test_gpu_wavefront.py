@@ -1,0 +1,104 @@
+"""The fused iteration (gf_iterate's t-wavefront launch, include/gf.h) against the two separate
+half-sweeps (bitwise) and against the CPU oracle."""
+import numpy as np
+import pytest
+import torch
+
+import gf_inputs as gi
+import oracle
+import paper_1305_3440_b200 as gf
+
+pytestmark = pytest.mark.gpu
+
+PREC = {"f64": gf.GF_F64, "f32": gf.GF_F32}
+CDTYPE = {"f64": torch.complex128, "f32": torch.complex64}
+
+
+def _field(dims, prec, recon, dev, gauge=gf.GF_LANDAU, seed=0):
+    return gf.GaugeField(dims, gauge=gauge, recon=recon, precisions=(prec,), seed=seed, device=dev)
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 8), (6, 4, 8, 4), (16, 8, 8, 8), (4, 16, 16, 16)])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("lanes,block", [(1, 64), (2, 64), (4, 64), (2, 128)])
+def test_fused_iterations_are_bitwise_the_half_sweeps(cuda_device, dims, prec, recon, lanes, block):
+    U = torch.from_numpy(gi.smooth_random_gauge(dims, 0.5, 23)).to(cuda_device).to(CDTYPE[prec]).contiguous()
+    sites_per_block = block // lanes
+    Sh = dims[1] * dims[2] * dims[3] // 2
+    a = _field(dims, prec, recon, cuda_device, seed=5)
+    b = _field(dims, prec, recon, cuda_device, seed=5)
+    for f in (a, b):
+        f.pack(U, PREC[prec])
+        f.set_tuning(PREC[prec], lanes, block)
+    a.set_wavefront(2)
+    l0 = gf.gf_launch_count(a.ctx)
+    a.iterate(7, gf.GF_STOCHASTIC, 1.0, 0.6, PREC[prec])
+    fused = gf.gf_launch_count(a.ctx) - l0 == 7
+    assert fused == (Sh % sites_per_block == 0)                   # otherwise it fell back to 14 half-sweeps
+    for it in range(7):
+        b.sweep(0, gf.GF_STOCHASTIC, 1.0, 0.6, PREC[prec])
+        b.sweep(1, gf.GF_STOCHASTIC, 1.0, 0.6, PREC[prec])
+    assert gf.gf_get_counter(a.ctx) == gf.gf_get_counter(b.ctx) == 14
+    assert torch.equal(a.unpack(PREC[prec]), b.unpack(PREC[prec]))
+    Fa, tha = a.measure(PREC[prec])                               # also checks that no tile gave up waiting
+    Fb, thb = b.measure(PREC[prec])
+    assert Fa == Fb and tha == thb
+    a.close()
+    b.close()
+
+
+@pytest.mark.parametrize("gauge", [gf.GF_LANDAU, gf.GF_COULOMB])
+def test_fused_iterations_match_oracle(cuda_device, gauge):
+    dims = (8, 8, 4, 8)
+    og = oracle.LANDAU if gauge == gf.GF_LANDAU else oracle.COULOMB
+    U = gi.smooth_random_gauge(dims, 0.5, 29)
+    fld = _field(dims, "f64", 18, cuda_device, gauge=gauge, seed=3)
+    fld.pack(torch.from_numpy(U).to(cuda_device), gf.GF_F64)
+    fld.set_wavefront(2)
+    fld.iterate(1, gf.GF_STOCHASTIC, 1.0, 0.7, gf.GF_F64)
+    Uo = U.copy()
+    for parity in (0, 1):
+        oracle.sweep(Uo, dims, parity, gauge=og, algo=oracle.STOCHASTIC, p=0.7, seed=3, half_sweep_counter=parity)
+    assert np.abs(fld.unpack(gf.GF_F64).cpu().numpy() - Uo).max() < 1e-12
+    fld.iterate(9, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+    for _ in range(9):
+        for parity in (0, 1):
+            oracle.sweep(Uo, dims, parity, gauge=og, algo=oracle.OVERRELAX, omega=1.7)
+    F, th = fld.measure(gf.GF_F64)
+    assert np.allclose(F, oracle.functional(Uo, dims, og), rtol=1e-10)
+    assert np.allclose(th, oracle.theta(Uo, dims, og), rtol=1e-10)
+    fld.close()
+
+
+def test_fused_iteration_with_frozen_slices_and_modes(cuda_device):
+    """Slice masks work inside the fused launch; contexts that are not eligible fall back silently."""
+    dims = (8, 4, 4, 8)
+    U = torch.from_numpy(gi.smooth_random_gauge(dims, 0.5, 31)).to(cuda_device)
+    mask = [1, 1, 0, 1, 0, 0, 1, 1]
+    a = _field(dims, "f64", 18, cuda_device, gauge=gf.GF_COULOMB)
+    b = _field(dims, "f64", 18, cuda_device, gauge=gf.GF_COULOMB)
+    for f in (a, b):
+        f.pack(U, gf.GF_F64)
+        f.set_slice_mask(mask)
+        f.set_tuning(gf.GF_F64, 2, 64)
+    a.set_wavefront(2)
+    b.set_wavefront(0)
+    l0, l1 = gf.gf_launch_count(a.ctx), gf.gf_launch_count(b.ctx)
+    a.iterate(5, gf.GF_OVERRELAX, 1.5, 0.0, gf.GF_F64)
+    b.iterate(5, gf.GF_OVERRELAX, 1.5, 0.0, gf.GF_F64)
+    assert gf.gf_launch_count(a.ctx) - l0 == 5 and gf.gf_launch_count(b.ctx) - l1 == 10
+    assert torch.equal(a.unpack(gf.GF_F64), b.unpack(gf.GF_F64))
+    c = _field(dims, "f64", 18, cuda_device)                      # default: off
+    c.pack(U, gf.GF_F64)
+    l0 = gf.gf_launch_count(c.ctx)
+    c.iterate(3, gf.GF_RELAX, 1.0, 0.0, gf.GF_F64)
+    assert gf.gf_launch_count(c.ctx) - l0 == 6
+    c.close()
+    a.attach_transform(("f64",))                                  # accumulation: not fused
+    l0 = gf.gf_launch_count(a.ctx)
+    a.iterate(2, gf.GF_OVERRELAX, 1.5, 0.0, gf.GF_F64)
+    assert gf.gf_launch_count(a.ctx) - l0 == 4
+    assert gf.binding.lib.gf_set_wavefront(a.ctx, 3) == gf.GF_EINVAL
+    a.close()
+    b.close()
