@@ -245,7 +245,7 @@ int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2);
 
 /* Kernel configuration of gf_sweep for `precision`: lanes_per_site in {1,2,4} threads cooperate
  * on one site (each owns 8/lanes links; K is combined with warp shuffles); block_threads in
- * {64,128,256,512}.  0 = the built-in choice for the variant (storage precision, recon, solver
+ * {64,128,256}.  0 = the built-in choice for the variant (storage precision, recon, solver
  * precision), measured on B200.  Results do not depend on it beyond the summation order inside K. */
 int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_threads);
 

@@ -952,7 +952,7 @@ extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int
     if (!ctx) return GF_EINVAL;
     if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
     if (!sweep_config_valid(lanes_per_site ? lanes_per_site : 1, block_threads ? block_threads : 64))
-        return fail(ctx, GF_EINVAL, "lanes must be 0,1,2,4 and block 0 or 64..512 (power of two)");
+        return fail(ctx, GF_EINVAL, "lanes must be 0,1,2,4 and block 0, 64, 128 or 256");
     ctx->lanes[precision] = lanes_per_site;
     ctx->block[precision] = block_threads;
     return GF_OK;

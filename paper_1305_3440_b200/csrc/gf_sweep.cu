@@ -122,7 +122,7 @@ __device__ __forceinline__ T shfl_xor_T(T v, int mask)
 enum { MODE_PLAIN = 0, MODE_ACC = 1, MODE_DEFER = 2 };
 
 template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
-__global__ void sweep_kernel(const SweepConsts<T, TK> P)
+__device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
 {
     constexpr int S = 32 / L;    // sites per warp
     constexpr int ND = 4 / L;    // directions per lane
@@ -285,6 +285,35 @@ __global__ void sweep_kernel(const SweepConsts<T, TK> P)
     }
 }
 
+template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
+__global__ void sweep_kernel(const SweepConsts<T, TK> P)
+{
+    sweep_body<T, TK, RECON, L, MODE, WAVE>(P);
+}
+
+// The fp32 / 18-real two-lane kernels sit at 134-141 registers, just above the 128 that let 16 instead
+// of 12 warps be resident; capping them (no spills with the fp32 solver) buys 3-4 % at 32^4.  Every
+// other variant is better off with the allocation the compiler picks on its own, hence a second
+// entry point instead of bounds on all of them.  Blocks have at most 256 threads (sweep_config_valid).
+template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
+__global__ void __launch_bounds__(256, 2) sweep_kernel_r128(const SweepConsts<T, TK> P)
+{
+    sweep_body<T, TK, RECON, L, MODE, WAVE>(P);
+}
+
+template <typename T, int RECON, int L> struct UseR128 {
+    static constexpr bool value = sizeof(T) == 4 && RECON == 18 && L == 2;
+};
+
+template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE>
+static void launch_kernel(uint32_t grid, int block, cudaStream_t st, const SweepConsts<T, TK>& P)
+{
+    if constexpr (UseR128<T, RECON, L>::value)
+        sweep_kernel_r128<T, TK, RECON, L, MODE, WAVE><<<grid, block, 0, st>>>(P);
+    else
+        sweep_kernel<T, TK, RECON, L, MODE, WAVE><<<grid, block, 0, st>>>(P);
+}
+
 template <typename T, typename TK, int RECON, int L>
 static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
 {
@@ -315,23 +344,23 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
         P.parity = 0;
         P.reverse = 0;
         const uint32_t wgrid = 2u * a.G.nt * a.wave_tiles;
-        sweep_kernel<T, TK, RECON, L, MODE_PLAIN, true><<<wgrid, block, 0, st>>>(P);
+        launch_kernel<T, TK, RECON, L, MODE_PLAIN, true>(wgrid, block, st, P);
         return cudaGetLastError();
     }
     const uint64_t threads = (uint64_t)a.G.Vh * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);
     if (a.gtrans && a.defer_temporal)
-        sweep_kernel<T, TK, RECON, L, MODE_DEFER><<<grid, block, 0, st>>>(P);
+        launch_kernel<T, TK, RECON, L, MODE_DEFER, false>(grid, block, st, P);
     else if (a.gtrans)
-        sweep_kernel<T, TK, RECON, L, MODE_ACC><<<grid, block, 0, st>>>(P);
+        launch_kernel<T, TK, RECON, L, MODE_ACC, false>(grid, block, st, P);
     else
-        sweep_kernel<T, TK, RECON, L, MODE_PLAIN><<<grid, block, 0, st>>>(P);
+        launch_kernel<T, TK, RECON, L, MODE_PLAIN, false>(grid, block, st, P);
     return cudaGetLastError();
 }
 
 bool sweep_config_valid(int lanes, int block)
 {
-    return (lanes == 1 || lanes == 2 || lanes == 4) && (block == 64 || block == 128 || block == 256 || block == 512);
+    return (lanes == 1 || lanes == 2 || lanes == 4) && (block == 64 || block == 128 || block == 256);
 }
 
 template <typename T, typename TK, int RECON>
