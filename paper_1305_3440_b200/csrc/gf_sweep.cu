@@ -137,11 +137,7 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     if (WAVE) {
         __shared__ uint32_t sh_tile[3];
         if (threadIdx.x == 0) {
-#ifdef GF_WAVE_BLOCKIDX
-            const WaveTile w = wave_schedule(blockIdx.x, G.nt, P.tiles);
-#else
             const WaveTile w = wave_schedule(atomicAdd(P.ticket, 1ull) - P.ticket_base, G.nt, P.tiles);
-#endif
             if (w.parity) {
                 wave_wait(P.done, w.t == 0 ? G.nt - 1u : w.t - 1u, P.done_target, P.error);
                 wave_wait(P.done, w.t, P.done_target, P.error);
@@ -277,9 +273,7 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     }
     if (WAVE && parity == 0u) {
         // publish: all of this tile's stores, then one count on its time slice
-#ifndef GF_WAVE_NOFENCE
         __threadfence();
-#endif
         __syncthreads();
         if (threadIdx.x == 0) atomicAdd(P.done + wave_t, 1u);
     }
