@@ -399,3 +399,35 @@ def test_no_writes_outside_the_lent_buffers(cuda_device, dims, prec, recon):
     assert torch.isfinite(torch.view_as_real(out)).all()
     for b, n in zip(bufs, nbytes):
         assert bool((b[:guard] == 0xA5).all()) and bool((b[guard + n:] == 0xA5).all())
+
+
+# ------------------------------------------------------------------------------------- fuzz
+
+def test_random_small_lattices_against_oracle(cuda_device):
+    """40 seeded random combinations of (dims, gauge, algorithm, storage, lanes, block, fused iteration):
+    two iterations on the device against the oracle, links within the one-sweep tolerance x 4."""
+    rng = np.random.default_rng(2024)
+    for case in range(40):
+        dims = tuple(int(2 * rng.integers(1, 6)) for _ in range(4))
+        prec = ("f64", "f32")[int(rng.integers(0, 2))]
+        recon = (18, 12)[int(rng.integers(0, 2))]
+        gauge = (gf.GF_LANDAU, gf.GF_COULOMB)[int(rng.integers(0, 2))]
+        algo = (gf.GF_RELAX, gf.GF_OVERRELAX, gf.GF_STOCHASTIC)[int(rng.integers(0, 3))]
+        lanes, block = (1, 2, 4)[int(rng.integers(0, 3))], (64, 128, 256)[int(rng.integers(0, 3))]
+        omega, p, seed = 1.0 + 0.9 * float(rng.random()), float(rng.random()), int(rng.integers(0, 2 ** 40))
+        U = gi.smooth_random_gauge(dims, 0.5, 100 + case)
+        fld = make_field(dims, prec, cuda_device, gauge=gauge, recon=recon, seed=seed)
+        fld.pack(to_device(U, prec, cuda_device), PREC[prec])
+        fld.set_tuning(PREC[prec], lanes, block)
+        fld.set_wavefront(int(rng.integers(0, 3)))
+        fld.iterate(2, algo, omega, p, PREC[prec])
+        Uo = oracle_input(U, prec)
+        og = oracle.LANDAU if gauge == gf.GF_LANDAU else oracle.COULOMB
+        for it in range(2):
+            for parity in (0, 1):
+                oracle.sweep(Uo, dims, parity, og, algo, omega, p, seed=seed, half_sweep_counter=2 * it + parity)
+        err = np.abs(get_links(fld, prec) - Uo).max()
+        assert err < 4 * LINK_TOL[prec], (case, dims, prec, recon, gauge, algo, lanes, block, err)
+        F, th = fld.measure(PREC[prec])
+        assert np.allclose(F, oracle.functional(Uo, dims, og), rtol=0, atol=1e-5 if prec == "f32" else 1e-12)
+        fld.close()
