@@ -42,7 +42,7 @@ VARIANTS = {            # name: (precision key, recon, bytes per real)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep_kernel launch at 32^4, from the `ncu --set full`
 # captures summarised in profiles/r1_sweep_variants_ncu.md (average of a forward and a reverse launch; cold L2)
-NCU_TRAFFIC_BYTES = {"f64-18": 1149.6e6, "f64-12": 747.7e6, "f32-18": 547.0e6, "f32-12": 346.8e6}
+NCU_TRAFFIC_BYTES = {"f64-18": 1149.6e6, "f64-12": 746.6e6, "f32-18": 547.3e6, "f32-12": 345.9e6}
 
 
 def measured_peaks():
