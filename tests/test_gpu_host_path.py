@@ -1,0 +1,80 @@
+"""The host-buffer entry points bench.py's end-to-end measurement uses (gf_load_host / gf_store_host):
+canonical field in pinned HOST memory -> device -> sweeps -> back to the host, against the oracle; and
+the pipelined form (several lattices in flight, one context / stream / host thread each)."""
+import threading
+
+import numpy as np
+import pytest
+import torch
+
+import gf_inputs as gi
+import oracle
+import paper_1305_3440_b200 as gf
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("prec,cdtype,recon,tol", [("f64", torch.complex128, 18, 1e-12), ("f64", torch.complex128, 12, 1e-12),
+                                                   ("f32", torch.complex64, 18, 1e-5)])
+def test_load_sweep_store_through_host_buffers(cuda_device, prec, cdtype, recon, tol):
+    dims = (6, 4, 8, 4)
+    P = gf.GF_F64 if prec == "f64" else gf.GF_F32
+    U = gi.smooth_random_gauge(dims, 0.5, 61)
+    host = torch.from_numpy(U).to(cdtype).pin_memory()
+    fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device, staging=True)
+    fld.load_host(host, P)
+    fld.iterate(2, gf.GF_OVERRELAX, 1.6, 0.0, P)
+    out = torch.empty_like(host).pin_memory()
+    fld.store_host(out, P)                           # synchronises: `out` is complete
+    Uo = np.ascontiguousarray(host.numpy().astype(np.complex128))
+    for _ in range(2):
+        for parity in (0, 1):
+            oracle.sweep(Uo, dims, parity, algo=oracle.OVERRELAX, omega=1.6)
+    assert np.abs(out.numpy().astype(np.complex128) - Uo).max() < 2 * tol
+    assert torch.equal(host, torch.from_numpy(U).to(cdtype))           # the input buffer is not written
+    fld.close()
+
+
+def test_pipelined_lattices_do_not_disturb_each_other(cuda_device):
+    """Four lattices in flight as in bench.py's e2e leg (own context, stream, pinned buffer and host
+    thread): every one ends bitwise where a lone run of the same input ends."""
+    dims = (8, 8, 8, 8)
+    inputs = [torch.from_numpy(gi.smooth_random_gauge(dims, 0.5, 70 + i)).pin_memory() for i in range(4)]
+    want = []
+    for h in inputs:
+        f = gf.GaugeField(dims, precisions=("f64",), device=cuda_device, staging=True)
+        f.load_host(h, gf.GF_F64)
+        f.iterate(6, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+        o = torch.empty_like(h).pin_memory()
+        f.store_host(o, gf.GF_F64)
+        want.append(o.clone())
+        f.close()
+    fields, outs = [], [torch.empty_like(h).pin_memory() for h in inputs]
+    for _ in inputs:
+        with torch.cuda.stream(torch.cuda.Stream(device=cuda_device)):
+            fields.append(gf.GaugeField(dims, precisions=("f64",), device=cuda_device, staging=True))
+    errors = []
+
+    def worker(f, h, o):
+        try:
+            torch.cuda.set_device(cuda_device)
+            for _ in range(3):                       # the same step three times over: last result must match
+                f.load_host(h, gf.GF_F64)
+                for _ in range(3):
+                    f.iterate(2, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+                    f.measure(gf.GF_F64)
+                f.store_host(o, gf.GF_F64)
+        except Exception as e:                       # surfaced below
+            errors.append(e)
+
+    threads = [threading.Thread(target=worker, args=a) for a in zip(fields, inputs, outs)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    torch.cuda.synchronize()
+    assert not errors, errors
+    for o, w in zip(outs, want):
+        assert torch.equal(o, w)
+    for f in fields:
+        f.close()
