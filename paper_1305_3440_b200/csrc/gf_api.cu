@@ -50,7 +50,8 @@ struct gf_ctx {
     CUresult (*write32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
     double* workspace;
     double* partials;           // workspace: per-block partial sums
-    double* slice_out;          // workspace: 2 doubles per time slice
+    double* slice_out;          // 2 doubles per time slice, written by the last reduction kernel: the DEVICE ADDRESS OF
+                                // host_pinned (zero-copy: the result is in host memory when the stream has drained)
     double* host_pinned;        // 2 * Nt doubles
     cudaStream_t stream;
     uint64_t seed;
@@ -154,8 +155,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
     c->mg = measure_grid(dims);
     c->partials = c->workspace;
-    c->slice_out = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
-    c->dev_mask = reinterpret_cast<uint8_t*>(c->slice_out + (size_t)dims[0] * 2);
+    c->dev_mask = reinterpret_cast<uint8_t*>(c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2 + (size_t)dims[0] * 2);
     c->wave_ticket = reinterpret_cast<unsigned long long*>(c->dev_mask + kMaxNt);
     c->wave_error = reinterpret_cast<uint32_t*>(c->wave_ticket + 1);
     c->wave_done = c->wave_error + 2;
@@ -196,6 +196,12 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
         return GF_ENOMEM;
     }
     c->host_mask = reinterpret_cast<uint8_t*>(c->host_pinned + 2 * kMaxNt);
+    if (cudaHostGetDevicePointer(reinterpret_cast<void**>(&c->slice_out), c->host_pinned, 0) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFreeHost(c->host_pinned);
+        delete c;
+        return GF_ECUDA;
+    }
     *out = c;
     return GF_OK;
 }
@@ -521,7 +527,6 @@ static int measure_to_host(gf_ctx* ctx, int precision)
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
     GF_SLAB_END(ctx);
     ctx->launches += 2;
-    e = cudaMemcpyAsync(ctx->host_pinned, ctx->slice_out, sizeof(double) * 2 * ctx->dims[0], cudaMemcpyDeviceToHost, ctx->stream);
     uint32_t* wave_err = reinterpret_cast<uint32_t*>(ctx->host_mask + kMaxNt);
     if (e == cudaSuccess && ctx->wave_ticket_total)
         e = cudaMemcpyAsync(wave_err, ctx->wave_error, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
@@ -900,8 +905,7 @@ extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision)
 static int slices_to_host(gf_ctx* ctx, const char* what)
 {
     ctx->launches += 2;
-    cudaError_t e = cudaMemcpyAsync(ctx->host_pinned, ctx->slice_out, sizeof(double) * 2 * ctx->dims[0], cudaMemcpyDeviceToHost, ctx->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, what);
     return GF_OK;
 }
