@@ -282,64 +282,45 @@ cudaError_t launch_unitarity(int precision, int recon, const void* links, const 
 
 // ---------------------------------------------------------------------- pack / unpack / cast
 // a11: canonical AoS (site s, mu, 3x3 row-major complex) <-> the private chunked layout.
-// A block moves TILE_H consecutive half-indices of BOTH parities = 2 * TILE_H consecutive canonical
-// sites (s = 2h + xodd), through a shared-memory tile, so that both sides are coalesced: the private
-// layout is read / written with one 16-byte chunk per lane (thread = (h, mu)), the canonical AoS
-// array as one contiguous run of 2 * TILE_H * 72 reals.  One real of padding per site keeps the
-// transposing side at a 2-way bank conflict.
-constexpr int TILE_H = 32;
-constexpr int SITE_REALS = 72;           // 4 links x 18 reals
-constexpr int SITE_PITCH = SITE_REALS + 1;
-
+// One thread per site; the AoS side is strided (16 of every 32-byte sector per instruction).  A
+// version that transposes through a shared-memory tile is 3.6x faster in isolation (unpack 0.81 ->
+// 0.23 ms at 32^4) but was measured to slow the pipelined end-to-end step from 41 to 50 ms: kernels
+// that need shared memory do not share SMs smoothly with the register-bound sweep kernels of the
+// other lattices in flight.  These conversions run once per field, so the simple form stays.
 template <typename T, int RECON, typename TC>
-__global__ void __launch_bounds__(4 * TILE_H) pack_kernel(T* __restrict__ links, const Geom G, const TC* __restrict__ canonical)
+__global__ void pack_kernel(T* __restrict__ links, const Geom G, const TC* __restrict__ canonical)
 {
-    __shared__ TC tile[2 * TILE_H * SITE_PITCH];
-    const uint32_t h0 = blockIdx.x * TILE_H;
-    const uint32_t nh = min((uint32_t)TILE_H, G.Vh - h0);
-    const TC* src = canonical + (size_t)2 * h0 * SITE_REALS;
-    for (uint32_t e = threadIdx.x; e < 2u * nh * SITE_REALS; e += blockDim.x) {
-        const uint32_t ls = e / SITE_REALS;
-        tile[ls * SITE_PITCH + (e - ls * SITE_REALS)] = src[e];
-    }
-    __syncthreads();
-    const uint32_t hl = threadIdx.x % TILE_H, mu = threadIdx.x / TILE_H;
-    if (hl >= nh) return;
-    const uint32_t h = h0 + hl;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    const Site s = decode_site(G, h, parity);
+    const size_t site = 2u * (size_t)h + s.xodd;
 #pragma unroll
-    for (uint32_t parity = 0; parity < 2; ++parity) {
-        const uint32_t ls = 2u * hl + decode_site(G, h, parity).xodd;
+    for (int mu = 0; mu < 4; ++mu) {
+        const TC* src = canonical + (site * 4 + mu) * 18;
         T m[18];
 #pragma unroll
-        for (int k = 0; k < 18; ++k) m[k] = (T)tile[ls * SITE_PITCH + mu * 18 + k];
-        store_link<RECON>(links + block_offset<T>(parity, (int)mu, RECON, G.Vh), G.Vh, h, m);
+        for (int k = 0; k < 18; ++k) m[k] = (T)src[k];
+        store_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, m);
     }
 }
 
 template <typename T, int RECON, typename TC>
-__global__ void __launch_bounds__(4 * TILE_H) unpack_kernel(const T* __restrict__ links, const Geom G, TC* __restrict__ canonical)
+__global__ void unpack_kernel(const T* __restrict__ links, const Geom G, TC* __restrict__ canonical)
 {
-    __shared__ TC tile[2 * TILE_H * SITE_PITCH];
-    const uint32_t h0 = blockIdx.x * TILE_H;
-    const uint32_t nh = min((uint32_t)TILE_H, G.Vh - h0);
-    const uint32_t hl = threadIdx.x % TILE_H, mu = threadIdx.x / TILE_H;
-    if (hl < nh) {
-        const uint32_t h = h0 + hl;
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= 2u * G.Vh) return;
+    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
+    const Site s = decode_site(G, h, parity);
+    const size_t site = 2u * (size_t)h + s.xodd;
 #pragma unroll
-        for (uint32_t parity = 0; parity < 2; ++parity) {
-            const uint32_t ls = 2u * hl + decode_site(G, h, parity).xodd;
-            T m[18];
-            load_link<RECON>(links + block_offset<T>(parity, (int)mu, RECON, G.Vh), G.Vh, h, m);
-            if (RECON == 12) reconstruct_row2(m);
+    for (int mu = 0; mu < 4; ++mu) {
+        T m[18];
+        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, m);
+        if (RECON == 12) reconstruct_row2(m);
+        TC* dst = canonical + (site * 4 + mu) * 18;
 #pragma unroll
-            for (int k = 0; k < 18; ++k) tile[ls * SITE_PITCH + mu * 18 + k] = (TC)m[k];
-        }
-    }
-    __syncthreads();
-    TC* dst = canonical + (size_t)2 * h0 * SITE_REALS;
-    for (uint32_t e = threadIdx.x; e < 2u * nh * SITE_REALS; e += blockDim.x) {
-        const uint32_t ls = e / SITE_REALS;
-        dst[e] = tile[ls * SITE_PITCH + (e - ls * SITE_REALS)];
+        for (int k = 0; k < 18; ++k) dst[k] = (TC)m[k];
     }
 }
 
@@ -394,7 +375,7 @@ __global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int repr
 template <typename T, int RECON>
 static cudaError_t pack_run(void* links, const Geom& G, const void* canonical, int canonical_is_f64, cudaStream_t st)
 {
-    const uint32_t block = 4 * TILE_H, grid = (G.Vh + TILE_H - 1) / TILE_H;
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
     if (canonical_is_f64)
         pack_kernel<T, RECON, double><<<grid, block, 0, st>>>(static_cast<T*>(links), G, static_cast<const double*>(canonical));
     else
@@ -405,7 +386,7 @@ static cudaError_t pack_run(void* links, const Geom& G, const void* canonical, i
 template <typename T, int RECON>
 static cudaError_t unpack_run(const void* links, const Geom& G, void* canonical, int canonical_is_f64, cudaStream_t st)
 {
-    const uint32_t block = 4 * TILE_H, grid = (G.Vh + TILE_H - 1) / TILE_H;
+    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
     if (canonical_is_f64)
         unpack_kernel<T, RECON, double><<<grid, block, 0, st>>>(static_cast<const T*>(links), G, static_cast<double*>(canonical));
     else
