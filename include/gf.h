@@ -126,6 +126,15 @@ int gf_functional(gf_ctx* ctx, int precision, double* host_out);
 int gf_theta(gf_ctx* ctx, int precision, double* host_out);
 int gf_measure(gf_ctx* ctx, int precision, double* host_functional, double* host_theta);
 
+/* The same reduction without stalling the stream: gf_measure_async enqueues the F / theta pass over the
+ * field as it is at that point of the stream; the kernels write the per-slice sums straight into
+ * pinned host memory, slot 0..15.  gf_measure_collect synchronises the stream and returns the values
+ * of a slot exactly as gf_measure would have (either pointer may be NULL), then frees the slot.
+ * For following the convergence of a run without a host round trip per evaluation.
+ * Errors: GF_EINVAL (slot), GF_ESTATE (empty slot, no storage), GF_ECUDA. */
+int gf_measure_async(gf_ctx* ctx, int precision, int slot);
+int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional, double* host_theta);
+
 /* Iterates {gf_sweep(parity 0); gf_sweep(parity 1)} (= 1 iteration); after every
  * iteration that is a multiple of check_every (and after the last) evaluates theta (Coulomb:
  * max over slices) and stops when it is below theta_target.  precision GF_MIXED: fp32

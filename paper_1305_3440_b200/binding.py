@@ -47,6 +47,8 @@ def _load():
         "gf_functional": (i32, [vp, i32, dp]),
         "gf_theta": (i32, [vp, i32, dp]),
         "gf_measure": (i32, [vp, i32, dp, dp]),
+        "gf_measure_async": (i32, [vp, i32, i32]),
+        "gf_measure_collect": (i32, [vp, i32, dp, dp]),
         "gf_fix_until": (i32, [vp, i32, dbl, dbl, i32, dbl, i32, i32, ip, dp]),
         "gf_transform_bytes": (C.c_size_t, [ip, i32, i32]),
         "gf_set_transform": (i32, [vp, vp, vp]),
@@ -82,7 +84,7 @@ def _load():
 
 lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
-           "gf_sweep gf_iterate gf_set_wavefront gf_functional gf_theta gf_measure gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
+           "gf_sweep gf_iterate gf_set_wavefront gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
            "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
@@ -178,6 +180,18 @@ def gf_measure(ctx, precision, n_out=1, check=True):
     f = (C.c_double * n_out)()
     t = (C.c_double * n_out)()
     _rc(ctx, lib.gf_measure(ctx, precision, f, t), check)
+    return list(f), list(t)
+
+
+def gf_measure_async(ctx, precision, slot, check=True):
+    return _rc(ctx, lib.gf_measure_async(ctx, precision, int(slot)), check)
+
+
+def gf_measure_collect(ctx, slot, n_out=1, check=True):
+    """Returns (F list, theta list) of what gf_measure_async put into the slot."""
+    f = (C.c_double * n_out)()
+    t = (C.c_double * n_out)()
+    _rc(ctx, lib.gf_measure_collect(ctx, int(slot), f, t), check)
     return list(f), list(t)
 
 

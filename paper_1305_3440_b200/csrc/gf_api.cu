@@ -20,6 +20,7 @@ static int upload_mask(gf_ctx* ctx);
 namespace {
 constexpr int kMeasureBlock = 128;
 constexpr int kMaxNt = 4096;
+constexpr int kAsyncSlots = 16;
 }
 
 struct gf_ctx {
@@ -53,6 +54,9 @@ struct gf_ctx {
     double* slice_out;          // 2 doubles per time slice, written by the last reduction kernel: the DEVICE ADDRESS OF
                                 // host_pinned (zero-copy: the result is in host memory when the stream has drained)
     double* host_pinned;        // 2 * Nt doubles
+    double* host_slots;         // kAsyncSlots x 2 * Nt doubles (pinned): results of gf_measure_async
+    double* slots_dev;          // device address of host_slots
+    int slot_precision[16];     // precision measured into the slot, or -1 when empty
     cudaStream_t stream;
     uint64_t seed;
     uint32_t counter;
@@ -196,6 +200,15 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
         return GF_ENOMEM;
     }
     c->host_mask = reinterpret_cast<uint8_t*>(c->host_pinned + 2 * kMaxNt);
+    for (int k = 0; k < kAsyncSlots; ++k) c->slot_precision[k] = -1;
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_slots), sizeof(double) * 2 * dims[0] * kAsyncSlots) != cudaSuccess ||
+        cudaHostGetDevicePointer(reinterpret_cast<void**>(&c->slots_dev), c->host_slots, 0) != cudaSuccess) {
+        cudaGetLastError();
+        if (c->host_slots) cudaFreeHost(c->host_slots);
+        cudaFreeHost(c->host_pinned);
+        delete c;
+        return GF_ENOMEM;
+    }
     if (cudaHostGetDevicePointer(reinterpret_cast<void**>(&c->slice_out), c->host_pinned, 0) != cudaSuccess) {
         cudaGetLastError();
         cudaFreeHost(c->host_pinned);
@@ -210,6 +223,7 @@ extern "C" void gf_destroy(gf_ctx* ctx)
 {
     if (!ctx) return;
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
+    if (ctx->host_slots) cudaFreeHost(ctx->host_slots);
     delete ctx;
 }
 
@@ -538,10 +552,10 @@ static int measure_to_host(gf_ctx* ctx, int precision)
 
 // Normalises the slice sums: Landau 1/(Nc Nd V) and 1/(Nc V); Coulomb per slice
 // 1/(Nc 3 Ns^3) and 1/(Nc Ns^3).  Returns max_t theta_t (Landau: theta).
-static double finish_measure(const gf_ctx* ctx, double* host_F, double* host_theta)
+static double finish_measure(const gf_ctx* ctx, double* host_F, double* host_theta, const double* sums = nullptr)
 {
     const int nt = ctx->dims[0];
-    const double* s = ctx->host_pinned;
+    const double* s = sums ? sums : ctx->host_pinned;
     if (ctx->gauge == GF_COULOMB) {
         const double Vs = (double)(ctx->V / nt);
         double worst = 0.0;
@@ -573,6 +587,34 @@ extern "C" int gf_measure(gf_ctx* ctx, int precision, double* host_functional, d
     rc = measure_to_host(ctx, precision);
     if (rc) return rc;
     finish_measure(ctx, host_functional, host_theta);
+    return GF_OK;
+}
+
+extern "C" int gf_measure_async(gf_ctx* ctx, int precision, int slot)
+{
+    int rc = check_prec(ctx, precision);
+    if (rc) return rc;
+    if (slot < 0 || slot >= kAsyncSlots) return fail(ctx, GF_EINVAL, "slot must be 0..%d", kAsyncSlots - 1);
+    const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
+    GF_SLAB_BEGIN(ctx);
+    cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0, ctx->mg,
+                                   ctx->partials, ctx->slots_dev + (size_t)slot * 2 * ctx->dims[0], ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
+    GF_SLAB_END(ctx);
+    ctx->launches += 2;
+    ctx->slot_precision[slot] = precision;
+    return GF_OK;
+}
+
+extern "C" int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional, double* host_theta)
+{
+    if (!ctx) return GF_EINVAL;
+    if (slot < 0 || slot >= kAsyncSlots) return fail(ctx, GF_EINVAL, "slot must be 0..%d", kAsyncSlots - 1);
+    if (ctx->slot_precision[slot] < 0) return fail(ctx, GF_ESTATE, "nothing was measured into slot %d", slot);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_measure_collect");
+    finish_measure(ctx, host_functional, host_theta, ctx->host_slots + (size_t)slot * 2 * ctx->dims[0]);
+    ctx->slot_precision[slot] = -1;
     return GF_OK;
 }
 

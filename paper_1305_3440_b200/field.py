@@ -96,6 +96,12 @@ class GaugeField:
     def measure(self, precision):
         return B.gf_measure(self.ctx, precision, self.n_out)
 
+    def measure_async(self, precision, slot):
+        B.gf_measure_async(self.ctx, precision, slot)
+
+    def measure_collect(self, slot):
+        return B.gf_measure_collect(self.ctx, slot, self.n_out)
+
     def fix_until(self, algo, omega, p, precision, theta_target, max_iter, check_every=1):
         return B.gf_fix_until(self.ctx, algo, omega, p, precision, theta_target, max_iter, check_every)
 

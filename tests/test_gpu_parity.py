@@ -431,3 +431,28 @@ def test_random_small_lattices_against_oracle(cuda_device):
         F, th = fld.measure(PREC[prec])
         assert np.allclose(F, oracle.functional(Uo, dims, og), rtol=0, atol=1e-5 if prec == "f32" else 1e-12)
         fld.close()
+
+
+def test_measure_async_equals_measure(cuda_device):
+    """gf_measure_async / gf_measure_collect: several evaluations in flight between sweeps give exactly
+    the values the synchronous gf_measure gives at the same points (Landau and Coulomb)."""
+    from paper_1305_3440_b200 import binding as B
+    dims = (6, 4, 6, 4)
+    U = to_device(gi.smooth_random_gauge(dims, 0.5, 9), "f64", cuda_device)
+    for gauge in (gf.GF_LANDAU, gf.GF_COULOMB):
+        a = make_field(dims, "f64", cuda_device, gauge=gauge)
+        b = make_field(dims, "f64", cuda_device, gauge=gauge)
+        a.pack(U, gf.GF_F64)
+        b.pack(U, gf.GF_F64)
+        want = []
+        for k in range(5):
+            a.iterate(2, gf.GF_OVERRELAX, 1.6, 0.0, gf.GF_F64)
+            want.append(a.measure(gf.GF_F64))
+            b.iterate(2, gf.GF_OVERRELAX, 1.6, 0.0, gf.GF_F64)
+            b.measure_async(gf.GF_F64, k)
+        got = [b.measure_collect(k) for k in range(5)]
+        assert got == want
+        assert B.lib.gf_measure_collect(b.ctx, 0, None, None) == gf.GF_ESTATE          # collected slots are empty again
+        assert B.lib.gf_measure_async(b.ctx, gf.GF_F64, 16) == gf.GF_EINVAL
+        a.close()
+        b.close()
