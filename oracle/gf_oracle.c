@@ -23,10 +23,15 @@
  *   parity(s) = (t + x + y + z) mod 2.
  *
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): see the list in
- * DESIGN.md section "Oracle pins".  Unpinned choices (several readings are
- * equally valid and the paper does not decide): the overall normalisation of
- * A_mu (A1), per-SU(2)-factor overrelaxation (A7), one random draw per
- * (site, subgroup) (A8).  For those the header says: parity unpinned.
+ * DESIGN.md section "Oracle pins"; tests/test_oracle_mutants.py re-runs them on
+ * single-line mutants of this file (each must fail a pin).  Unpinned CHOICES OF
+ * READING (several readings are equally valid and the paper does not decide):
+ * the overall normalisation of A_mu (A1), per-SU(2)-factor overrelaxation (A7),
+ * one random draw per (site, subgroup) (A8).  For those the header says: parity
+ * unpinned -- the paper cannot tell the readings apart; what this file computes
+ * UNDER each reading is pinned (closed forms per subgroup, the ordered product
+ * of the three factors with distinct draws, every function incl. the
+ * unitarity checker against fields with a known defect).
  *
  * Build: gcc -O2 -std=c99 -ffp-contract=off -fcx-limited-range [-fopenmp]
  *        -shared -fPIC gf_oracle.c -o libgf_oracle.so -lm   (oracle/build.py)

@@ -55,6 +55,29 @@ def test_site_uniforms_are_24_bit_fractions_of_the_philox_words():
         assert 0.0 <= u[k] < 1.0
 
 
+def test_site_uniforms_keep_all_24_leading_bits():
+    """Reading A8 / SURVEY O4: u_k = (word_k >> 8) * 2^-24 -- the top 24 bits, bit 8 included (a 23-bit
+    fraction (w >> 9) * 2^-23 agrees whenever bit 8 is clear, as in the golden vector above), from words
+    0, 1, 2 in that order of the counter (s_lo, s_hi, half-sweep counter, 0) under the key (seed_lo, seed_hi)."""
+    rng = np.random.default_rng(41)
+    bit8 = [0, 0, 0]
+    for _ in range(100):
+        seed = int(rng.integers(0, 2 ** 63)) * 2 + int(rng.integers(0, 2))
+        ctr = int(rng.integers(0, 2 ** 32))
+        s = int(rng.integers(0, 2 ** 40))
+        words = oracle.philox4x32_10([s & 0xffffffff, s >> 32, ctr, 0], [seed & 0xffffffff, seed >> 32])
+        u = oracle.site_uniforms(seed, ctr, s)
+        for k in range(3):
+            assert u[k] == (words[k] >> 8) / 2.0 ** 24
+            assert u[k] * 2 ** 24 == float(words[k] >> 8)          # a 24-bit integer, exactly
+            bit8[k] += (words[k] >> 8) & 1
+    assert all(20 < b < 80 for b in bit8)                          # the lowest kept bit is set about half the time
+    # all-ones site, counter and seed: the high words of s and of the seed are used
+    u = oracle.site_uniforms(0xffffffffffffffff, 0xffffffff, 0xffffffffffffffff)
+    w3 = oracle.philox4x32_10([0xffffffff] * 3 + [0], [0xffffffff] * 2)
+    assert list(u) == [(w >> 8) / 2.0 ** 24 for w in w3[:3]]
+
+
 # ------------------------------------------------- eq. 9: the SU(2) closed form (PAPER.md:73)
 
 def test_eq9_literal_for_an_su2_block():
@@ -114,6 +137,60 @@ def test_site_g_is_the_ordered_product_of_three_subgroup_maximisers():
     assert np.allclose(g, gc, atol=1e-14)
     assert np.allclose(g @ g.conj().T, np.eye(3), atol=1e-14)
     assert abs(np.linalg.det(g) - 1) < 1e-14
+
+
+def test_site_g_composition_with_overrelaxation_and_stochastic_draws():
+    """Readings A5-A8 for the variants of PAPER.md:80 and :84: EVERY one of the three SU(2) factors is
+    overrelaxed with the same omega, and subgroup k takes the draw u_k -- pinned against the ordered numpy
+    product of the separately pinned su2_vector / su2_update steps, with three different draws straddling p."""
+    rng = np.random.default_rng(30)
+    for trial in range(4):
+        K = rng.standard_normal((3, 3)) + 1j * rng.standard_normal((3, 3))
+        cases = [(oracle.OVERRELAX, 1.7, 0.0, (0.0, 0.0, 0.0))]
+        # every pattern of "square / do not square" over the three subgroups
+        for mask in range(8):
+            cases.append((oracle.STOCHASTIC, 1.0, 0.5, tuple(0.1 if mask >> k & 1 else 0.9 for k in range(3))))
+        seen = []
+        for algo, omega, p, u in cases:
+            g = oracle.site_g(K, algo, omega, p, u)
+            Kc, gc = K.copy(), np.eye(3, dtype=complex)
+            for k, (i, j) in enumerate(SUBGROUPS):
+                E = embed(oracle.su2_update(oracle.su2_vector(Kc, i, j), algo, omega, p, u[k]), i, j)
+                Kc, gc = E @ Kc, E @ gc
+            assert np.allclose(g, gc, atol=1e-14), (algo, u)
+            assert np.allclose(g @ g.conj().T, np.eye(3), atol=1e-14) and abs(np.linalg.det(g) - 1) < 1e-14
+            seen.append(g)
+        for a in range(len(seen)):                       # all nine variants really are different updates
+            for b in range(a + 1, len(seen)):
+                assert np.abs(seen[a] - seen[b]).max() > 1e-3
+
+
+def test_site_g_closed_form_per_subgroup_on_a_real_rotation():
+    """K = a real rotation by phi embedded in ONE subgroup (i,j): the other two subgroups see a real diagonal
+    block, i.e. v proportional to (1,0,0,0), and do nothing, so g must be exactly the embedded SU(2) answer:
+      relaxation (eq. 9):        rotation by -phi  (g K = 1)
+      overrelaxation (A7):       rotation by -phi', tan phi' = omega sin phi / (omega cos phi + 1 - omega)
+      stochastic (A8), u_k < p:  rotation by -2 phi; u_k >= p: rotation by -phi,
+    whichever of the three subgroups it is -- also the last one -- and whatever the OTHER two draws are."""
+    omega, p = 1.7, 0.5
+    for k, (i, j) in enumerate(SUBGROUPS):
+        for phi in (0.3, -0.8, 1.2):
+            def rot(angle):
+                R = np.eye(3, dtype=complex)
+                R[i, i] = R[j, j] = math.cos(angle)
+                R[i, j], R[j, i] = math.sin(angle), -math.sin(angle)
+                return R
+            K = 2.5 * rot(phi)
+            assert np.allclose(oracle.site_g(K, oracle.RELAX), rot(-phi), atol=1e-15)
+            phi_or = math.atan2(omega * math.sin(phi), omega * math.cos(phi) + 1 - omega)
+            assert abs(phi_or) > abs(phi) * 1.2                      # it does overshoot
+            assert np.allclose(oracle.site_g(K, oracle.OVERRELAX, omega), rot(-phi_or), atol=1e-15)
+            others_low = [0.9] * 3
+            others_low[k] = 0.1                                      # only subgroup k squares
+            assert np.allclose(oracle.site_g(K, oracle.STOCHASTIC, 1.0, p, others_low), rot(-2 * phi), atol=1e-15)
+            others_high = [0.1] * 3
+            others_high[k] = 0.9                                     # every subgroup but k squares (the identity)
+            assert np.allclose(oracle.site_g(K, oracle.STOCHASTIC, 1.0, p, others_high), rot(-phi), atol=1e-15)
 
 
 def test_zero_K_gives_identity():
@@ -274,6 +351,60 @@ def test_plaquette_is_gauge_invariant_and_links_stay_in_SU3():
         d_unit, d_det = oracle.unitarity_defect(W, DIMS)
         assert d_unit < 1e-12 and d_det < 1e-12
         assert not np.allclose(W, U)
+
+
+def test_unitarity_defect_on_links_with_a_known_defect():
+    """SURVEY 8(c) O6 / acceptance (4): out[0] = max_{links, entries} |U U^dagger - 1|, out[1] = max |det U - 1|,
+    on fields whose defect is known in closed form -- the checker behind every "links stay in SU(3)" assertion.
+      U -> (1 + d) U:            U U^dagger - 1 = (2d + d^2) 1,    det = (1 + d)^3
+      two rows swapped:          still unitary,                    det = -1
+      U -> e^{i phi} U:          still unitary,                    det = e^{3 i phi}, |det - 1| = 2 |sin(3 phi / 2)|
+      U = 1 + e E_01 (shear):    U U^dagger - 1 = e (E_01 + E_10) + e^2 E_00,  det = 1
+    each planted on a single link (first, last, middle, any mu) of an otherwise exact SU(3) field."""
+    dims = (4, 4, 6, 2)
+    U0 = gi.hot_links(dims, 77)
+    base = oracle.unitarity_defect(U0, dims)
+    assert base[0] < 1e-14 and base[1] < 1e-14
+    flat_shape = (-1, 4, 3, 3)
+    V = int(np.prod(dims))
+    spots = [(0, 0), (V - 1, 3), (V // 2 + 3, 1), (17, 2)]
+    d = 1e-3
+    for s, mu in spots:
+        U = U0.copy()
+        U.reshape(flat_shape)[s, mu] *= 1 + d
+        du, dd = oracle.unitarity_defect(U, dims)
+        assert abs(du - (2 * d + d * d)) < 1e-14 and abs(dd - ((1 + d) ** 3 - 1)) < 1e-14
+        U = U0.copy()
+        L = U.reshape(flat_shape)[s, mu]
+        L[[0, 1]] = L[[1, 0]]
+        du, dd = oracle.unitarity_defect(U, dims)
+        assert du < 1e-14 and abs(dd - 2.0) < 1e-14
+        U = U0.copy()
+        phi = 0.2
+        U.reshape(flat_shape)[s, mu] *= np.exp(1j * phi)
+        du, dd = oracle.unitarity_defect(U, dims)
+        assert du < 1e-14 and abs(dd - 2 * abs(math.sin(1.5 * phi))) < 1e-14
+        U = U0.copy()
+        e = 0.25
+        shear = np.eye(3, dtype=complex)
+        shear[0, 1] = e
+        U.reshape(flat_shape)[s, mu] = shear
+        du, dd = oracle.unitarity_defect(U, dims)
+        assert abs(du - e) < 1e-15 and dd < 1e-14          # dd: the rounding of the other (Haar) links
+    # the two outputs are maxima over all links, independently: two different links carry the two worst defects
+    U = U0.copy()
+    U.reshape(flat_shape)[5, 0] *= 1 + d
+    U.reshape(flat_shape)[9, 3] *= np.exp(0.4j)
+    du, dd = oracle.unitarity_defect(U, dims)
+    assert abs(du - (2 * d + d * d)) < 1e-14 and abs(dd - 2 * math.sin(0.6)) < 1e-14
+    # and against a library routine on a generically perturbed field
+    rng = np.random.default_rng(78)
+    U = U0 + 1e-3 * (rng.standard_normal(U0.shape) + 1j * rng.standard_normal(U0.shape))
+    du, dd = oracle.unitarity_defect(np.ascontiguousarray(U), dims)
+    UUd = np.einsum("...ab,...cb->...ac", U, U.conj()) - np.eye(3)
+    assert abs(du - np.abs(UUd).max()) < 1e-15
+    assert abs(dd - np.abs(np.linalg.det(U) - 1).max()) < 1e-15
+    assert du > 1e-3 and dd > 1e-4
 
 
 def test_F_non_decreasing_under_relaxation():
