@@ -146,7 +146,9 @@ int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional, double* h
  * untouched fp64 input is transformed by the re-projected G (gf_transform_cast +
  * gf_apply_transform), and fp64 iterations continue, accumulating into the fp64 transformation:
  * the result equals G(x) U_mu(x) G(x+mu)^dagger of the input to fp64 accuracy and G is returned
- * in the fp64 transformation buffer.  *iters_out = iterations done (both phases), *theta_out = last theta.
+ * in the fp64 transformation buffer.  *iters_out = iterations done (both phases), *theta_out = last theta;
+ * with GF_MIXED / GF_MIXED_EXACT theta is always (re-)measured on the fp64 result, also when the fp32 phase
+ * already met the target or used up max_iter.
  * Returns GF_OK, or GF_NOT_CONVERGED (valid outputs) when max_iter was reached.  Synchronises. */
 int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int precision, double theta_target,
                  int max_iter, int check_every, int* iters_out, double* theta_out);
@@ -203,6 +205,11 @@ int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precision, int dst_
  * gf_set_slice_mask: explicit control for gf_sweep: host_active[t] != 0 means the sites of slice t
  * are visited (N_t bytes, HOST pointer, copied before returning); NULL = all slices.  gf_fix_until
  * with freeze_slices manages the mask itself and leaves it off.
+ * While a deferred update is outstanding the transformation buffer of that precision holds the only copy of
+ * what still has to be applied to U_0: gf_transform_identity, gf_transform_pack, gf_transform_cast INTO it and
+ * gf_set_transform replacing it return GF_ESTATE until gf_coulomb_finish (or a call that finishes implicitly)
+ * has run; gf_apply_transform / gf_cast into ANOTHER precision's field drop that field's own outstanding update
+ * (the field is overwritten).
  * Errors: GF_EINVAL (Landau context, bad flag), GF_ESTATE (no transformation buffer). */
 int gf_set_coulomb_mode(gf_ctx* ctx, int defer_temporal, int freeze_slices);
 int gf_coulomb_finish(gf_ctx* ctx, int precision);
@@ -235,6 +242,16 @@ int gf_set_slice_mask(gf_ctx* ctx, const uint8_t* host_active);
 int gf_set_slab(gf_ctx* ctx, int rank, int nranks, void* dev_prev_links_f64, void* dev_prev_links_f32,
                 void* dev_next_links_f64, void* dev_next_links_f32, uint32_t* dev_flag_own,
                 uint32_t* dev_flag_prev, uint32_t* dev_flag_next);
+
+/* Devices.  A context belongs to the CUDA device that was current in gf_init_lattice (the one its buffers and
+ * stream live on); every call makes that device current for its duration and restores the caller's, so one
+ * process may drive contexts on several GPUs.  gf_get_device returns it.  gf_enable_peer(ctx, peer_device):
+ * enables peer access from the context's device to peer_device (no-op for the same device or when already
+ * enabled) -- needed before gf_set_slab is given pointers into a field on another GPU of the same process.
+ * Errors: GF_EINVAL (no such device), GF_ECUDA (the two devices are not peers).  Multi-GPU slabs have not run
+ * on hardware in this repository's pool (one GPU); see DESIGN.md section 12. */
+int gf_enable_peer(gf_ctx* ctx, int peer_device);
+int gf_get_device(const gf_ctx* ctx, int* device_out);
 
 /* Sets the Philox key and the half-sweep counter (checkpoint/resume: the RNG state is just these). */
 int gf_set_rng(gf_ctx* ctx, uint64_t seed, uint32_t half_sweep_counter);

@@ -61,6 +61,8 @@ def _load():
         "gf_coulomb_finish": (i32, [vp, i32]),
         "gf_set_slice_mask": (i32, [vp, C.c_char_p]),
         "gf_set_slab": (i32, [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp]),
+        "gf_enable_peer": (i32, [vp, i32]),
+        "gf_get_device": (i32, [vp, ip]),
         "gf_set_rng": (i32, [vp, u64, u32]),
         "gf_get_counter": (i32, [vp, C.POINTER(u32)]),
         "gf_reunitarize": (i32, [vp, i32]),
@@ -86,7 +88,7 @@ lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
            "gf_sweep gf_iterate gf_set_wavefront gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
-           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
+           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_enable_peer gf_get_device gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
 
 
@@ -267,6 +269,16 @@ def gf_set_slice_mask(ctx, active, check=True):
 def gf_set_slab(ctx, rank, nranks, prev_f64, prev_f32, next_f64, next_f32, flag_own, flag_prev, flag_next, check=True):
     return _rc(ctx, lib.gf_set_slab(ctx, int(rank), int(nranks), prev_f64 or None, prev_f32 or None, next_f64 or None,
                                     next_f32 or None, flag_own or None, flag_prev or None, flag_next or None), check)
+
+
+def gf_enable_peer(ctx, peer_device, check=True):
+    return _rc(ctx, lib.gf_enable_peer(ctx, int(peer_device)), check)
+
+
+def gf_get_device(ctx):
+    d = C.c_int(-1)
+    _rc(ctx, lib.gf_get_device(ctx, C.byref(d)))
+    return d.value
 
 
 def gf_plaquette(ctx, precision, check=True):

@@ -1,6 +1,8 @@
 // gf_api.cu -- the C ABI of include/gf.h: argument checks, the context, the host-side fix loop
 // and the mixed-precision hand-off.  No arithmetic of the method runs on the
-// host: every step is one of the kernels in gf_sweep.cu / gf_aux.cu.
+// host: every step is one of the kernels in gf_sweep.cu / gf_aux.cu, the reductions included
+// (sums over time slices and the normalisations of F and theta are done by reduce_slices_kernel);
+// the host compares theta with the target and, in Coulomb gauge, takes the maximum over slices.
 #include <cuda.h>
 
 #include <cstdarg>
@@ -14,6 +16,7 @@
 using namespace gf;
 
 extern "C" int gf_transform_identity(gf_ctx* ctx, int precision);
+static int write_identity(gf_ctx* ctx, int precision);
 extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision);
 static int upload_mask(gf_ctx* ctx);
 
@@ -49,8 +52,11 @@ struct gf_ctx {
     uint32_t epoch;             // operations this slab has enqueued
     CUresult (*wait32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
     CUresult (*write32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+    int device;                 // CUDA device the buffers and the stream belong to; every entry point runs under it
     double* workspace;
     double* partials;           // workspace: per-block partial sums
+    double* slice_tmp;          // workspace: 2 doubles per time slice (reduce_slices_kernel, whole-lattice sums)
+    uint32_t* reduce_counter;   // workspace: blocks of the last reduction stage that have finished (zero between launches)
     double* slice_out;          // 2 doubles per time slice, written by the last reduction kernel: the DEVICE ADDRESS OF
                                 // host_pinned (zero-copy: the result is in host memory when the stream has drained)
     double* host_pinned;        // 2 * Nt doubles
@@ -86,6 +92,24 @@ static int cuda_fail(gf_ctx* ctx, cudaError_t e, const char* what)
 {
     return fail(ctx, GF_ECUDA, "%s: %s", what, cudaGetErrorString(e));
 }
+
+// Makes the context's device current for the duration of a call (streams, launches and stream memory
+// operations need it) and restores the caller's device afterwards: one process may drive contexts on
+// several GPUs (slabs.SlabSet).
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const gf_ctx* ctx)
+    {
+        if (ctx && cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) switched = cudaSetDevice(ctx->device) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
 
 static bool dims_ok(const int dims[4])
 {
@@ -152,6 +176,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->recon = recon;
     c->links[PREC_F32] = dev_links_f32;
     c->links[PREC_F64] = dev_links_f64;
+    c->device = dev;
     c->workspace = static_cast<double*>(dev_workspace);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->seed = seed;
@@ -159,9 +184,11 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
     c->mg = measure_grid(dims);
     c->partials = c->workspace;
-    c->dev_mask = reinterpret_cast<uint8_t*>(c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2 + (size_t)dims[0] * 2);
+    c->slice_tmp = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
+    c->dev_mask = reinterpret_cast<uint8_t*>(c->slice_tmp + (size_t)dims[0] * 2);
     c->wave_ticket = reinterpret_cast<unsigned long long*>(c->dev_mask + kMaxNt);
     c->wave_error = reinterpret_cast<uint32_t*>(c->wave_ticket + 1);
+    c->reduce_counter = c->wave_error + 1;
     c->wave_done = c->wave_error + 2;
     c->wave_mode = 0;         // opt-in: see gf_set_wavefront
 
@@ -211,6 +238,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     }
     if (cudaHostGetDevicePointer(reinterpret_cast<void**>(&c->slice_out), c->host_pinned, 0) != cudaSuccess) {
         cudaGetLastError();
+        cudaFreeHost(c->host_slots);
         cudaFreeHost(c->host_pinned);
         delete c;
         return GF_ECUDA;
@@ -222,6 +250,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
 extern "C" void gf_destroy(gf_ctx* ctx)
 {
     if (!ctx) return;
+    DeviceGuard guard(ctx);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     if (ctx->host_slots) cudaFreeHost(ctx->host_slots);
     delete ctx;
@@ -271,10 +300,41 @@ static int slab_end(gf_ctx* ctx)
         if (rc_) return rc_;            \
     } while (0)
 
+// Slabs on different GPUs driven by one process: the kernels of this context dereference pointers into the
+// neighbour's field, which needs peer access from this context's device to the neighbour's.
+extern "C" int gf_enable_peer(gf_ctx* ctx, int peer_device)
+{
+    DeviceGuard guard(ctx);
+    if (!ctx) return GF_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) return cuda_fail(ctx, cudaGetLastError(), "gf_enable_peer");
+    if (peer_device < 0 || peer_device >= ndev) return fail(ctx, GF_EINVAL, "no CUDA device %d", peer_device);
+    if (peer_device == ctx->device) return GF_OK;
+    int can = 0;
+    cudaError_t e = cudaDeviceCanAccessPeer(&can, ctx->device, peer_device);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_enable_peer");
+    if (!can) return fail(ctx, GF_ECUDA, "device %d cannot access device %d as a peer", ctx->device, peer_device);
+    e = cudaDeviceEnablePeerAccess(peer_device, 0);
+    if (e == cudaErrorPeerAccessAlreadyEnabled) {
+        cudaGetLastError();
+        e = cudaSuccess;
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaDeviceEnablePeerAccess");
+    return GF_OK;
+}
+
+extern "C" int gf_get_device(const gf_ctx* ctx, int* device_out)
+{
+    if (!ctx || !device_out) return GF_EINVAL;
+    *device_out = ctx->device;
+    return GF_OK;
+}
+
 extern "C" int gf_set_slab(gf_ctx* ctx, int rank, int nranks, void* dev_prev_links_f64, void* dev_prev_links_f32,
                            void* dev_next_links_f64, void* dev_next_links_f32, uint32_t* dev_flag_own,
                            uint32_t* dev_flag_prev, uint32_t* dev_flag_next)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (nranks < 1 || rank < 0 || rank >= nranks) return fail(ctx, GF_EINVAL, "bad slab rank %d of %d", rank, nranks);
     if ((uint64_t)ctx->V * (uint64_t)nranks >= (uint64_t(1) << 32)) return fail(ctx, GF_EINVAL, "global volume must stay below 2^32 sites");
@@ -315,10 +375,11 @@ extern "C" int gf_set_slab(gf_ctx* ctx, int rank, int nranks, void* dev_prev_lin
 
 extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
-    ctx->pending[precision] = 0;      // the field is overwritten: nothing left to apply
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    ctx->pending[precision] = 0;      // the field is overwritten: nothing left to apply
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_pack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_pack");
@@ -329,6 +390,7 @@ extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_
 
 extern "C" int gf_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     rc = gf_coulomb_finish(ctx, precision);
@@ -346,6 +408,7 @@ static size_t canonical_bytes(const gf_ctx* ctx, int is_f64) { return ctx->V * 4
 
 extern "C" int gf_load_host(gf_ctx* ctx, const void* host_canonical, int canonical_is_f64, int precision, void* dev_staging)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (!host_canonical || !dev_staging) return fail(ctx, GF_EINVAL, "null host or staging pointer");
@@ -356,6 +419,7 @@ extern "C" int gf_load_host(gf_ctx* ctx, const void* host_canonical, int canonic
 
 extern "C" int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is_f64, int precision, void* dev_staging)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (!host_canonical || !dev_staging) return fail(ctx, GF_EINVAL, "null host or staging pointer");
@@ -400,7 +464,7 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
         if (!ctx->gtrans[precision])
             return fail(ctx, GF_ESTATE, "deferred temporal links need a transformation buffer for precision %d (gf_set_transform)", precision);
         if (!ctx->pending[precision]) {      // G(x) restarts from the identity: it is what gf_coulomb_finish will apply
-            int rc = gf_transform_identity(ctx, precision);
+            int rc = write_identity(ctx, precision);
             if (rc) return rc;
             ctx->pending[precision] = 1;
         }
@@ -501,6 +565,7 @@ static int enqueue_iteration(gf_ctx* ctx, int algo, double omega, double p, int 
 
 extern "C" int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, int precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (n < 0) return fail(ctx, GF_EINVAL, "negative iteration count");
@@ -515,6 +580,7 @@ extern "C" int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, 
 
 extern "C" int gf_set_wavefront(gf_ctx* ctx, int mode)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (mode < 0 || mode > 2) return fail(ctx, GF_EINVAL, "wavefront mode must be 0 (off), 1 (automatic) or 2 (whenever eligible)");
     ctx->wave_mode = mode;
@@ -523,6 +589,7 @@ extern "C" int gf_set_wavefront(gf_ctx* ctx, int mode)
 
 extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (parity != 0 && parity != 1) return fail(ctx, GF_EINVAL, "parity must be 0 or 1");
@@ -531,13 +598,43 @@ extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double 
     return enqueue_sweep(ctx, parity, algo, omega, p, precision);
 }
 
-// Runs the measurement kernels and leaves per-slice sums (F, theta) in ctx->host_pinned.
+// Last reduction stage of F / theta: Landau 1/(Nc Nd V) and 1/(Nc V) over the whole lattice (on slabs:
+// this slab's share of the global sums, the caller adds the slabs up); Coulomb per slice 1/(Nc 3 Ns^3) and 1/(Nc Ns^3).
+static ReduceTail measure_tail(const gf_ctx* ctx)
+{
+    ReduceTail t;
+    t.slice_tmp = ctx->slice_tmp;
+    t.counter = ctx->reduce_counter;
+    if (ctx->gauge == GF_COULOMB) {
+        const double Vs = (double)(ctx->V / ctx->dims[0]);
+        t.combine = 0;
+        t.scale0 = 1.0 / (3.0 * 3.0 * Vs);
+        t.scale1 = 1.0 / (3.0 * Vs);
+    } else {
+        t.combine = 1;
+        t.scale0 = 1.0 / (3.0 * 4.0 * (double)ctx->V * ctx->slab_n);
+        t.scale1 = 1.0 / (3.0 * (double)ctx->V * ctx->slab_n);
+    }
+    return t;
+}
+
+static ReduceTail lattice_tail(const gf_ctx* ctx, double scale)
+{
+    ReduceTail t;
+    t.slice_tmp = ctx->slice_tmp;
+    t.counter = ctx->reduce_counter;
+    t.combine = 1;
+    t.scale0 = t.scale1 = scale;
+    return t;
+}
+
+// Runs the measurement kernels and leaves F and theta (Coulomb: per slice, interleaved) in ctx->host_pinned.
 static int measure_to_host(gf_ctx* ctx, int precision)
 {
     const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0, ctx->mg,
-                                   ctx->partials, ctx->slice_out, ctx->stream);
+                                   ctx->partials, measure_tail(ctx), ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
     GF_SLAB_END(ctx);
     ctx->launches += 2;
@@ -550,38 +647,28 @@ static int measure_to_host(gf_ctx* ctx, int precision)
     return GF_OK;
 }
 
-// Normalises the slice sums: Landau 1/(Nc Nd V) and 1/(Nc V); Coulomb per slice
-// 1/(Nc 3 Ns^3) and 1/(Nc Ns^3).  Returns max_t theta_t (Landau: theta).
+// Copies the results the reduction kernels left in (mapped) host memory: Landau (F, theta), Coulomb (F_t, theta_t)
+// per slice.  Returns theta, in Coulomb gauge max_t theta_t -- what the fix loop compares with its target.
 static double finish_measure(const gf_ctx* ctx, double* host_F, double* host_theta, const double* sums = nullptr)
 {
-    const int nt = ctx->dims[0];
     const double* s = sums ? sums : ctx->host_pinned;
-    if (ctx->gauge == GF_COULOMB) {
-        const double Vs = (double)(ctx->V / nt);
-        double worst = 0.0;
-        for (int t = 0; t < nt; ++t) {
-            const double F = s[2 * t] / (3.0 * 3.0 * Vs), th = s[2 * t + 1] / (3.0 * Vs);
-            if (host_F) host_F[t] = F;
-            if (host_theta) host_theta[t] = th;
-            if (th > worst || t == 0) worst = th;
-        }
-        return worst;
+    if (ctx->gauge != GF_COULOMB) {
+        if (host_F) host_F[0] = s[0];
+        if (host_theta) host_theta[0] = s[1];
+        return s[1];
     }
-    double F = 0.0, th = 0.0;
-    for (int t = 0; t < nt; ++t) {
-        F += s[2 * t];
-        th += s[2 * t + 1];
+    double worst = 0.0;
+    for (int t = 0; t < ctx->dims[0]; ++t) {
+        if (host_F) host_F[t] = s[2 * t];
+        if (host_theta) host_theta[t] = s[2 * t + 1];
+        if (s[2 * t + 1] > worst || t == 0) worst = s[2 * t + 1];
     }
-    // on slabs: this slab's share of the global sums (the caller adds the slabs up)
-    F /= 3.0 * 4.0 * (double)ctx->V * ctx->slab_n;
-    th /= 3.0 * (double)ctx->V * ctx->slab_n;
-    if (host_F) host_F[0] = F;
-    if (host_theta) host_theta[0] = th;
-    return th;
+    return worst;
 }
 
 extern "C" int gf_measure(gf_ctx* ctx, int precision, double* host_functional, double* host_theta)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     rc = measure_to_host(ctx, precision);
@@ -592,13 +679,14 @@ extern "C" int gf_measure(gf_ctx* ctx, int precision, double* host_functional, d
 
 extern "C" int gf_measure_async(gf_ctx* ctx, int precision, int slot)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (slot < 0 || slot >= kAsyncSlots) return fail(ctx, GF_EINVAL, "slot must be 0..%d", kAsyncSlots - 1);
     const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0, ctx->mg,
-                                   ctx->partials, ctx->slots_dev + (size_t)slot * 2 * ctx->dims[0], ctx->stream);
+                                   ctx->partials, measure_tail(ctx), ctx->slots_dev + (size_t)slot * 2 * ctx->dims[0], ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
     GF_SLAB_END(ctx);
     ctx->launches += 2;
@@ -608,6 +696,7 @@ extern "C" int gf_measure_async(gf_ctx* ctx, int precision, int slot)
 
 extern "C" int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional, double* host_theta)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (slot < 0 || slot >= kAsyncSlots) return fail(ctx, GF_EINVAL, "slot must be 0..%d", kAsyncSlots - 1);
     if (ctx->slot_precision[slot] < 0) return fail(ctx, GF_ESTATE, "nothing was measured into slot %d", slot);
@@ -620,12 +709,14 @@ extern "C" int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional
 
 extern "C" int gf_functional(gf_ctx* ctx, int precision, double* host_out)
 {
+    DeviceGuard guard(ctx);
     if (ctx && !host_out) return fail(ctx, GF_EINVAL, "null output");
     return gf_measure(ctx, precision, host_out, nullptr);
 }
 
 extern "C" int gf_theta(gf_ctx* ctx, int precision, double* host_out)
 {
+    DeviceGuard guard(ctx);
     if (ctx && !host_out) return fail(ctx, GF_EINVAL, "null output");
     return gf_measure(ctx, precision, nullptr, host_out);
 }
@@ -660,10 +751,9 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
         if (freeze) {
             // reading A17b: a slice below the target stops being swept; nothing that enters its F_t and
             // theta_t changes afterwards, so max_t theta_t above remains the stopping criterion
-            const double Vs = (double)(ctx->V / ctx->dims[0]);
             bool changed = false;
             for (int t = 0; t < ctx->dims[0]; ++t)
-                if (ctx->host_mask[t] && ctx->host_pinned[2 * t + 1] / (3.0 * Vs) < target) {
+                if (ctx->host_mask[t] && ctx->host_pinned[2 * t + 1] < target) {
                     ctx->host_mask[t] = 0;
                     changed = true;
                 }
@@ -678,9 +768,25 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
     return rc;
 }
 
+// Second phase of the mixed-precision runs.  The fp64 field has just been produced from the fp32 phase (cast +
+// re-projection, or the replayed transformation): theta is re-measured on IT -- the value returned always
+// refers to the fp64 result, never to the fp32 field -- and the fp64 iterations run while it is above the
+// target and iterations are left.
+static int finish_in_f64(gf_ctx* ctx, int algo, double omega, double p, double target, int max_iter, int check_every,
+                         int* it_io, double* theta_out)
+{
+    int e = measure_to_host(ctx, GF_F64);
+    if (e != GF_OK) return e;
+    *theta_out = finish_measure(ctx, nullptr, nullptr);
+    if (*theta_out < target) return GF_OK;
+    if (*it_io >= max_iter) return GF_NOT_CONVERGED;
+    return fix_phase(ctx, algo, omega, p, GF_F64, target, max_iter, check_every, it_io, theta_out);
+}
+
 extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int precision, double theta_target,
                             int max_iter, int check_every, int* iters_out, double* theta_out)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     const bool mixed = precision == GF_MIXED || precision == GF_MIXED_EXACT;
     if (precision != GF_F32 && precision != GF_F64 && !mixed) return fail(ctx, GF_EINVAL, "bad precision");
@@ -706,12 +812,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
         if (rc < 0) return rc;
         int e = gf_cast(ctx, GF_F32, GF_F64);
         if (e != GF_OK) return e;
-        if (rc == GF_OK && !(theta < theta_target)) rc = fix_phase(ctx, algo, omega, p, GF_F64, theta_target, max_iter, check_every, &it, &theta);
-        else if (rc == GF_NOT_CONVERGED) {
-            e = measure_to_host(ctx, GF_F64);
-            if (e != GF_OK) return e;
-            theta = finish_measure(ctx, nullptr, nullptr);
-        }
+        rc = finish_in_f64(ctx, algo, omega, p, theta_target, max_iter, check_every, &it, &theta);
     } else if (precision == GF_MIXED_EXACT) {
         // fp32 sweeps on a copy, recording G(x); then the untouched fp64 input is transformed by the
         // re-projected G (gauge equivalent to the input at fp64 accuracy) and the fp64 phase goes on
@@ -725,13 +826,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
         e = gf_transform_cast(ctx, GF_F32, GF_F64);
         if (e == GF_OK) e = gf_apply_transform(ctx, GF_F64, GF_F64, GF_F64);
         if (e != GF_OK) return e;
-        if (rc == GF_OK && !(theta < theta_target)) rc = fix_phase(ctx, algo, omega, p, GF_F64, theta_target, max_iter, check_every, &it, &theta);
-        else {
-            e = measure_to_host(ctx, GF_F64);
-            if (e != GF_OK) return e;
-            theta = finish_measure(ctx, nullptr, nullptr);
-            if (rc == GF_OK && !(theta < theta_target)) rc = GF_NOT_CONVERGED;
-        }
+        rc = finish_in_f64(ctx, algo, omega, p, theta_target, max_iter, check_every, &it, &theta);
     } else {
         if (max_iter == 0) {
             rc = measure_to_host(ctx, precision);
@@ -754,6 +849,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
 
 extern "C" int gf_set_rng(gf_ctx* ctx, uint64_t seed, uint32_t half_sweep_counter)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     ctx->seed = seed;
     ctx->counter = half_sweep_counter;
@@ -769,6 +865,7 @@ extern "C" int gf_get_counter(const gf_ctx* ctx, uint32_t* half_sweep_counter_ou
 
 extern "C" int gf_reunitarize(gf_ctx* ctx, int precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     rc = gf_coulomb_finish(ctx, precision);
@@ -783,14 +880,15 @@ extern "C" int gf_reunitarize(gf_ctx* ctx, int precision)
 
 extern "C" int gf_cast(gf_ctx* ctx, int from_precision, int to_precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, from_precision);
     if (rc) return rc;
     rc = check_prec(ctx, to_precision);
     if (rc) return rc;
+    if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_cast needs two different precisions");
     rc = gf_coulomb_finish(ctx, from_precision);
     if (rc) return rc;
-    ctx->pending[to_precision] = 0;
-    if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_cast needs two different precisions");
+    ctx->pending[to_precision] = 0;   // the destination field is overwritten: nothing left to apply to it
     const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_cast(from_precision, to_precision, ctx->recon, ctx->links[from_precision], ctx->links[to_precision],
@@ -804,9 +902,12 @@ extern "C" int gf_cast(gf_ctx* ctx, int from_precision, int to_precision)
 // ---------------------------------------------------------- the accumulated transformation
 extern "C" int gf_set_transform(gf_ctx* ctx, void* dev_g_f64, void* dev_g_f32)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (((uintptr_t)dev_g_f64 | (uintptr_t)dev_g_f32) & 15u) return fail(ctx, GF_EINVAL, "transformation buffers must be 16-byte aligned");
     if (ctx->slab_n > 1 && (dev_g_f64 || dev_g_f32)) return fail(ctx, GF_ESTATE, "the transformation field is not available on slabs");
+    if ((ctx->pending[PREC_F64] && dev_g_f64 != ctx->gtrans[PREC_F64]) || (ctx->pending[PREC_F32] && dev_g_f32 != ctx->gtrans[PREC_F32]))
+        return fail(ctx, GF_ESTATE, "a transformation buffer holds a deferred temporal update: call gf_coulomb_finish before replacing it");
     ctx->gtrans[PREC_F64] = dev_g_f64;
     ctx->gtrans[PREC_F32] = dev_g_f32;
     return GF_OK;
@@ -820,19 +921,38 @@ static int check_transform(gf_ctx* ctx, int precision)
     return GF_OK;
 }
 
-extern "C" int gf_transform_identity(gf_ctx* ctx, int precision)
+// While a deferred temporal update is outstanding (gf_set_coulomb_mode) the transformation buffer holds the only
+// copy of what still has to be applied to U_0: nothing may overwrite it before gf_coulomb_finish.
+static int check_transform_writable(gf_ctx* ctx, int precision)
 {
     int rc = check_transform(ctx, precision);
     if (rc) return rc;
+    if (ctx->pending[precision])
+        return fail(ctx, GF_ESTATE, "the transformation buffer of precision %d holds a deferred temporal update: call gf_coulomb_finish first",
+                    precision);
+    return GF_OK;
+}
+
+static int write_identity(gf_ctx* ctx, int precision)
+{
     cudaError_t e = launch_transform_identity(precision, ctx->recon, ctx->gtrans[precision], ctx->G, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_identity");
     ctx->launches += 1;
     return GF_OK;
 }
 
+extern "C" int gf_transform_identity(gf_ctx* ctx, int precision)
+{
+    DeviceGuard guard(ctx);
+    int rc = check_transform_writable(ctx, precision);
+    if (rc) return rc;
+    return write_identity(ctx, precision);
+}
+
 extern "C" int gf_transform_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision)
 {
-    int rc = check_transform(ctx, precision);
+    DeviceGuard guard(ctx);
+    int rc = check_transform_writable(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
     cudaError_t e = launch_transform_pack(precision, ctx->recon, ctx->gtrans[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
@@ -843,6 +963,7 @@ extern "C" int gf_transform_pack(gf_ctx* ctx, const void* dev_canonical, int can
 
 extern "C" int gf_transform_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64, int precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_transform(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
@@ -854,9 +975,10 @@ extern "C" int gf_transform_unpack(gf_ctx* ctx, void* dev_canonical, int canonic
 
 extern "C" int gf_transform_cast(gf_ctx* ctx, int from_precision, int to_precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_transform(ctx, from_precision);
     if (rc) return rc;
-    rc = check_transform(ctx, to_precision);
+    rc = check_transform_writable(ctx, to_precision);
     if (rc) return rc;
     if (from_precision == to_precision) return fail(ctx, GF_EINVAL, "gf_transform_cast needs two different precisions");
     const int reproject = from_precision == GF_F32 && to_precision == GF_F64;
@@ -869,6 +991,7 @@ extern "C" int gf_transform_cast(gf_ctx* ctx, int from_precision, int to_precisi
 
 extern "C" int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precision, int dst_precision)
 {
+    DeviceGuard guard(ctx);
     int rc = check_transform(ctx, g_precision);
     if (rc) return rc;
     rc = check_prec(ctx, src_precision);
@@ -877,6 +1000,11 @@ extern "C" int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precisio
     if (rc) return rc;
     rc = gf_coulomb_finish(ctx, src_precision);
     if (rc) return rc;
+    if (dst_precision != src_precision && ctx->pending[dst_precision]) {
+        // the destination field is overwritten: its own outstanding update has nothing left to act on.  If its G is
+        // the transformation asked for, it has to be used as it stands, so only the flag is dropped.
+        ctx->pending[dst_precision] = 0;
+    }
     cudaError_t e = launch_apply_transform(g_precision, src_precision, dst_precision, ctx->recon, ctx->gtrans[g_precision],
                                            ctx->links[src_precision], ctx->links[dst_precision], ctx->G, 0, 4, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_apply_transform");
@@ -887,6 +1015,7 @@ extern "C" int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precisio
 // ------------------------------------------------------------------- Coulomb specialisation
 extern "C" int gf_set_coulomb_mode(gf_ctx* ctx, int defer_temporal, int freeze_slices)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if ((defer_temporal != 0 && defer_temporal != 1) || (freeze_slices != 0 && freeze_slices != 1))
         return fail(ctx, GF_EINVAL, "defer_temporal and freeze_slices must be 0 or 1");
@@ -914,6 +1043,7 @@ static int upload_mask(gf_ctx* ctx)
 
 extern "C" int gf_set_slice_mask(gf_ctx* ctx, const uint8_t* host_active)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (ctx->gauge != GF_COULOMB && host_active) return fail(ctx, GF_EINVAL, "slice masks exist in Coulomb gauge only");
     if (!host_active) {
@@ -930,6 +1060,7 @@ extern "C" int gf_set_slice_mask(gf_ctx* ctx, const uint8_t* host_active)
 
 extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
     if (!ctx->pending[precision]) return GF_OK;
@@ -954,6 +1085,7 @@ static int slices_to_host(gf_ctx* ctx, const char* what)
 
 extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     rc = gf_coulomb_finish(ctx, precision);
@@ -961,40 +1093,39 @@ extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)
     if (!host_out) return fail(ctx, GF_EINVAL, "null output");
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_plaquette(precision, ctx->recon, ctx->links[precision], ctx->next_links[precision], ctx->G, ctx->mg,
-                                     ctx->partials, ctx->slice_out, ctx->stream);
+                                     ctx->partials, lattice_tail(ctx, 1.0 / (6.0 * 3.0 * (double)ctx->V * ctx->slab_n)), ctx->slice_out,
+                                     ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_plaquette launch");
     GF_SLAB_END(ctx);
     rc = slices_to_host(ctx, "gf_plaquette copy");
     if (rc) return rc;
-    double sum = 0.0;
-    for (int t = 0; t < ctx->dims[0]; ++t) sum += ctx->host_pinned[2 * t];
-    *host_out = sum / (6.0 * 3.0 * (double)ctx->V * ctx->slab_n);
+    *host_out = ctx->host_pinned[0];
     return GF_OK;
 }
 
 extern "C" int gf_unitarity(gf_ctx* ctx, int precision, double* host_out2)
 {
+    DeviceGuard guard(ctx);
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!host_out2) return fail(ctx, GF_EINVAL, "null output");
     GF_SLAB_BEGIN(ctx);
-    cudaError_t e = launch_unitarity(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, ctx->slice_out, ctx->stream);
+    cudaError_t e = launch_unitarity(precision, ctx->recon, ctx->links[precision], ctx->G, ctx->mg, ctx->partials, lattice_tail(ctx, 1.0),
+                                     ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_unitarity launch");
     GF_SLAB_END(ctx);
     rc = slices_to_host(ctx, "gf_unitarity copy");
     if (rc) return rc;
-    host_out2[0] = host_out2[1] = 0.0;
-    for (int t = 0; t < ctx->dims[0]; ++t) {
-        if (ctx->host_pinned[2 * t] > host_out2[0]) host_out2[0] = ctx->host_pinned[2 * t];
-        if (ctx->host_pinned[2 * t + 1] > host_out2[1]) host_out2[1] = ctx->host_pinned[2 * t + 1];
-    }
+    host_out2[0] = ctx->host_pinned[0];
+    host_out2[1] = ctx->host_pinned[1];
     return GF_OK;
 }
 
 extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_threads)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (precision != GF_F32 && precision != GF_F64) return fail(ctx, GF_EINVAL, "precision must be GF_F32 or GF_F64");
     if (!sweep_config_valid(lanes_per_site ? lanes_per_site : 1, block_threads ? block_threads : 64))
@@ -1006,6 +1137,7 @@ extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int
 
 extern "C" int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (!(theta_handoff > 0.0)) return fail(ctx, GF_EINVAL, "the hand-off theta must be positive");
     ctx->handoff = theta_handoff;
@@ -1014,6 +1146,7 @@ extern "C" int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff)
 
 extern "C" int gf_set_traversal(gf_ctx* ctx, int zigzag)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (zigzag != 0 && zigzag != 1) return fail(ctx, GF_EINVAL, "traversal must be 0 (forward) or 1 (zigzag)");
     ctx->zigzag = zigzag;
@@ -1022,6 +1155,7 @@ extern "C" int gf_set_traversal(gf_ctx* ctx, int zigzag)
 
 extern "C" int gf_set_solver_precision(gf_ctx* ctx, int solver_precision)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (solver_precision != GF_F32 && solver_precision != GF_F64 && solver_precision != GF_SOLVER_AUTO)
         return fail(ctx, GF_EINVAL, "solver precision must be GF_F32, GF_F64 or GF_SOLVER_AUTO");
@@ -1031,6 +1165,7 @@ extern "C" int gf_set_solver_precision(gf_ctx* ctx, int solver_precision)
 
 extern "C" int gf_debug_philox(gf_ctx* ctx, int n, const uint32_t* dev_counters, const uint32_t* dev_keys, uint32_t* dev_out)
 {
+    DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
     if (n < 0 || !dev_counters || !dev_keys || !dev_out) return fail(ctx, GF_EINVAL, "bad arguments");
     if (n == 0) return GF_OK;

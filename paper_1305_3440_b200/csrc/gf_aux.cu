@@ -48,17 +48,54 @@ __device__ __forceinline__ void block_reduce2(double a, double b, double* out)
     }
 }
 
-// One block per time slice: combines that slice's per-block partials in a fixed order.
+// a9, last stage.  One block per time slice combines that slice's per-block partials in a fixed order and
+// scales them (the normalisations of PAPER.md:39 and :52).  COMBINE = 0 (Coulomb gauge: one value per
+// time slice): out[2t], out[2t+1].  COMBINE = 1 (values of the whole lattice): the slice values go to
+// slice_tmp and the block that finishes last -- known from a counter it resets -- folds all N_t of
+// them, again in a fixed order, into out[0], out[1].  `out` may be mapped pinned host memory: the host
+// reads finished results and does no arithmetic of the method.
+
 template <typename Op>
-__global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32_t per_slice, double* __restrict__ out)
+__global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32_t per_slice, const ReduceTail tail,
+                                     double* __restrict__ out)
 {
+    __shared__ double res[2];
+    __shared__ uint32_t last;
     const double* p = partials + (size_t)blockIdx.x * per_slice * 2;
     double a = 0.0, b = 0.0;
     for (uint32_t i = threadIdx.x; i < per_slice; i += blockDim.x) {
         a = Op::apply(a, p[2 * i]);
         b = Op::apply(b, p[2 * i + 1]);
     }
-    block_reduce2<Op>(a, b, out + 2 * blockIdx.x);
+    block_reduce2<Op>(a, b, res);
+    if (!tail.combine) {
+        if (threadIdx.x == 0) {
+            out[2 * blockIdx.x] = res[0] * tail.scale0;
+            out[2 * blockIdx.x + 1] = res[1] * tail.scale1;
+        }
+        return;
+    }
+    if (threadIdx.x == 0) {
+        tail.slice_tmp[2 * blockIdx.x] = res[0];
+        tail.slice_tmp[2 * blockIdx.x + 1] = res[1];
+        __threadfence();
+        last = atomicAdd(tail.counter, 1u) == gridDim.x - 1u ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    a = b = 0.0;
+    for (uint32_t t = threadIdx.x; t < gridDim.x; t += blockDim.x) {
+        a = Op::apply(a, __ldcg(tail.slice_tmp + 2 * t));
+        b = Op::apply(b, __ldcg(tail.slice_tmp + 2 * t + 1));
+    }
+    __syncthreads();                                    // block_reduce2's scratch is reused
+    block_reduce2<Op>(a, b, res);
+    if (threadIdx.x == 0) {
+        out[0] = res[0] * tail.scale0;
+        out[1] = res[1] * tail.scale1;
+        *tail.counter = 0u;
+    }
 }
 
 // thread -> (slice t, parity, site) of the measurement grids: blockIdx.y = t, blockIdx.x = 2*chunk + parity
@@ -232,52 +269,52 @@ static dim3 measure_dims(const Geom& G, const MeasureGrid& mg) { return dim3(2u 
 
 template <typename T, int RECON> struct MeasureLauncher {
     static cudaError_t run(const void* links, const void* prev_links, const Geom& G, int mu0, const MeasureGrid& mg, double* partials,
-                           double* slice_out, cudaStream_t st)
+                           const ReduceTail& tail, double* slice_out, cudaStream_t st)
     {
         measure_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
                                                                            static_cast<const T*>(prev_links ? prev_links : links), G, mu0, mg, partials);
-        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
+        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
         return cudaGetLastError();
     }
 };
 
 template <typename T, int RECON> struct PlaquetteLauncher {
     static cudaError_t run(const void* links, const void* next_links, const Geom& G, const MeasureGrid& mg, double* partials,
-                           double* slice_out, cudaStream_t st)
+                           const ReduceTail& tail, double* slice_out, cudaStream_t st)
     {
         plaquette_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
                                                                              static_cast<const T*>(next_links ? next_links : links), G, mg, partials);
-        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
+        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
         return cudaGetLastError();
     }
 };
 
 template <typename T, int RECON> struct UnitarityLauncher {
     static cudaError_t run(const void* links, const Geom& G, const MeasureGrid& mg, double* partials,
-                           double* slice_out, cudaStream_t st)
+                           const ReduceTail& tail, double* slice_out, cudaStream_t st)
     {
         unitarity_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mg, partials);
-        reduce_slices_kernel<OpMax><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, slice_out);
+        reduce_slices_kernel<OpMax><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
         return cudaGetLastError();
     }
 };
 
 cudaError_t launch_measure(int precision, int recon, const void* links, const void* prev_links, const Geom& G, int mu0,
-                           const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
+                           const MeasureGrid& mg, double* partials, const ReduceTail& tail, double* slice_out, cudaStream_t st)
 {
-    return dispatch<MeasureLauncher>(precision, recon, links, prev_links, G, mu0, mg, partials, slice_out, st);
+    return dispatch<MeasureLauncher>(precision, recon, links, prev_links, G, mu0, mg, partials, tail, slice_out, st);
 }
 
 cudaError_t launch_plaquette(int precision, int recon, const void* links, const void* next_links, const Geom& G,
-                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
+                             const MeasureGrid& mg, double* partials, const ReduceTail& tail, double* slice_out, cudaStream_t st)
 {
-    return dispatch<PlaquetteLauncher>(precision, recon, links, next_links, G, mg, partials, slice_out, st);
+    return dispatch<PlaquetteLauncher>(precision, recon, links, next_links, G, mg, partials, tail, slice_out, st);
 }
 
 cudaError_t launch_unitarity(int precision, int recon, const void* links, const Geom& G,
-                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st)
+                             const MeasureGrid& mg, double* partials, const ReduceTail& tail, double* slice_out, cudaStream_t st)
 {
-    return dispatch<UnitarityLauncher>(precision, recon, links, G, mg, partials, slice_out, st);
+    return dispatch<UnitarityLauncher>(precision, recon, links, G, mg, partials, tail, slice_out, st);
 }
 
 // ---------------------------------------------------------------------- pack / unpack / cast

@@ -42,6 +42,14 @@ struct MeasureGrid {
     uint32_t block;         // threads per block
 };
 
+// last stage of a reduction (gf_aux.cu, reduce_slices_kernel)
+struct ReduceTail {
+    double* slice_tmp;      // 2 * N_t doubles of workspace
+    uint32_t* counter;      // device word, zero between launches
+    int combine;            // 0: one (scaled) pair per time slice; 1: one pair for the whole lattice in out[0], out[1]
+    double scale0, scale1;  // normalisations applied to the two sums on the device
+};
+
 // every launcher returns cudaGetLastError() after the launch
 // solver_f64: with fp32 storage, accumulate K(x) and run the SU(2) solves in fp64 registers
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);
@@ -49,11 +57,11 @@ bool sweep_config_valid(int lanes, int block);
 
 // prev_links / next_links: the fields of the slabs below / above in t (NULL = this field, periodic)
 cudaError_t launch_measure(int precision, int recon, const void* links, const void* prev_links, const Geom& G, int mu0,
-                           const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
+                           const MeasureGrid& mg, double* partials, const ReduceTail& tail, double* slice_out, cudaStream_t st);
 cudaError_t launch_plaquette(int precision, int recon, const void* links, const void* next_links, const Geom& G,
-                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
+                             const MeasureGrid& mg, double* partials, const ReduceTail& tail, double* slice_out, cudaStream_t st);
 cudaError_t launch_unitarity(int precision, int recon, const void* links, const Geom& G,
-                             const MeasureGrid& mg, double* partials, double* slice_out, cudaStream_t st);
+                             const MeasureGrid& mg, double* partials, const ReduceTail& tail, double* slice_out, cudaStream_t st);
 cudaError_t launch_pack(int precision, int recon, void* links, const Geom& G, const void* canonical,
                         int canonical_is_f64, cudaStream_t st);
 cudaError_t launch_unpack(int precision, int recon, const void* links, const Geom& G, void* canonical,

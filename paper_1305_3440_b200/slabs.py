@@ -6,10 +6,12 @@ the library's kernels; the slabs share the boundary temporal links in place thro
 pointers (no halo buffers, no collective on the data path).
 
 * ``SlabSet``: all slabs driven by ONE process -- several slabs on one GPU (how the tests check the
-  scheme on this pool's single GPU) or one slab per visible GPU with peer access.
+  scheme on this pool's single GPU).  With several devices each context runs under its own device
+  (the library switches devices per call) and peer access to the two neighbours' devices is enabled
+  with ``gf_enable_peer``; that multi-device path is UNMEASURED ON HARDWARE (this pool has one GPU).
 * ``SlabRank``: one slab per process under ``torch.distributed`` (one rank per GPU); the neighbours'
   fields and flags are mapped with CUDA IPC (torch's shared CUDA storages) and theta is summed
-  with one scalar all-reduce.  Needs >= 2 GPUs: NOT exercised on this pool.
+  with one scalar all-reduce.  Needs >= 2 GPUs: UNMEASURED ON HARDWARE on this pool.
 """
 import torch
 
@@ -50,9 +52,13 @@ class SlabSet:
                 self.fields.append(GaugeField(self.dims, gauge=gauge, recon=recon, precisions=precisions, seed=seed, device=dev))
             self.streams.append(st)
             self.flags.append(torch.zeros(4, dtype=torch.int32, device=dev))
-        torch.cuda.synchronize()
+        for dev in {f.device for f in self.fields}:
+            torch.cuda.synchronize(dev)
         for r, f in enumerate(self.fields):
             lo, hi = neighbours(r, nslabs)
+            for other in (self.fields[lo], self.fields[hi]):
+                if other.device != f.device:        # this slab's kernels dereference pointers into the neighbour's field
+                    B.gf_enable_peer(f.ctx, other.device.index)
             B.gf_set_slab(f.ctx, r, nslabs, _ptr(self.fields[lo], B.GF_F64), _ptr(self.fields[lo], B.GF_F32),
                           _ptr(self.fields[hi], B.GF_F64), _ptr(self.fields[hi], B.GF_F32),
                           self.flags[r].data_ptr(), self.flags[lo].data_ptr(), self.flags[hi].data_ptr())
@@ -61,19 +67,23 @@ class SlabSet:
         for f in self.fields:
             f.close()
 
+    def _sync(self):
+        for dev in {f.device for f in self.fields}:
+            torch.cuda.synchronize(dev)
+
     # every method below issues the same operation on every slab, in slab order
     def pack(self, canonical, precision):
         nt = self.dims[0]
         parts = [canonical[r * nt:(r + 1) * nt].to(f.device).contiguous() for r, f in enumerate(self.fields)]
-        torch.cuda.synchronize()            # the slices were made on torch's stream, the slabs run on their own
+        self._sync()                        # the slices were made on torch's stream, the slabs run on their own
         for f, part in zip(self.fields, parts):
             f.pack(part, precision)
-        torch.cuda.synchronize()
+        self._sync()
 
     def unpack(self, precision, dtype=torch.complex128):
-        torch.cuda.synchronize()
+        self._sync()
         parts = [f.unpack(precision, dtype) for f in self.fields]
-        torch.cuda.synchronize()
+        self._sync()
         return torch.cat([p.to(parts[0].device) for p in parts], dim=0)
 
     def sweep(self, parity, algo, omega, p, precision):
