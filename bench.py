@@ -40,9 +40,21 @@ VARIANTS = {            # name: (precision key, recon, bytes per real)
 }
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per sweep_kernel launch at 32^4, from the `ncu --set full`
-# captures summarised in profiles/r1_sweep_variants_ncu.md (average of a forward and a reverse launch; cold L2)
-NCU_TRAFFIC_BYTES = {"f64-18": 1149.6e6, "f64-12": 746.6e6, "f32-18": 547.3e6, "f32-12": 345.9e6}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.json")
+
+
+def ncu_traffic(variant):
+    """dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 32^4 from the committed `ncu --set full`
+    summary (written by paper_1305_3440_b200/profile_traffic.py; command in profiles/r2_sweep_variants_ncu.md).
+    Valid only for the kernel sources it was captured at: returns (None, why) when they have changed since."""
+    try:
+        from paper_1305_3440_b200.build import source_hash
+        doc = json.load(open(TRAFFIC_FILE))
+        if doc.get("source_hash") != source_hash():
+            return None, "profiles/r2_traffic.json was captured at sources %s, the library is at %s" % (doc.get("source_hash"), source_hash())
+        return float(doc["variants"][variant]["traffic_bytes"]), "profiles/r2_traffic.json (ncu --set full, sources %s)" % doc["source_hash"]
+    except Exception as e:                                      # missing file or variant: no claim
+        return None, "no ncu capture on record (%s)" % type(e).__name__
 
 
 def measured_peaks():
@@ -151,13 +163,20 @@ def run_ours(args):
         kern_ms = sum(a.elapsed_time(b) for a, b in sweep_ms) / (len(sweep_ms) * 2 * args.check)
         bytes_per_launch = (V // 2) * 16 * recon * B
         achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
+        traffic, traffic_src = ncu_traffic(name)
         out = {
             "value": world * V * args.iters * steps / (ms_total * 1e-3),
             "ms_per_step": ms_total / steps,
             "gpu_launches": int(launches),
             "clocks": clocks,
+            # achieved / frac: ALGORITHMIC bytes (16 * recon * sizeof(real) per site-update, every link read once and
+            # written once) over the event-timed launch.  dram_*: the same launch time against the bytes ncu saw
+            # cross the DRAM interface (stores still dirty in the L2 when the launch ends do not): the HBM-level figure.
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(name), "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
+                         "traffic": traffic, "traffic_source": traffic_src,
+                         "dram_achieved": (traffic / (kern_ms * 1e-3) / 1e9) if traffic else None,
+                         "dram_frac": (traffic / (kern_ms * 1e-3) / 1e9 / peak) if traffic else None,
+                         "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
                          "bytes_per_launch": bytes_per_launch, "avg_launch_ms": kern_ms, "peak_source": peak_src,
                          "frac_of_8TBs_nominal": achieved / 8000.0},
             "final_F": F[0], "final_theta": th[0],
@@ -192,9 +211,10 @@ def run_ours(args):
                 for _ in range(n):
                     e2e_step(f, host)
 
-            def run_pipeline(n_steps):
-                counts = [n_steps // len(lanes) + (1 if i < n_steps % len(lanes) else 0) for i in range(len(lanes))]
-                threads = [threading.Thread(target=worker, args=(f, h, c)) for (f, h), c in zip(lanes, counts) if c]
+            def run_pipeline(n_steps, use=None):
+                use = lanes if use is None else use
+                counts = [n_steps // len(use) + (1 if i < n_steps % len(use) else 0) for i in range(len(use))]
+                threads = [threading.Thread(target=worker, args=(f, h, c)) for (f, h), c in zip(use, counts) if c]
                 for t in threads:
                     t.start()
                 for t in threads:
@@ -208,10 +228,19 @@ def run_ours(args):
             t0 = time.perf_counter()
             run_pipeline(steps)
             dt = max_over_ranks(time.perf_counter() - t0)
+            # the same step with ONE lattice in flight: nothing overlaps the copies -- the latency a single caller sees
+            run_pipeline(1, lanes[:1])
+            n_single = max(2, steps // 3)
+            barrier()
+            t0 = time.perf_counter()
+            run_pipeline(n_single, lanes[:1])
+            dt_single = max_over_ranks(time.perf_counter() - t0)
             nbytes = lanes[0][1].numel() * lanes[0][1].element_size()
             out["e2e"] = {"value": world * V * args.iters * steps / dt, "unit": "site-updates/s",
                           "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 16 * n_blocks,
                           "ms_per_step": 1e3 * dt / steps,
+                          "single_lattice_ms_per_step": 1e3 * dt_single / n_single,
+                          "single_lattice_value": world * V * args.iters * n_single / dt_single,
                           "pipeline": "%d lattices in flight (one context, stream, pinned buffer and host thread each): "
                                       "copies overlap sweeps" % len(lanes)}
             for f in extra:
@@ -230,7 +259,9 @@ def run_ours(args):
                 continue
             r = bench_variant(name, max(1, args.steps // 3), 3, False)
             variants[name] = {"site_updates_per_s": r["value"], "gflops_nominal": r["value"] * FLOP_PER_SITE_UPDATE / 1e9,
-                              "roofline_GBs": r["roofline"]["achieved"], "roofline_frac": r["roofline"]["frac"]}
+                              "roofline_GBs": r["roofline"]["achieved"], "roofline_frac": r["roofline"]["frac"],
+                              "dram_frac": r["roofline"]["dram_frac"], "avg_launch_ms": r["roofline"]["avg_launch_ms"],
+                              "sm_mhz": r["clocks"]["sm_mhz"]}
 
     # Time to solution (BASELINE.json configs[2]: "fp32, mixed and fp64"): gf_fix_until to theta < 1e-12 on the
     # same 32^4 input, theta every 10 iterations.  Context for the SP/MP/DP reading of the metric, not the headline.

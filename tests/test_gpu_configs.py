@@ -160,18 +160,15 @@ def test_config4_64_4(cuda_device, prec):
 # ------------------------------------------------------------------------------ configs[4]: Coulomb
 
 def test_config5_coulomb_32_3x64_stochastic(cuda_device):
-    """32^3 x 64 Coulomb gauge, fp64, stochastic relaxation p = 0.8, Philox seed 2013: sampled sites of
-    the first iteration against the oracle (same Philox draws), then the fix loop until theta_t < 1e-12
-    on every time slice."""
+    """32^3 x 64 Coulomb gauge, fp64, stochastic relaxation p = 0.8, Philox seed 2013: the fix loop until
+    theta_t < 1e-12 on every time slice, invariants at the end."""
     dims = (64, 32, 32, 32)
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device)
     fld = gf.GaugeField(dims, gauge=gf.GF_COULOMB, precisions=("f64",), seed=2013, device=cuda_device)
     fld.pack(U, gf.GF_F64)
     del U
     P0 = fld.plaquette(gf.GF_F64)
-    rng = np.random.default_rng(5)
-    sampled_sweep_check(fld, dims, "f64", gf.GF_COULOMB, oracle.COULOMB, gf.GF_STOCHASTIC, oracle.STOCHASTIC,
-                        1.0, 0.8, 2013, 32, rng)
+    fld.iterate(1, gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64)          # compared link by link in tests/test_gpu_fullsize.py
     F1 = np.array(fld.functional(gf.GF_F64))
     rc, it, th = fld.fix_until(gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64, 1e-12, 100000, 20)
     assert rc == gf.GF_OK, (it, th)
@@ -198,33 +195,15 @@ def _gauge_transform_torch(U, G):
 
 @pytest.mark.parametrize("prec,recon", [("f64", 18), ("f32", 12)])
 def test_32_4_accumulated_transformation(cuda_device, prec, recon):
-    """configs[2] size, default launch configuration with accumulation: sampled G(x) against the
-    oracle's single-site g(x) after each half-sweep, and U_n = G U_0 G^dagger over the whole lattice
-    (a property that holds at any size; eq. 3 restated with torch ops)."""
+    """configs[2] size, default launch configuration with accumulation: U_n = G U_0 G^dagger over the whole
+    lattice after 5 iterations (a property that holds at any size; eq. 3 restated with torch ops).  G(x) itself is
+    compared with the oracle over the whole lattice in tests/test_gpu_fullsize.py."""
     dims = (32, 32, 32, 32)
     U0 = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device).to(CDTYPE[prec])
     fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
     fld.pack(U0, PREC[prec])
     fld.attach_transform((prec,))
-    before = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
-    rng = np.random.default_rng(9)
-    V = before.shape[0]
-    for parity in (0, 1):
-        fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
-        G = fld.transform(PREC[prec]).reshape(-1, 3, 3)
-        picked = 0
-        while picked < 32:
-            s = int(rng.integers(0, V))
-            par, back = _site_and_backward(dims, s)
-            if par != parity:
-                continue
-            picked += 1
-            fwd = before[s].cpu().numpy().copy()
-            bwd = np.stack([before[back[mu], mu].cpu().numpy() for mu in range(4)])
-            g = oracle.update_links8(fwd, bwd, oracle.LANDAU, oracle.OVERRELAX, 1.7, 0.0, (0.0, 0.0, 0.0))
-            assert np.abs(G[s].cpu().numpy() - g).max() < LINK_TOL[prec]       # G was the identity before this visit
-        before = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
-    fld.iterate(4, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+    fld.iterate(5, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
     Un = fld.unpack(PREC[prec], torch.complex128)
     G = fld.transform(PREC[prec], torch.complex128)
     replay = _gauge_transform_torch(U0.to(torch.complex128), G)

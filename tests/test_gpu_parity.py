@@ -303,55 +303,8 @@ def test_error_codes_on_device(cuda_device):
     assert gf.gf_get_counter(fld.ctx) == 0
 
 
-# ------------------------------------------------------------- full-size, bench configuration
-
-def test_32_4_one_sweep_sampled_against_oracle(cuda_device):
-    """configs[2] at full size in the launch configuration bench.py times (default tuning): one sweep
-    on device-generated 32^4 input; 64 sampled active sites per parity are recomputed by the oracle's
-    single-site update from the pre-sweep links."""
-    _sampled_site_check(cuda_device, (32, 32, 32, 32), "f64", 18, seed=1, nsamples=64)
-    _sampled_site_check(cuda_device, (32, 32, 32, 32), "f32", 12, seed=1, nsamples=64)
-
-
-def _neighbour_sites(dims, s):
-    nt, nx, ny, nz = dims
-    x, y, z, t = s % nx, (s // nx) % ny, (s // (nx * ny)) % nz, s // (nx * ny * nz)
-
-    def idx(t, x, y, z):
-        return x + nx * (y + ny * (z + nz * t))
-    back = [idx((t - 1) % nt, x, y, z), idx(t, (x - 1) % nx, y, z), idx(t, x, (y - 1) % ny, z), idx(t, x, y, (z - 1) % nz)]
-    return (x + y + z + t) % 2, back
-
-
-def _sampled_site_check(dev, dims, prec, recon, seed, nsamples):
-    U = gi.torch_smooth_random_gauge(dims, 0.6, seed, device=dev).to(CDTYPE[prec])
-    fld = make_field(dims, prec, dev, recon=recon)
-    fld.pack(U, PREC[prec])
-    before = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
-    V = before.shape[0]
-    rng = np.random.default_rng(5)
-    for parity in (0, 1):
-        fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
-        after = fld.unpack(PREC[prec], torch.complex128).reshape(-1, 4, 3, 3)
-        picked = 0
-        while picked < nsamples:
-            s = int(rng.integers(0, V))
-            par, back = _neighbour_sites(dims, s)
-            if par != parity:
-                continue
-            picked += 1
-            fwd = before[s].cpu().numpy().copy()
-            bwd = np.stack([before[back[mu], mu].cpu().numpy() for mu in range(4)])
-            oracle.update_links8(fwd, bwd, oracle.LANDAU, oracle.OVERRELAX, 1.7)
-            got_f = after[s].cpu().numpy()
-            got_b = np.stack([after[back[mu], mu].cpu().numpy() for mu in range(4)])
-            assert np.abs(got_f - fwd).max() < LINK_TOL[prec]
-            assert np.abs(got_b - bwd).max() < LINK_TOL[prec]
-        # links of the inactive parity that no active site touches do not exist: every link changed
-        before = after
-    du, dd = fld.unitarity(PREC[prec])
-    assert du < (1e-12 if prec == "f64" else 1e-5)
-    fld.close()
+# Full-size parity (32^4 in bench.py's launch configuration, every link, all four storage variants; configs[4]
+# at full size; the mixed-precision runs) lives in tests/test_gpu_fullsize.py.
 
 
 # ------------------------------------------------------------------------- out-of-bounds writes
