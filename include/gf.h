@@ -100,22 +100,28 @@ int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is_f64, int p
 int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision);
 
 /* n iterations = n x {parity 0, parity 1}, asynchronous; the Philox counter advances by 2 per
- * iteration exactly as 2n gf_sweep calls would, and the links produced are bitwise the same.
- * When the context is eligible (one lattice, no transformation buffer attached for `precision`,
- * N_t >= 4, block_threads / lanes_per_site divides the sites of a time slice and parity) each
- * iteration is ONE fused launch: the tiles of both parities are handed out in a t-wavefront order
- * (parity-1 sites of slice t right after the parity-0 sites of slice t+2) and every parity-1 tile
- * waits, inside the kernel, for the completion counters of the three time slices it depends on.
- * The second touch of every link then hits the L2 cache: DRAM traffic per iteration is the field
- * read once and written once instead of twice each (measured at 32^4 fp32/18: 657 MB instead of
- * 1150 MB per iteration).  gf_set_wavefront: 0 (default) = never fuse, 1 = fuse when a time slice of
- * links is at most 24 MB (so that ~3 slices stay in the 126 MB L2), 2 = fuse whenever eligible.
- * Off by default: the sweep kernel is latency-bound once DRAM is relieved, so the fused launch is
- * not faster yet.  gf_fix_until iterates through the same path.
- * Errors: as gf_sweep; a later gf_measure / gf_fix_until reports GF_ECUDA if a tile ever gave up
- * waiting (never expected; the wait is bounded so that a fault cannot hang the GPU). */
+ * iteration exactly as 2n gf_sweep calls would.
+ *
+ * The streamed kernel and the fused iteration.  Besides the register kernel behind gf_sweep
+ * the library has a second organisation of the same site update: persistent blocks whose producer warp streams
+ * tiles of 32 sites into a shared-memory ring with TMA bulk copies while consumer warps (one thread per site) compute
+ * out of shared memory.  With it ONE launch can do both half-sweeps of an iteration in a wavefront over the (t,z)
+ * planes: the parity-1 tiles follow the parity-0 tiles `lag` planes behind and every parity-1 tile waits, in the
+ * kernel, for the completion counters of the five planes its links were updated from.  The second touch of every
+ * link then hits the L2 cache: the field crosses the DRAM interface once per iteration instead of twice.
+ * Eligible: a whole lattice (no slabs), no transformation buffer attached for `precision`, no slice mask, N_t >= 4,
+ * Nx/2 even and dividing 32, (Nx/2) * Ny a multiple of 32; otherwise an iteration is two gf_sweep launches.
+ * gf_set_wavefront: 0 = never (default until section 13's measurements say otherwise), 1 = fuse when a time slice of
+ * links is at most 24 MB (so that the ~3 slices between the two fronts stay in the 126 MB L2), 2 = fuse whenever
+ * eligible, 3 = as 2 and gf_sweep itself also goes through the streamed kernel when eligible.
+ * gf_set_wave_tuning: lag in planes (0 = automatic: N_z + planes in flight + 2) and number of persistent blocks
+ * (0 = one per SM).  The links are those of the register kernel with one lane per site (gf_set_tuning lanes = 1).
+ * Errors: as gf_sweep; if a tile ever gives up waiting for a dependency (never expected; the wait is bounded so that
+ * a fault cannot hang the GPU) nothing more is stored by that launch and the next call that synchronises the stream
+ * (gf_measure, gf_measure_collect, gf_fix_until, gf_store_host, gf_plaquette, gf_unitarity) returns GF_ECUDA. */
 int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, int precision);
 int gf_set_wavefront(gf_ctx* ctx, int mode);
+int gf_set_wave_tuning(gf_ctx* ctx, int lag_planes, int blocks);
 
 /* F (eq. 2) and theta (eq. 4-5, with A_mu the traceless
  * anti-Hermitian part of U_mu) of the field of `precision`, accumulated in fp64 with a fixed

@@ -14,12 +14,14 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libgf_b200.so")
-SOURCES = ["gf_sweep.cu", "gf_aux.cu", "gf_api.cu"]
+SOURCES = ["gf_sweep.cu", "gf_wave.cu", "gf_aux.cu", "gf_api.cu"]
 HEADERS = [os.path.join(CSRC, "gf_device.cuh"), os.path.join(CSRC, "gf_internal.h"),
            os.path.join(INCLUDE, "gf.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
+# kernel-variant experiments (e.g. GF_EXTRA_NVCC_FLAGS="-DGF_LAZY12_F64=22"; see profiles/): rebuild with --force
+NVCC_FLAGS += os.environ.get("GF_EXTRA_NVCC_FLAGS", "").split()
 
 
 def source_hash() -> str:

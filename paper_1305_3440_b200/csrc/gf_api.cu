@@ -19,6 +19,15 @@ extern "C" int gf_transform_identity(gf_ctx* ctx, int precision);
 static int write_identity(gf_ctx* ctx, int precision);
 extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision);
 static int upload_mask(gf_ctx* ctx);
+static int sync_and_check(gf_ctx* ctx, const char* what);
+static uint64_t wave_total_tiles_for(const Geom& G, int mode)
+{
+    WaveArgs a;
+    memset(&a, 0, sizeof(a));
+    a.G = G;
+    a.mode = mode;
+    return wave_total_tiles(a);
+}
 
 namespace {
 constexpr int kMeasureBlock = 128;
@@ -38,8 +47,12 @@ struct gf_ctx {
     uint8_t* host_mask;         // pinned copy
     int mask_on;                // the sweeps consult dev_mask
     double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
-    // fused iteration (t-wavefront, gf_sweep.cu): device state in the workspace, running totals on the host
-    int wave_mode;              // 0 never, 1 when eligible and a time slice is small enough for the L2, 2 whenever eligible
+    // streamed sweep / fused iteration (gf_wave.cu): device state in the workspace, running totals on the host
+    int wave_mode;              // 0 never, 1 fused iteration when eligible and a time slice is small enough for the L2,
+                                // 2 whenever eligible, 3 = 2 and single half-sweeps go through the streamed kernel too
+    int wave_lag;               // planes between the two parity fronts; 0 = automatic
+    int wave_ctas;              // persistent blocks; 0 = one per SM
+    int sm_count;
     unsigned long long* wave_ticket;
     uint32_t *wave_done, *wave_error;
     unsigned long long wave_ticket_total;
@@ -147,8 +160,9 @@ extern "C" size_t gf_workspace_bytes(const int dims[4])
 {
     if (!dims_ok(dims)) return 0;
     const MeasureGrid mg = measure_grid(dims);
-    // + the slice mask + the wavefront state (ticket, error word, one completion counter per time slice)
-    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt + 16 + sizeof(uint32_t) * kMaxNt;
+    // + the slice mask + the wavefront state (ticket, error word, reduction counter, one completion counter per (t,z) plane)
+    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt + 16 +
+           sizeof(uint32_t) * (size_t)dims[0] * dims[3];
 }
 
 extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
@@ -216,7 +230,8 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->slab_rank = 0;
     c->slab_n = 1;
 
-    if (cudaMemsetAsync(c->wave_ticket, 0, 16 + sizeof(uint32_t) * kMaxNt, c->stream) != cudaSuccess) {
+    c->sm_count = prop.multiProcessorCount;
+    if (cudaMemsetAsync(c->wave_ticket, 0, 16 + sizeof(uint32_t) * (size_t)dims[0] * dims[3], c->stream) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return GF_ECUDA;
@@ -426,9 +441,8 @@ extern "C" int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is
     rc = gf_unpack(ctx, dev_staging, canonical_is_f64, precision);
     if (rc) return rc;
     cudaError_t e = cudaMemcpyAsync(host_canonical, dev_staging, canonical_bytes(ctx, canonical_is_f64), cudaMemcpyDeviceToHost, ctx->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_store_host copy");
-    return GF_OK;
+    return sync_and_check(ctx, "gf_store_host copy");
 }
 
 static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
@@ -439,8 +453,9 @@ static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
     return GF_OK;
 }
 
-// Launch configuration chosen by measurement on B200 at 32^4 (profiles/r1_tune_32x32x32x32.txt,
-// DESIGN.md "Kernels"): two lanes per site everywhere except fp64 / 12-real (four).
+// Launch configuration chosen by measurement on B200 at 32^4 (profiles/r1_tune_32x32x32x32.txt, profiles/r2_tune_f64_12.txt,
+// DESIGN.md "Kernels"): two lanes per site everywhere except fp64 / 12-real, where one lane per site (no redundant
+// solve, third rows never held in registers) is the variant that stays bandwidth-bound under the power cap.
 static void default_tuning(int precision, int recon, int solver_f64, int accumulate, int defer, int* lanes, int* block)
 {
     if (defer && precision == GF_F32) {      // 6 links + G: one lane per site is balanced and fits the registers
@@ -449,9 +464,8 @@ static void default_tuning(int precision, int recon, int solver_f64, int accumul
         return;
     }
     if (precision == GF_F64) {
-        *lanes = recon == GF_RECON12 ? 4 : 2;
+        *lanes = recon == GF_RECON12 ? 1 : 2;
         *block = recon == GF_RECON12 ? 64 : 128;
-        if (accumulate && recon == GF_RECON12) *lanes = 1;      // one lane does the G(x) update: no imbalance with one lane per site
     } else {
         *lanes = 2;
         *block = (recon == GF_RECON18 && !solver_f64) ? 128 : 64;
@@ -502,43 +516,37 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     return GF_OK;
 }
 
-// Largest time slice (bytes of link storage) for which the fused iteration is chosen automatically: the
-// second touch of a link comes about 2.5 slices after the first and has to find it in the L2
-// (126 MB L2, read-modify-write hits up to a reuse distance of ~75 MB).
+// Largest time slice (bytes of link storage) for which the fused iteration is chosen automatically: the second
+// touch of a link comes about `lag` planes (two to three time slices) after the first and has to find it in the L2.
 static const size_t kWaveMaxSliceBytes = (size_t)24 << 20;
 
-static bool wave_eligible(const gf_ctx* ctx, int precision, int lanes, int block, uint32_t* tiles)
+// The streamed kernel handles the plain site update of one whole lattice: no transformation buffer, no slice mask,
+// no slabs; the lattice must tile (wave_supported).
+static bool stream_eligible(const gf_ctx* ctx, int precision)
 {
-    if (ctx->wave_mode == 0 || ctx->slab_n > 1 || ctx->gtrans[precision] || ctx->dims[0] < 4) return false;
-    const uint32_t sites_per_block = (uint32_t)(block / lanes);
-    if (ctx->mg.Sh % sites_per_block) return false;             // the tiles must cover a slice exactly
+    return ctx->slab_n == 1 && !ctx->gtrans[precision] && !ctx->mask_on && wave_supported(ctx->G) &&
+           wave_total_tiles_for(ctx->G, 2) < (uint64_t(1) << 32);
+}
+
+static bool fused_eligible(const gf_ctx* ctx, int precision)
+{
+    if (ctx->wave_mode == 0 || ctx->dims[0] < 4 || !stream_eligible(ctx, precision)) return false;
     if (ctx->wave_mode == 1) {
         const size_t slice = (size_t)ctx->mg.Sh * 2 * 4 * (size_t)ctx->recon * (precision == GF_F64 ? 8 : 4);
         if (slice > kWaveMaxSliceBytes) return false;
     }
-    *tiles = ctx->mg.Sh / sites_per_block;
     return true;
 }
 
-// One iteration = parity 0 then parity 1 (PAPER.md:88): a single fused launch when eligible, else two half-sweeps.
-static int enqueue_iteration(gf_ctx* ctx, int algo, double omega, double p, int precision)
+// mode 0 / 1: one half-sweep of that parity; mode 2: one fused iteration
+static int enqueue_streamed(gf_ctx* ctx, int mode, int algo, double omega, double p, int precision)
 {
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
-    int lanes, block;
-    default_tuning(precision, ctx->recon, solver_f64, 0, 0, &lanes, &block);
-    if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
-    if (ctx->block[precision]) block = ctx->block[precision];
-    uint32_t tiles = 0;
-    if (!wave_eligible(ctx, precision, lanes, block, &tiles)) {
-        int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
-        if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
-        return e;
-    }
-    SweepArgs a;
+    WaveArgs a;
     memset(&a, 0, sizeof(a));
     a.links = ctx->links[precision];
-    a.slice_active = ctx->mask_on ? ctx->dev_mask : nullptr;
     a.G = ctx->G;
+    a.site_offset = 0;
     a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
     a.algo = algo;
     a.omega = omega;
@@ -546,21 +554,41 @@ static int enqueue_iteration(gf_ctx* ctx, int algo, double omega, double p, int 
     a.key0 = (uint32_t)ctx->seed;
     a.key1 = (uint32_t)(ctx->seed >> 32);
     a.counter = ctx->counter;
-    a.wave = 1;
-    a.wave_ticket = ctx->wave_ticket;
-    a.wave_ticket_base = ctx->wave_ticket_total;
-    a.wave_done = ctx->wave_done;
-    a.wave_done_target = ctx->wave_done_total + tiles;
-    a.wave_tiles = tiles;
-    a.wave_error = ctx->wave_error;
-    cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, lanes, block, a, ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_iterate launch");
-    ctx->wave_ticket_total += 2ull * (unsigned long long)ctx->dims[0] * tiles;
-    ctx->wave_done_total += tiles;
-    ctx->counter += 2;
-    ctx->sweeps += 2;
+    a.mode = mode;
+    a.num_ctas = ctx->wave_ctas > 0 ? ctx->wave_ctas : ctx->sm_count;
+    const uint32_t M = wave_tiles_per_plane(ctx->G), nz = (uint32_t)ctx->dims[3], planes = (uint32_t)ctx->dims[0] * nz;
+    if (mode == 2) {
+        // the parity-1 front follows the parity-0 front by one time slice (the dependency on plane q + Nz) plus the
+        // planes whose parity-0 tiles can be in flight at once (every block's ring), so that the waits rarely spin
+        uint32_t lag = ctx->wave_lag > 0 ? (uint32_t)ctx->wave_lag
+                                         : nz + ((uint32_t)a.num_ctas * wave_stages(precision, ctx->recon) + 2u * M - 1u) / (2u * M) + 2u;
+        if (lag < nz + 1u) lag = nz + 1u;
+        if (lag > planes - nz) lag = planes - nz;
+        a.lag = lag;
+    }
+    a.ticket = ctx->wave_ticket;
+    a.ticket_base = ctx->wave_ticket_total;
+    a.done = ctx->wave_done;
+    a.done_target = ctx->wave_done_total + M;
+    a.error = ctx->wave_error;
+    cudaError_t e = launch_wave(precision, solver_f64, ctx->recon, a, ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "streamed sweep launch");
+    ctx->wave_ticket_total += wave_ticket_advance(a);
+    const int half_sweeps = mode == 2 ? 2 : 1;
+    if (mode == 2) ctx->wave_done_total += M;
+    ctx->counter += half_sweeps;
+    ctx->sweeps += half_sweeps;
     ctx->launches += 1;
     return GF_OK;
+}
+
+// One iteration = parity 0 then parity 1 (PAPER.md:88): a single fused launch when eligible, else two half-sweeps.
+static int enqueue_iteration(gf_ctx* ctx, int algo, double omega, double p, int precision)
+{
+    if (fused_eligible(ctx, precision)) return enqueue_streamed(ctx, 2, algo, omega, p, precision);
+    int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
+    if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
+    return e;
 }
 
 extern "C" int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, int precision)
@@ -582,8 +610,18 @@ extern "C" int gf_set_wavefront(gf_ctx* ctx, int mode)
 {
     DeviceGuard guard(ctx);
     if (!ctx) return GF_EINVAL;
-    if (mode < 0 || mode > 2) return fail(ctx, GF_EINVAL, "wavefront mode must be 0 (off), 1 (automatic) or 2 (whenever eligible)");
+    if (mode < 0 || mode > 3)
+        return fail(ctx, GF_EINVAL, "wavefront mode must be 0 (off), 1 (automatic), 2 (whenever eligible) or 3 (2 + streamed half-sweeps)");
     ctx->wave_mode = mode;
+    return GF_OK;
+}
+
+extern "C" int gf_set_wave_tuning(gf_ctx* ctx, int lag_planes, int blocks)
+{
+    if (!ctx) return GF_EINVAL;
+    if (lag_planes < 0 || blocks < 0 || blocks > 4096) return fail(ctx, GF_EINVAL, "lag and block count must be >= 0 (0 = automatic)");
+    ctx->wave_lag = lag_planes;
+    ctx->wave_ctas = blocks;
     return GF_OK;
 }
 
@@ -595,6 +633,8 @@ extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double 
     if (parity != 0 && parity != 1) return fail(ctx, GF_EINVAL, "parity must be 0 or 1");
     rc = check_algo(ctx, algo, omega, p);
     if (rc) return rc;
+    if (ctx->wave_mode == 3 && !ctx->defer_temporal && stream_eligible(ctx, precision))
+        return enqueue_streamed(ctx, parity, algo, omega, p, precision);
     return enqueue_sweep(ctx, parity, algo, omega, p, precision);
 }
 
@@ -628,6 +668,20 @@ static ReduceTail lattice_tail(const gf_ctx* ctx, double scale)
     return t;
 }
 
+// Synchronises the stream; if streamed sweeps have run, also fetches their error word: a fused iteration whose
+// dependency wait gave up stores nothing further and the field is reported invalid at the next call that synchronises.
+static int sync_and_check(gf_ctx* ctx, const char* what)
+{
+    uint32_t* wave_err = reinterpret_cast<uint32_t*>(ctx->host_mask + kMaxNt);
+    cudaError_t e = cudaSuccess;
+    if (ctx->wave_ticket_total) e = cudaMemcpyAsync(wave_err, ctx->wave_error, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, what);
+    if (ctx->wave_ticket_total && *wave_err)
+        return fail(ctx, GF_ECUDA, "a fused iteration gave up waiting for a dependency: the link field is invalid");
+    return GF_OK;
+}
+
 // Runs the measurement kernels and leaves F and theta (Coulomb: per slice, interleaved) in ctx->host_pinned.
 static int measure_to_host(gf_ctx* ctx, int precision)
 {
@@ -638,13 +692,7 @@ static int measure_to_host(gf_ctx* ctx, int precision)
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
     GF_SLAB_END(ctx);
     ctx->launches += 2;
-    uint32_t* wave_err = reinterpret_cast<uint32_t*>(ctx->host_mask + kMaxNt);
-    if (e == cudaSuccess && ctx->wave_ticket_total)
-        e = cudaMemcpyAsync(wave_err, ctx->wave_error, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "measure copy");
-    if (ctx->wave_ticket_total && *wave_err) return fail(ctx, GF_ECUDA, "a fused iteration gave up waiting for a dependency (field invalid)");
-    return GF_OK;
+    return sync_and_check(ctx, "measure");
 }
 
 // Copies the results the reduction kernels left in (mapped) host memory: Landau (F, theta), Coulomb (F_t, theta_t)
@@ -700,8 +748,8 @@ extern "C" int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional
     if (!ctx) return GF_EINVAL;
     if (slot < 0 || slot >= kAsyncSlots) return fail(ctx, GF_EINVAL, "slot must be 0..%d", kAsyncSlots - 1);
     if (ctx->slot_precision[slot] < 0) return fail(ctx, GF_ESTATE, "nothing was measured into slot %d", slot);
-    cudaError_t e = cudaStreamSynchronize(ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_measure_collect");
+    int rc = sync_and_check(ctx, "gf_measure_collect");
+    if (rc) return rc;
     finish_measure(ctx, host_functional, host_theta, ctx->host_slots + (size_t)slot * 2 * ctx->dims[0]);
     ctx->slot_precision[slot] = -1;
     return GF_OK;
@@ -1078,9 +1126,7 @@ extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision)
 static int slices_to_host(gf_ctx* ctx, const char* what)
 {
     ctx->launches += 2;
-    cudaError_t e = cudaStreamSynchronize(ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, what);
-    return GF_OK;
+    return sync_and_check(ctx, what);
 }
 
 extern "C" int gf_plaquette(gf_ctx* ctx, int precision, double* host_out)

@@ -111,27 +111,25 @@ __host__ __device__ __forceinline__ size_t block_offset(uint32_t parity, int mu,
     return (size_t)(parity * 4u + (uint32_t)mu) * (size_t)recon * (size_t)Vh;   // in reals
 }
 
-// CG: load through L2 only (ld.global.cg).  Needed where another block of the SAME launch may have
-// written the link (the fused wavefront iteration): an L1 line could be stale.
-template <int RECON, bool CG = false>
+template <int RECON>
 __device__ __forceinline__ void load_link(const double* __restrict__ blk, uint32_t Vh, uint32_t h, double (&m)[18])
 {
     const double2* p = reinterpret_cast<const double2*>(blk) + h;
 #pragma unroll
     for (int c = 0; c < RECON / 2; ++c) {
-        const double2 v = CG ? __ldcg(p + (size_t)c * Vh) : p[(size_t)c * Vh];
+        const double2 v = p[(size_t)c * Vh];
         m[2 * c] = v.x;
         m[2 * c + 1] = v.y;
     }
 }
 
-template <int RECON, bool CG = false>
+template <int RECON>
 __device__ __forceinline__ void load_link(const float* __restrict__ blk, uint32_t Vh, uint32_t h, float (&m)[18])
 {
     const float4* p = reinterpret_cast<const float4*>(blk) + h;
 #pragma unroll
     for (int c = 0; c < RECON / 4; ++c) {
-        const float4 v = CG ? __ldcg(p + (size_t)c * Vh) : p[(size_t)c * Vh];
+        const float4 v = p[(size_t)c * Vh];
         m[4 * c] = v.x;
         m[4 * c + 1] = v.y;
         m[4 * c + 2] = v.z;
@@ -139,7 +137,7 @@ __device__ __forceinline__ void load_link(const float* __restrict__ blk, uint32_
     }
     if (RECON == 18) {
         const float2* t = reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + h;
-        const float2 v = CG ? __ldcg(t) : *t;
+        const float2 v = *t;
         m[16] = v.x;
         m[17] = v.y;
     }
@@ -183,6 +181,27 @@ __device__ __forceinline__ void reconstruct_row2(T (&m)[18])
         GF_IM(m, 2, b) = -im;
     }
 }
+
+// the same third row, written to r[6] = (re, im) x 3 instead of into the matrix
+template <typename T>
+__device__ __forceinline__ void row2_of(const T (&m)[18], T (&r)[6])
+{
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const int b1 = (b + 1) % 3, b2 = (b + 2) % 3;
+        const T re = GF_RE(m, 0, b1) * GF_RE(m, 1, b2) - GF_IM(m, 0, b1) * GF_IM(m, 1, b2)
+                   - GF_RE(m, 0, b2) * GF_RE(m, 1, b1) + GF_IM(m, 0, b2) * GF_IM(m, 1, b1);
+        const T im = GF_RE(m, 0, b1) * GF_IM(m, 1, b2) + GF_IM(m, 0, b1) * GF_RE(m, 1, b2)
+                   - GF_RE(m, 0, b2) * GF_IM(m, 1, b1) - GF_IM(m, 0, b2) * GF_RE(m, 1, b1);
+        r[2 * b] = re;
+        r[2 * b + 1] = -im;
+    }
+}
+
+// Tells the compiler that v may have changed: an expression recomputed from it afterwards is not merged with
+// the earlier computation (which would keep that result in registers in between).
+__device__ __forceinline__ void forget(double& v) { asm volatile("" : "+d"(v)); }
+__device__ __forceinline__ void forget(float& v) { asm volatile("" : "+f"(v)); }
 
 __device__ __forceinline__ float gf_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 __device__ __forceinline__ double gf_fma(double a, double b, double c) { return __fma_rn(a, b, c); }

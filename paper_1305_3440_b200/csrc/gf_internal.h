@@ -17,15 +17,6 @@ struct SweepArgs {
     const uint8_t* slice_active;   // per time slice, 0 = frozen; NULL = all active
     void* prev_links;       // slab below (same precision and layout), or NULL = this field (periodic)
     uint32_t site_offset;   // global site index of the slab's first site
-    // fused iteration (both parities in one launch, t-wavefront order; gf_sweep.cu): parity, reverse unused;
-    // the Philox counter is `counter` for parity 0 and counter + 1 for parity 1
-    int wave;
-    unsigned long long* wave_ticket;
-    unsigned long long wave_ticket_base;
-    uint32_t* wave_done;
-    uint32_t wave_done_target;
-    uint32_t wave_tiles;     // blocks per (time slice, parity) = Sh * lanes / block, must divide exactly
-    uint32_t* wave_error;
     Geom G;
     uint32_t parity;        // active parity
     int mu0;                // first direction entering K: 0 Landau, 1 Coulomb
@@ -34,6 +25,25 @@ struct SweepArgs {
     uint32_t key0, key1;    // Philox key = seed
     uint32_t counter;       // half-sweep counter (Philox counter word 2)
     uint32_t reverse;       // traverse the lattice backwards (L2 reuse between consecutive launches)
+};
+
+// the streamed sweep (gf_wave.cu): TMA bulk copies into a shared-memory ring, one thread per site
+struct WaveArgs {
+    void* links;
+    Geom G;
+    uint32_t site_offset;
+    int mu0, algo;
+    double omega, p;
+    uint32_t key0, key1;
+    uint32_t counter;               // half-sweep counter of the (first) half-sweep; the fused iteration uses counter, counter + 1
+    int mode;                       // 0 / 1: one half-sweep of that parity; 2: fused iteration (parity 0 then parity 1)
+    uint32_t lag;                   // mode 2: planes between the parity-0 and the parity-1 front; Nz < lag <= (Nt - 1) Nz
+    unsigned long long* ticket;     // device counter, monotonic over launches
+    unsigned long long ticket_base; // its value when this launch starts
+    uint32_t* done;                 // Nt * Nz device counters, monotonic over launches
+    uint32_t done_target;           // value every done[plane] reaches when the parity-0 tiles of this launch are complete
+    uint32_t* error;                // device word, set if a dependency wait gave up
+    int num_ctas;                   // persistent blocks
 };
 
 struct MeasureGrid {
@@ -54,6 +64,13 @@ struct ReduceTail {
 // solver_f64: with fp32 storage, accumulate K(x) and run the SU(2) solves in fp64 registers
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);
 bool sweep_config_valid(int lanes, int block);
+
+bool wave_supported(const Geom& G);                       // the lattice can be tiled (32 sites = whole x-rows inside one plane)
+uint32_t wave_stages(int precision, int recon);           // depth of the shared-memory ring of that variant
+unsigned long long wave_total_tiles(const WaveArgs& a);
+uint32_t wave_ticket_advance(const WaveArgs& a);          // by how much one launch moves the ticket counter
+uint32_t wave_tiles_per_plane(const Geom& G);             // parity-0 tiles of one plane: what one launch adds to every done[plane]
+cudaError_t launch_wave(int precision, int solver_f64, int recon, const WaveArgs& a, cudaStream_t st);
 
 // prev_links / next_links: the fields of the slabs below / above in t (NULL = this field, periodic)
 cudaError_t launch_measure(int precision, int recon, const void* links, const void* prev_links, const Geom& G, int mu0,

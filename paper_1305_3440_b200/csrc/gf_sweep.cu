@@ -31,79 +31,7 @@ template <typename T, typename TK> struct SweepConsts {
     double p;
     uint32_t key0, key1, counter;
     uint32_t reverse;       // 1: blocks walk the lattice from the last site to the first
-    // WAVE (fused iteration, see wave_schedule): work is handed out by ticket, not by blockIdx
-    unsigned long long* ticket;     // device counter, never reset: ticket = old value - ticket_base
-    unsigned long long ticket_base;
-    uint32_t* done;                 // per time slice: parity-0 tiles completed, monotonic over launches
-    uint32_t done_target;           // value of done[t] once all parity-0 tiles of slice t of THIS launch are complete
-    uint32_t tiles;                 // tiles (blocks) per time slice and parity
-    uint32_t* error;                // set to 1 if a dependency wait gave up (never expected)
 };
-
-// ---------------------------------------------------------------------------------------------
-// Fused iteration ("t-wavefront"): ONE launch does the parity-0 half-sweep and the parity-1
-// half-sweep of an iteration, ordered so that the second touch of every link finds
-// it in the 126 MB L2: the tiles are handed out in the order
-//     E(0) .. E(LAG) | E(s) then O(s-LAG) for s = LAG+1 .. Nt-1 | O(Nt-LAG) .. O(Nt-1), O(0)
-// (E(t) / O(t): the parity-0 / parity-1 sites of time slice t).  O(t) needs the parity-0 updates of
-// all its neighbours, i.e. E(t-1), E(t), E(t+1) complete (periodic in t): its block waits for the
-// three per-slice completion counters.  Tickets are taken when a block STARTS, so everything a
-// block waits for is held by blocks that are already running: no deadlock, whatever the hardware's
-// dispatch order.  E(a) and a concurrently running O(b) never touch the same link: E(a) touches
-// slices a, a-1, O(b) slices b, b-1, and O(b) only starts after E(b-1), E(b), E(b+1).  The links are
-// bitwise those of the two separate half-sweeps.  DRAM traffic per iteration: the field is read once
-// and written once instead of twice each.
-constexpr uint32_t WAVE_LAG = 2;
-
-struct WaveTile {
-    uint32_t parity, t, tile;
-};
-
-__device__ __forceinline__ WaveTile wave_schedule(unsigned long long ticket, uint32_t nt, uint32_t tiles)
-{
-    WaveTile w;
-    const unsigned long long headE = (unsigned long long)(WAVE_LAG + 1) * tiles;          // E(0..LAG)
-    const unsigned long long mid = (unsigned long long)(nt - WAVE_LAG - 1) * 2ull * tiles;  // steps LAG+1..Nt-1
-    if (ticket < headE) {
-        w.parity = 0;
-        w.t = (uint32_t)(ticket / tiles);
-        w.tile = (uint32_t)(ticket % tiles);
-    } else if (ticket < headE + mid) {
-        const unsigned long long k = ticket - headE;
-        const uint32_t s = WAVE_LAG + 1 + (uint32_t)(k / (2ull * tiles));
-        const uint32_t r = (uint32_t)(k % (2ull * tiles));
-        // all of E(s), then all of O(s-LAG): by the time an O tile starts, E(s-LAG+1) was handed out more
-        // than a slice of tiles earlier and is complete, so the dependency waits almost never spin
-        w.parity = r >= tiles ? 1u : 0u;
-        w.tile = w.parity ? r - tiles : r;
-        w.t = w.parity ? s - WAVE_LAG : s;                  // O(1) .. O(Nt-1-LAG)
-    } else {
-        const unsigned long long k = ticket - headE - mid;  // O(Nt-LAG) .. O(Nt-1), O(0)
-        w.parity = 1;
-        w.t = (nt - WAVE_LAG + (uint32_t)(k / tiles)) % nt;
-        w.tile = (uint32_t)(k % tiles);
-    }
-    return w;
-}
-
-__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p)
-{
-    uint32_t v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-
-// waits until done[t] has reached target (wrap-safe); gives up after ~seconds and reports
-__device__ __forceinline__ void wave_wait(const uint32_t* done, uint32_t t, uint32_t target, uint32_t* error)
-{
-    for (uint32_t spins = 0; (int32_t)(ld_acquire_u32(done + t) - target) < 0; ++spins) {
-        __nanosleep(100);
-        if (spins > (1u << 24)) {
-            *error = 1u;
-            break;
-        }
-    }
-}
 
 template <typename T>
 __device__ __forceinline__ T shfl_xor_T(T v, int mask)
@@ -121,7 +49,21 @@ __device__ __forceinline__ T shfl_xor_T(T v, int mask)
 // traffic; U_0(x) <- G(x) U_0(x) G(x+0)^dagger is applied once at the end (gf_coulomb_finish).
 enum { MODE_PLAIN = 0, MODE_ACC = 1, MODE_DEFER = 2 };
 
-template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
+// bit L set: the L-lanes-per-site kernel of that storage type is "lazy".  Measured at 32^4 (sustained runs under the
+// power cap, profiles/r2_tune_f64_12.txt): fp64 with one or two lanes per site goes from 226 to 166 registers (L = 2) and
+// from 81 % to 100 % of the HBM peak; with four lanes it changes nothing.
+#ifndef GF_LAZY12_F64
+#define GF_LAZY12_F64 6
+#endif
+#ifndef GF_LAZY12_F32
+#define GF_LAZY12_F32 0
+#endif
+// which 12-real variants drop the third rows between K(x) and the update (see sweep_body)
+template <typename T, int L> struct Lazy12 {
+    static constexpr bool value = sizeof(T) == 8 ? (GF_LAZY12_F64 >> L) & 1 : (GF_LAZY12_F32 >> L) & 1;
+};
+
+template <typename T, typename TK, int RECON, int L, int MODE>
 __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
 {
     constexpr int S = 32 / L;    // sites per warp
@@ -132,30 +74,10 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     // Alternate half-sweeps walk the lattice in opposite directions (blocks are dispatched in
     // ascending blockIdx order): the launch starts on the sites the previous one finished with,
     // whose links are still in the 126 MB L2.  The result does not depend on the order.
-    uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
-    uint32_t parity = P.parity, counter = P.counter, wave_t = 0;
-    if (WAVE) {
-        __shared__ uint32_t sh_tile[3];
-        if (threadIdx.x == 0) {
-            const WaveTile w = wave_schedule(atomicAdd(P.ticket, 1ull) - P.ticket_base, G.nt, P.tiles);
-            if (w.parity) {
-                wave_wait(P.done, w.t == 0 ? G.nt - 1u : w.t - 1u, P.done_target, P.error);
-                wave_wait(P.done, w.t, P.done_target, P.error);
-                wave_wait(P.done, w.t + 1u == G.nt ? 0u : w.t + 1u, P.done_target, P.error);
-            }
-            __threadfence();
-            sh_tile[0] = w.parity;
-            sh_tile[1] = w.t;
-            sh_tile[2] = w.t * P.tiles + w.tile;
-        }
-        __syncthreads();
-        parity = sh_tile[0];
-        wave_t = sh_tile[1];
-        bid = sh_tile[2];
-        counter += parity;
-    }
+    const uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+    const uint32_t parity = P.parity, counter = P.counter;
     const uint32_t warp = (bid * blockDim.x + threadIdx.x) >> 5;
-    if (!WAVE && warp * S >= G.Vh) return;              // warp-uniform (WAVE: the tiles cover the slices exactly)
+    if (warp * S >= G.Vh) return;                       // warp-uniform
     uint32_t h = warp * S + (lane % S);
     const int j = lane / S;
     bool live = h < G.Vh;
@@ -163,7 +85,7 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     const Site s = decode_site(G, h, parity);
     if (P.slice_active != nullptr) {                    // warp-uniform branch
         live = live && P.slice_active[s.c[0]] != 0;
-        if (!WAVE && !__any_sync(0xffffffffu, live)) return;     // the whole warp sits in frozen slices
+        if (!__any_sync(0xffffffffu, live)) return;     // the whole warp sits in frozen slices
     }
 
     if (MODE == MODE_ACC && j == 0) {
@@ -185,17 +107,21 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
         if (MODE == MODE_DEFER && d == 0 && j == 0) {
             // mu = 0: the temporal links stay where they are; their register slot carries G(x) instead,
             // loaded up front with the links (mu = 0 does not enter K in Coulomb gauge: mu0 = 1)
-            load_link<RECON, WAVE>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, Uf[d]);
+            load_link<RECON>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, Uf[d]);
 #pragma unroll
             for (int k = 0; k < 18; ++k) Ub[d][k] = T(0);
             continue;
         }
-        load_link<RECON, WAVE>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
+        load_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
         // the temporal link below the first local time slice belongs to the slab below
         const T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        load_link<RECON, WAVE>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
+        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
     }
-    if (RECON == 12) {
+    // 12-real storage.  LAZY12: the third rows are never kept: they are formed for K(x) and dropped, and formed
+    // again for the forward links in step a6 (U g^dagger does not need the third row of U at all) -- 24 flops per
+    // forward link for 12 registers per link held across the solve.
+    constexpr bool LAZY12 = RECON == 12 && Lazy12<T, L>::value;
+    if (RECON == 12 && !LAZY12) {
 #pragma unroll
         for (int d = 0; d < ND; ++d) {
             reconstruct_row2(Uf[d]);
@@ -211,13 +137,28 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
         if (mu >= P.mu0) {
+            if (LAZY12) {
+                T rf[6], rb[6];
+                row2_of(Uf[d], rf);
+                row2_of(Ub[d], rb);
 #pragma unroll
-            for (int a = 0; a < 3; ++a)
+                for (int a = 0; a < 3; ++a)
 #pragma unroll
-                for (int b = 0; b < 3; ++b) {
-                    GF_RE(K, a, b) += (TK)GF_RE(Uf[d], a, b) + (TK)GF_RE(Ub[d], b, a);
-                    GF_IM(K, a, b) += (TK)GF_IM(Uf[d], a, b) - (TK)GF_IM(Ub[d], b, a);
-                }
+                    for (int b = 0; b < 3; ++b) {
+                        const T fr = a < 2 ? GF_RE(Uf[d], a, b) : rf[2 * b], fi = a < 2 ? GF_IM(Uf[d], a, b) : rf[2 * b + 1];
+                        const T br = b < 2 ? GF_RE(Ub[d], b, a) : rb[2 * a], bi = b < 2 ? GF_IM(Ub[d], b, a) : rb[2 * a + 1];
+                        GF_RE(K, a, b) += (TK)fr + (TK)br;
+                        GF_IM(K, a, b) += (TK)fi - (TK)bi;
+                    }
+            } else {
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) {
+                        GF_RE(K, a, b) += (TK)GF_RE(Uf[d], a, b) + (TK)GF_RE(Ub[d], b, a);
+                        GF_IM(K, a, b) += (TK)GF_IM(Uf[d], a, b) - (TK)GF_IM(Ub[d], b, a);
+                    }
+            }
         }
     }
 #pragma unroll
@@ -244,18 +185,24 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     for (int k = 0; k < 18; ++k) g[k] = (T)gk[k];
 
     // a6: U_mu(x) <- g U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) g^dagger  (eq. 3)
-    if (!WAVE && !live) return;
-    if (live) {
+    if (!live) return;
+    {
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
         if (MODE == MODE_DEFER && d == 0 && j == 0) {   // G(x) <- g(x) G(x)
             T out[18];
+            if (LAZY12) reconstruct_row2(Uf[d]);
             mul_g_U<ROWS>(g, Uf[d], out);
             store_link<RECON>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, out);
             continue;
         }
         T out[18];
+        if (LAZY12) {                                   // the third row of the forward link again, not merged with a3's
+            forget(GF_RE(Uf[d], 0, 1));
+            forget(GF_RE(Uf[d], 0, 2));
+            reconstruct_row2(Uf[d]);
+        }
         mul_g_U<ROWS>(g, Uf[d], out);
         store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, out);
         mul_U_gdag<ROWS>(Ub[d], g, out);
@@ -265,47 +212,56 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     if (MODE == MODE_ACC && j == 0) {
         T* blk = P.gtrans + (size_t)parity * RECON * G.Vh;
         T Gt[18], out[18];
-        load_link<RECON, WAVE>(blk, G.Vh, h, Gt);
+        load_link<RECON>(blk, G.Vh, h, Gt);
         if (RECON == 12) reconstruct_row2(Gt);
         mul_g_U<ROWS>(g, Gt, out);
         store_link<RECON>(blk, G.Vh, h, out);
     }
     }
-    if (WAVE && parity == 0u) {
-        // publish: all of this tile's stores, then one count on its time slice
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) atomicAdd(P.done + wave_t, 1u);
-    }
 }
 
-template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
+template <typename T, typename TK, int RECON, int L, int MODE>
 __global__ void sweep_kernel(const SweepConsts<T, TK> P)
 {
-    sweep_body<T, TK, RECON, L, MODE, WAVE>(P);
+    sweep_body<T, TK, RECON, L, MODE>(P);
 }
 
 // The fp32 / 18-real two-lane kernels sit at 134-141 registers, just above the 128 that let 16 instead
 // of 12 warps be resident; capping them (no spills with the fp32 solver) buys 3-4 % at 32^4.  Every
 // other variant is better off with the allocation the compiler picks on its own, hence a second
 // entry point instead of bounds on all of them.  Blocks have at most 256 threads (sweep_config_valid).
-template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE = false>
+template <typename T, typename TK, int RECON, int L, int MODE>
 __global__ void __launch_bounds__(256, 2) sweep_kernel_r128(const SweepConsts<T, TK> P)
 {
-    sweep_body<T, TK, RECON, L, MODE, WAVE>(P);
+    sweep_body<T, TK, RECON, L, MODE>(P);
 }
 
 template <typename T, int RECON, int L> struct UseR128 {
     static constexpr bool value = sizeof(T) == 4 && RECON == 18 && L == 2;
 };
 
-template <typename T, typename TK, int RECON, int L, int MODE, bool WAVE>
+// exploration hook: a register cap for one (fp64, 12-real, L) variant, chosen at compile time
+#ifndef GF_CAP_L
+#define GF_CAP_L 0
+#define GF_CAP_MAXT 64
+#define GF_CAP_MINB 1
+#endif
+template <typename T, typename TK, int RECON, int L, int MODE>
+__global__ void __launch_bounds__(GF_CAP_MAXT, GF_CAP_MINB) sweep_kernel_cap(const SweepConsts<T, TK> P)
+{
+    sweep_body<T, TK, RECON, L, MODE>(P);
+}
+
+template <typename T, typename TK, int RECON, int L, int MODE>
 static void launch_kernel(uint32_t grid, int block, cudaStream_t st, const SweepConsts<T, TK>& P)
 {
     if constexpr (UseR128<T, RECON, L>::value)
-        sweep_kernel_r128<T, TK, RECON, L, MODE, WAVE><<<grid, block, 0, st>>>(P);
-    else
-        sweep_kernel<T, TK, RECON, L, MODE, WAVE><<<grid, block, 0, st>>>(P);
+        sweep_kernel_r128<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+    else if constexpr (sizeof(T) == 8 && RECON == 12 && L == GF_CAP_L) {
+        if (block <= GF_CAP_MAXT) sweep_kernel_cap<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+        else sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+    } else
+        sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
 }
 
 template <typename T, typename TK, int RECON, int L>
@@ -327,28 +283,14 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     P.key1 = a.key1;
     P.counter = a.counter;
     P.reverse = a.reverse;
-    if (a.wave) {
-        // one launch = one iteration: 2 * Nt * tiles blocks, work handed out by ticket
-        P.ticket = a.wave_ticket;
-        P.ticket_base = a.wave_ticket_base;
-        P.done = a.wave_done;
-        P.done_target = a.wave_done_target;
-        P.tiles = a.wave_tiles;
-        P.error = a.wave_error;
-        P.parity = 0;
-        P.reverse = 0;
-        const uint32_t wgrid = 2u * a.G.nt * a.wave_tiles;
-        launch_kernel<T, TK, RECON, L, MODE_PLAIN, true>(wgrid, block, st, P);
-        return cudaGetLastError();
-    }
     const uint64_t threads = (uint64_t)a.G.Vh * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);
     if (a.gtrans && a.defer_temporal)
-        launch_kernel<T, TK, RECON, L, MODE_DEFER, false>(grid, block, st, P);
+        launch_kernel<T, TK, RECON, L, MODE_DEFER>(grid, block, st, P);
     else if (a.gtrans)
-        launch_kernel<T, TK, RECON, L, MODE_ACC, false>(grid, block, st, P);
+        launch_kernel<T, TK, RECON, L, MODE_ACC>(grid, block, st, P);
     else
-        launch_kernel<T, TK, RECON, L, MODE_PLAIN, false>(grid, block, st, P);
+        launch_kernel<T, TK, RECON, L, MODE_PLAIN>(grid, block, st, P);
     return cudaGetLastError();
 }
 

@@ -40,13 +40,17 @@ def main():
     ap.add_argument("--variants", nargs="+", default=["f64-18", "f64-12", "f32-18", "f32-12"])
     ap.add_argument("--algo", default="overrelax", choices=sorted(ALGOS))
     ap.add_argument("--iters", type=int, default=50)
+    ap.add_argument("--solver", default="auto", choices=["auto", "f32", "f64"],
+                    help="arithmetic of K(x) and the SU(2) solves with fp32 storage (gf_set_solver_precision)")
+    ap.add_argument("--configs", nargs="*", default=None, metavar="L:B",
+                    help="only these lanes:block pairs (default: the library default and all nine)")
     args = ap.parse_args()
     dev = torch.device("cuda:0")
     dims = tuple(args.dims)
     V = dims[0] * dims[1] * dims[2] * dims[3]
     peak = measured_hbm_gbs()
-    print("# %s, %s, %d iterations per row, percentages of %.1f GB/s; L0 b0 = library default" % (
-        "x".join(map(str, dims)), args.algo, args.iters, peak))
+    print("# %s, %s, solver %s, %d iterations per row, percentages of %.1f GB/s; L0 b0 = library default" % (
+        "x".join(map(str, dims)), args.algo, args.solver, args.iters, peak))
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=dev)
     for name in args.variants:
         pkey, recon = name.split("-")
@@ -56,8 +60,12 @@ def main():
         nbytes = 16 * recon * (8 if pkey == "f64" else 4)
         fld = gf.GaugeField(dims, recon=recon, precisions=(pkey,), device=dev)
         fld.pack(U.to(cdtype).contiguous(), prec)
-        for lanes in (0, 1, 2, 4):
-            for block in ((0,) if lanes == 0 else (64, 128, 256)):
+        fld.set_solver_precision({"auto": gf.GF_SOLVER_AUTO, "f32": gf.GF_F32, "f64": gf.GF_F64}[args.solver])
+        pairs = [(0, 0)] + [(l, b) for l in (1, 2, 4) for b in (64, 128, 256)]
+        if args.configs:
+            pairs = [tuple(int(x) for x in c.split(":")) for c in args.configs]
+        for lanes, block in pairs:
+            if True:
                 fld.set_tuning(prec, lanes, block)
                 fld.iterate(10, ALGOS[args.algo], 1.7, 0.8, prec)
                 torch.cuda.synchronize()

@@ -108,6 +108,29 @@ def test_one_sweep_links_match_oracle(cuda_device, dims, prec, recon, lanes):
             fld.close()
 
 
+def one_ulp_drift(U, dims, og, oalgo, omega, p, seed, samples=3):
+    """How far apart two EXACT (fp64 oracle) runs of 10 sweeps end when their inputs differ by one fp32 ulp in
+    every real (random direction; the largest of `samples` independent perturbations): the relative differences
+    of F and theta.  Oracle-only; used to derive the fp32 tolerance of the stochastic variant."""
+    a32 = np.ascontiguousarray(U.astype(np.complex64)).view(np.float32)
+    rng = np.random.default_rng(12345)
+
+    def run(start):
+        W = np.ascontiguousarray(start.view(np.complex64).astype(np.complex128))
+        for it in range(10):
+            for parity in (0, 1):
+                oracle.sweep(W, dims, parity, og, oalgo, omega, p, seed=seed, half_sweep_counter=2 * it + parity)
+        return np.atleast_1d(oracle.functional(W, dims, og)), np.atleast_1d(oracle.theta(W, dims, og))
+
+    F0, t0 = run(a32)
+    dF = dth = 0.0
+    for _ in range(samples):
+        towards = np.where(rng.random(a32.shape) < 0.5, -np.inf, np.inf).astype(np.float32)
+        F1, t1 = run(np.nextafter(a32, towards))
+        dF, dth = max(dF, float(np.abs(F1 / F0 - 1).max())), max(dth, float(np.abs(t1 / t0 - 1).max()))
+    return dF, dth
+
+
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (8, 8, 8, 8)])
 @pytest.mark.parametrize("prec", ["f64", "f32"])
 @pytest.mark.parametrize("recon", [18, 12])
@@ -115,10 +138,18 @@ def test_ten_sweeps_F_theta_match_oracle(cuda_device, dims, prec, recon):
     for field, U in (("smooth", gi.smooth_random_gauge(dims, 0.5, 41)), ("hot", gi.hot_links(dims, 42))):
         for gauge, og in ((gf.GF_LANDAU, oracle.LANDAU), (gf.GF_COULOMB, oracle.COULOMB)):
             for name, algo, oalgo, omega, p in ALGOS[1:]:
-                # north_star's 1e-10 / 1e-5 is for the overrelaxation runs of the configs.  The stochastic
-                # g -> g^2 step is microcanonical (it does not contract rounding differences), so in fp32 the
-                # two correct implementations drift apart faster: DESIGN.md ("Tolerances") allows 1e-4 there.
-                rtol = 1e-4 if (prec == "f32" and name == "stochastic") else REL_TOL[prec]
+                # north_star: 1e-10 (fp64) / 1e-5 (fp32) relative after 10 sweeps.  One derived exception (DESIGN.md,
+                # "Tolerances"): the stochastic g -> g^2 step is microcanonical, it does not contract differences, and
+                # two EXACT runs whose inputs differ by one fp32 ulp already end further apart than 1e-5 (measured
+                # right here, by the oracle alone).  An fp32 run rounds every link to fp32 once per half-sweep, 20
+                # such perturbations in 10 sweeps, adding in quadrature: the bound for fp32 + stochastic is
+                # sqrt(20) x the one-ulp drift, never below north_star's 1e-5.  (A wrong draw or a wrong update
+                # changes theta by factors, not by 1e-4.)
+                rtol_F = rtol_th = REL_TOL[prec]
+                if prec == "f32" and name == "stochastic":
+                    dF, dth = one_ulp_drift(U, dims, og, oalgo, omega, p, 7)
+                    rtol_F, rtol_th = max(rtol_F, 20 ** 0.5 * dF), max(rtol_th, 20 ** 0.5 * dth)
+                    assert rtol_th < 1e-2                   # the exception stays a small tolerance
                 fld = make_field(dims, prec, cuda_device, gauge, recon, seed=7)
                 fld.pack(to_device(U, prec, cuda_device), PREC[prec])
                 Uo = oracle_input(U, prec)
@@ -129,8 +160,8 @@ def test_ten_sweeps_F_theta_match_oracle(cuda_device, dims, prec, recon):
                 F, th = fld.measure(PREC[prec])
                 Fo = np.atleast_1d(oracle.functional(Uo, dims, og))
                 tho = np.atleast_1d(oracle.theta(Uo, dims, og))
-                assert np.allclose(F, Fo, rtol=rtol, atol=0), (field, name, gauge)
-                assert np.allclose(th, tho, rtol=rtol, atol=0), (field, name, gauge, th, tho)
+                assert np.allclose(F, Fo, rtol=rtol_F, atol=0), (field, name, gauge, rtol_F, np.abs(np.array(F) / Fo - 1).max())
+                assert np.allclose(th, tho, rtol=rtol_th, atol=0), (field, name, gauge, rtol_th, np.abs(np.array(th) / tho - 1).max())
                 # the links themselves drift apart as rounding differences are amplified sweep after sweep
                 # (strongly on the hot field); only a loose bound is meaningful here
                 assert np.abs(get_links(fld, prec) - Uo).max() < (1e-8 if prec == "f64" else 0.1)
