@@ -16,8 +16,8 @@
  *   Canonical link layout (what callers hold): contiguous complex array of shape
  *   (N_t, N_z, N_y, N_x, 4, 3, 3): site s = x + N_x (y + N_y (z + N_z t)), then mu, then the
  *   3x3 matrix row-major, (re, im) interleaved; complex128 or complex64.
- *   The internal device layout (parity-split, 16-byte-chunk structure of arrays, 18 or 12 reals
- *   per link) is private; gf_pack / gf_unpack convert.
+ *   The internal device layout (parity-split, tiles of 32 / 64 sites stored as 16-byte chunks, 18 or
+ *   12 reals per link) is private; gf_pack / gf_unpack convert.
  *
  * Memory and streams
  *   Every DEVICE buffer (link storage, workspace, canonical staging) is allocated by the caller
@@ -51,7 +51,8 @@ enum { GF_F32 = 0, GF_F64 = 1, GF_MIXED = 2, GF_MIXED_EXACT = 3 }; /* precision 
 enum { GF_RELAX = 0, GF_OVERRELAX = 1, GF_STOCHASTIC = 2 }; /* algo: PAPER.md:73, :80, :84 */
 enum { GF_RECON18 = 18, GF_RECON12 = 12 };                /* reals stored per link */
 
-/* Bytes of device memory one internal link field needs: 8 * (V/2) * recon * sizeof(real).
+/* Bytes of device memory one internal link field needs: 8 * ceil(V/2 to whole layout tiles) * recon * sizeof(real)
+ * (tiles of 32 sites in fp64, 64 in fp32: exactly V * 4 * recon * sizeof(real) when V/2 is a multiple of that).
  * precision is GF_F32 or GF_F64.  Returns 0 for invalid arguments. */
 size_t gf_storage_bytes(const int dims[4], int precision, int recon);
 
@@ -110,7 +111,8 @@ int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int prec
  * kernel, for the completion counters of the five planes its links were updated from.  The second touch of every
  * link then hits the L2 cache: the field crosses the DRAM interface once per iteration instead of twice.
  * Eligible: a whole lattice (no slabs), no transformation buffer attached for `precision`, no slice mask, N_t >= 4,
- * Nx/2 even and dividing 32, (Nx/2) * Ny a multiple of 32; otherwise an iteration is two gf_sweep launches.
+ * and a layout tile (W = 32 sites in fp64, 64 in fp32) made of whole x-rows inside one plane: Nx/2 divides W and W
+ * divides (Nx/2) * Ny; otherwise an iteration is two gf_sweep launches.
  * gf_set_wavefront: 0 = never (default until section 13's measurements say otherwise), 1 = fuse when a time slice of
  * links is at most 24 MB (so that the ~3 slices between the two fronts stay in the 126 MB L2), 2 = fuse whenever
  * eligible, 3 = as 2 and gf_sweep itself also goes through the streamed kernel when eligible.

@@ -26,6 +26,7 @@ static uint64_t wave_total_tiles_for(const Geom& G, int mode)
     memset(&a, 0, sizeof(a));
     a.G = G;
     a.mode = mode;
+    a.precision = PREC_F64;          // the narrower tiles: the larger count
     return wave_total_tiles(a);
 }
 
@@ -147,8 +148,9 @@ static MeasureGrid measure_grid(const int dims[4])
 extern "C" size_t gf_storage_bytes(const int dims[4], int precision, int recon)
 {
     if (!dims_ok(dims) || (precision != GF_F32 && precision != GF_F64) || (recon != 18 && recon != 12)) return 0;
-    const size_t V = (size_t)dims[0] * dims[1] * dims[2] * dims[3];
-    return V * 4 * (size_t)recon * (precision == GF_F64 ? 8 : 4);
+    const size_t Vh = (size_t)dims[0] * dims[1] * dims[2] * dims[3] / 2;
+    const size_t tile = precision == GF_F64 ? Tile<double>::W : Tile<float>::W;     // sites per layout tile (gf_device.cuh)
+    return (Vh + tile - 1) / tile * tile * 8 * (size_t)recon * (precision == GF_F64 ? 8 : 4);
 }
 
 extern "C" size_t gf_transform_bytes(const int dims[4], int precision, int recon)
@@ -212,6 +214,8 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     G.ny = dims[2];
     G.nz = dims[3];
     G.Vh = (uint32_t)(c->V / 2);
+    G.Vp[PREC_F32] = (G.Vh + Tile<float>::W - 1u) / Tile<float>::W * Tile<float>::W;
+    G.Vp[PREC_F64] = (G.Vh + Tile<double>::W - 1u) / Tile<double>::W * Tile<double>::W;
     G.extent[0] = dims[0]; G.extent[1] = dims[1]; G.extent[2] = dims[2]; G.extent[3] = dims[3];
     G.stride[1] = 1;
     G.stride[2] = G.nxh;
@@ -524,7 +528,7 @@ static const size_t kWaveMaxSliceBytes = (size_t)24 << 20;
 // no slabs; the lattice must tile (wave_supported).
 static bool stream_eligible(const gf_ctx* ctx, int precision)
 {
-    return ctx->slab_n == 1 && !ctx->gtrans[precision] && !ctx->mask_on && wave_supported(ctx->G) &&
+    return ctx->slab_n == 1 && !ctx->gtrans[precision] && !ctx->mask_on && wave_supported(ctx->G, precision) &&
            wave_total_tiles_for(ctx->G, 2) < (uint64_t(1) << 32);
 }
 
@@ -544,6 +548,7 @@ static int enqueue_streamed(gf_ctx* ctx, int mode, int algo, double omega, doubl
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
     WaveArgs a;
     memset(&a, 0, sizeof(a));
+    a.precision = precision;
     a.links = ctx->links[precision];
     a.G = ctx->G;
     a.site_offset = 0;
@@ -556,7 +561,7 @@ static int enqueue_streamed(gf_ctx* ctx, int mode, int algo, double omega, doubl
     a.counter = ctx->counter;
     a.mode = mode;
     a.num_ctas = ctx->wave_ctas > 0 ? ctx->wave_ctas : ctx->sm_count;
-    const uint32_t M = wave_tiles_per_plane(ctx->G), nz = (uint32_t)ctx->dims[3], planes = (uint32_t)ctx->dims[0] * nz;
+    const uint32_t M = wave_tiles_per_plane(ctx->G, precision), nz = (uint32_t)ctx->dims[3], planes = (uint32_t)ctx->dims[0] * nz;
     if (mode == 2) {
         // the parity-1 front follows the parity-0 front by one time slice (the dependency on plane q + Nz) plus the
         // planes whose parity-0 tiles can be in flight at once (every block's ring), so that the waits rarely spin
@@ -569,13 +574,13 @@ static int enqueue_streamed(gf_ctx* ctx, int mode, int algo, double omega, doubl
     a.ticket = ctx->wave_ticket;
     a.ticket_base = ctx->wave_ticket_total;
     a.done = ctx->wave_done;
-    a.done_target = ctx->wave_done_total + M;
+    a.done_target = ctx->wave_done_total + wave_counts_per_plane(ctx->G, precision);
     a.error = ctx->wave_error;
     cudaError_t e = launch_wave(precision, solver_f64, ctx->recon, a, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "streamed sweep launch");
     ctx->wave_ticket_total += wave_ticket_advance(a);
     const int half_sweeps = mode == 2 ? 2 : 1;
-    if (mode == 2) ctx->wave_done_total += M;
+    if (mode == 2) ctx->wave_done_total += wave_counts_per_plane(ctx->G, precision);
     ctx->counter += half_sweeps;
     ctx->sweeps += half_sweeps;
     ctx->launches += 1;

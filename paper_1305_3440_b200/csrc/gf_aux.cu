@@ -133,9 +133,9 @@ __global__ void measure_kernel(const T* __restrict__ links, const T* __restrict_
     for (int mu = 0; mu < 4; ++mu) {
         if (mu < mu0) continue;
         T Uf[18], Ub[18];
-        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, s.h, Uf);
+        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G), s.h, Uf);
         const T* back = (mu == 0 && s.c[0] == 0) ? prev_links : links;     // slab below for the first local slice
-        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, backward_index(G, s, mu), Ub);
+        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), backward_index(G, s, mu), Ub);
         if (RECON == 12) {
             reconstruct_row2(Uf);
             reconstruct_row2(Ub);
@@ -170,7 +170,7 @@ template <typename T, int RECON>
 __device__ __forceinline__ void load_full_d(const T* links, const Geom& G, uint32_t parity, int mu, uint32_t h, double (&m)[18])
 {
     T u[18];
-    load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, u);
+    load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G), h, u);
     if (RECON == 12) reconstruct_row2(u);
 #pragma unroll
     for (int k = 0; k < 18; ++k) m[k] = (double)u[k];
@@ -338,7 +338,7 @@ __global__ void pack_kernel(T* __restrict__ links, const Geom G, const TC* __res
         T m[18];
 #pragma unroll
         for (int k = 0; k < 18; ++k) m[k] = (T)src[k];
-        store_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, m);
+        store_link<RECON>(links + block_offset<T>(parity, mu, RECON, G), h, m);
     }
 }
 
@@ -353,7 +353,7 @@ __global__ void unpack_kernel(const T* __restrict__ links, const Geom G, TC* __r
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
         T m[18];
-        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, m);
+        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G), h, m);
         if (RECON == 12) reconstruct_row2(m);
         TC* dst = canonical + (site * 4 + mu) * 18;
 #pragma unroll
@@ -398,7 +398,7 @@ __global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int repr
     if (h >= G.Vh) return;
     const uint32_t pm = blockIdx.y;                  // parity*4 + mu
     TS u[18];
-    load_link<RECON>(src + (size_t)pm * RECON * G.Vh, G.Vh, h, u);
+    load_link<RECON>(src + (size_t)pm * RECON * padded_vh<TS>(G), h, u);
     double m[18];
 #pragma unroll
     for (int k = 0; k < 18; ++k) m[k] = (double)u[k];
@@ -406,7 +406,7 @@ __global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int repr
     TD o[18];
 #pragma unroll
     for (int k = 0; k < 18; ++k) o[k] = (TD)m[k];
-    store_link<RECON>(dst + (size_t)pm * RECON * G.Vh, G.Vh, h, o);
+    store_link<RECON>(dst + (size_t)pm * RECON * padded_vh<TD>(G), h, o);
 }
 
 template <typename T, int RECON>
@@ -482,14 +482,14 @@ __global__ void transform_convert_kernel(T* __restrict__ gtrans, const Geom G, T
     const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
     const Site s = decode_site(G, h, parity);
     TC* c = canonical + (2u * (size_t)h + s.xodd) * 18;
-    T* blk = gtrans + (size_t)parity * RECON * G.Vh;
+    T* blk = gtrans + (size_t)parity * RECON * padded_vh<T>(G);
     T m[18];
     if (TO_INTERNAL) {
 #pragma unroll
         for (int k = 0; k < 18; ++k) m[k] = (T)c[k];
-        store_link<RECON>(blk, G.Vh, h, m);
+        store_link<RECON>(blk, h, m);
     } else {
-        load_link<RECON>(blk, G.Vh, h, m);
+        load_link<RECON>(blk, h, m);
         if (RECON == 12) reconstruct_row2(m);
 #pragma unroll
         for (int k = 0; k < 18; ++k) c[k] = (TC)m[k];
@@ -506,7 +506,7 @@ __global__ void transform_identity_kernel(T* __restrict__ gtrans, const Geom G)
 #pragma unroll
     for (int k = 0; k < 18; ++k) m[k] = T(0);
     m[0] = m[8] = m[16] = T(1);
-    store_link<RECON>(gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, m);
+    store_link<RECON>(gtrans + (size_t)parity * RECON * padded_vh<T>(G), h, m);
 }
 
 template <typename T, int RECON, bool TO_INTERNAL>
@@ -563,7 +563,7 @@ template <typename TG, int RECON>
 __device__ __forceinline__ void load_transform_d(const TG* gtrans, const Geom& G, uint32_t parity, uint32_t h, double (&m)[18])
 {
     TG u[18];
-    load_link<RECON>(gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, u);
+    load_link<RECON>(gtrans + (size_t)parity * RECON * padded_vh<TG>(G), h, u);
     if (RECON == 12) reconstruct_row2(u);
 #pragma unroll
     for (int k = 0; k < 18; ++k) m[k] = (double)u[k];
@@ -589,7 +589,7 @@ __global__ void apply_transform_kernel(const TG* __restrict__ gtrans, const TS* 
         TD o[18];
 #pragma unroll
         for (int k = 0; k < 18; ++k) o[k] = (TD)out[k];
-        store_link<RECON>(dst + block_offset<TD>(parity, mu, RECON, G.Vh), G.Vh, h, o);
+        store_link<RECON>(dst + block_offset<TD>(parity, mu, RECON, G), h, o);
     }
 }
 

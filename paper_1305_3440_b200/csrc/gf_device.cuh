@@ -40,6 +40,7 @@ __device__ __forceinline__ uint32_t fdiv(uint32_t n, const FastDiv& f)
 struct Geom {
     uint32_t nxh, ny, nz, nt;   // Nx/2, Ny, Nz, Nt
     uint32_t Vh;                // sites per parity
+    uint32_t Vp[2];             // Vh rounded up to whole layout tiles: [0] fp32 (64 sites), [1] fp64 (32 sites)
     uint32_t stride[4];         // distance in h of one step in mu (mu=1: unused)
     uint32_t extent[4];         // N_mu
     FastDiv div_nxh, div_ny, div_nz;
@@ -92,73 +93,100 @@ __device__ __forceinline__ uint32_t forward_index(const Geom& G, const Site& s, 
 }
 
 // --------------------------------------------------------------------------------- link layout
-// field[parity][mu] is a block of RECON*Vh reals; inside a block the link of half-index h is
-// split into 16-byte chunks, chunk c of all sites contiguous:  block[c][h].
-//   fp64: chunk = double2 = one complex entry (9 or 6 chunks).
-//   fp32: chunk = float4 = two complex entries (RECON18: 4 chunks + one float2 tail array;
-//         RECON12: 3 chunks).
-// A warp reading chunk c of 32 consecutive sites moves 512 contiguous bytes with one 128-bit
-// load per lane; a neighbour shifted by one site stays 16-byte aligned.
-// Registers hold a link as m[18] = row-major (re, im) pairs.
+// field[parity][mu] is a block of RECON * Vp reals (Vp = Vh rounded up to whole tiles).  Inside a block the sites
+// are grouped in TILES of TW consecutive half-indices (TW = 32 for fp64, 64 for fp32); a tile stores its links
+// as 16-byte chunks, chunk c of the TW sites contiguous:  block[tile][c][i],  i = h mod TW.
+//   fp64: chunk = double2 = one complex entry (9 or 6 chunks of 512 bytes per tile).
+//   fp32: chunk = float4 = two complex entries (RECON18: 4 chunks of 1024 bytes + the float2 tails of the tile,
+//         512 bytes; RECON12: 3 chunks).
+// A warp reading chunk c of 32 consecutive sites moves 512 contiguous bytes with one 128-bit load per lane, and a
+// neighbour shifted by one site stays 16-byte aligned, as with chunk planes over the whole lattice; but all the
+// chunks of a link for one tile now form ONE contiguous run of 32 * RECON * 8 = 4608 / 3072 bytes (the same in fp32
+// with its 64-site tiles), which is what the TMA bulk copies of the streamed kernel (gf_wave.cu) move per
+// request -- a bulk copy costs ~35 ns of TMA time whatever its size (profiles/r2_tma_request_size.txt) -- and the
+// chunks of one link share DRAM pages.  Registers hold a link as m[18] = row-major (re, im) pairs.
 
 template <typename T> struct Vec16;
 template <> struct Vec16<double> { using type = double2; };
 template <> struct Vec16<float> { using type = float4; };
 
+template <typename T> struct Tile {
+    static constexpr uint32_t W = 256u / (uint32_t)sizeof(T);      // sites per tile: 32 (fp64), 64 (fp32)
+    static constexpr uint32_t SHIFT = sizeof(T) == 8 ? 5u : 6u;
+};
+
 template <typename T>
-__host__ __device__ __forceinline__ size_t block_offset(uint32_t parity, int mu, int recon, uint32_t Vh)
+__host__ __device__ __forceinline__ uint32_t padded_vh(const Geom& G)
 {
-    return (size_t)(parity * 4u + (uint32_t)mu) * (size_t)recon * (size_t)Vh;   // in reals
+    return G.Vp[sizeof(T) == 8 ? 1 : 0];
 }
 
-template <int RECON>
-__device__ __forceinline__ void load_link(const double* __restrict__ blk, uint32_t Vh, uint32_t h, double (&m)[18])
+// offset in reals of the block field[parity][mu]
+template <typename T>
+__host__ __device__ __forceinline__ size_t block_offset(uint32_t parity, int mu, int recon, const Geom& G)
 {
-    const double2* p = reinterpret_cast<const double2*>(blk) + h;
+    return (size_t)(parity * 4u + (uint32_t)mu) * (size_t)recon * (size_t)padded_vh<T>(G);
+}
+
+// 16-byte units per (link, tile): RECON * TW * sizeof(T) / 16
+template <typename T, int RECON> struct TileUnits {
+    static constexpr uint32_t value = (uint32_t)RECON * Tile<T>::W * (uint32_t)sizeof(T) / 16u;
+};
+
+template <int RECON>
+__device__ __forceinline__ void load_link(const double* __restrict__ blk, uint32_t h, double (&m)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + (size_t)(h >> 5) * TileUnits<double, RECON>::value + (h & 31u);
 #pragma unroll
     for (int c = 0; c < RECON / 2; ++c) {
-        const double2 v = p[(size_t)c * Vh];
+        const double2 v = p[c * 32];
         m[2 * c] = v.x;
         m[2 * c + 1] = v.y;
     }
 }
 
 template <int RECON>
-__device__ __forceinline__ void load_link(const float* __restrict__ blk, uint32_t Vh, uint32_t h, float (&m)[18])
+__device__ __forceinline__ void load_link(const float* __restrict__ blk, uint32_t h, float (&m)[18])
 {
-    const float4* p = reinterpret_cast<const float4*>(blk) + h;
+    const float4* p = reinterpret_cast<const float4*>(blk) + (size_t)(h >> 6) * TileUnits<float, RECON>::value + (h & 63u);
 #pragma unroll
     for (int c = 0; c < RECON / 4; ++c) {
-        const float4 v = p[(size_t)c * Vh];
+        const float4 v = p[c * 64];
         m[4 * c] = v.x;
         m[4 * c + 1] = v.y;
         m[4 * c + 2] = v.z;
         m[4 * c + 3] = v.w;
     }
     if (RECON == 18) {
-        const float2* t = reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + h;
-        const float2 v = *t;
+        const float2 v = *(reinterpret_cast<const float2*>(p - (h & 63u) + 256) + (h & 63u));
         m[16] = v.x;
         m[17] = v.y;
     }
 }
 
 template <int RECON>
-__device__ __forceinline__ void store_link(double* __restrict__ blk, uint32_t Vh, uint32_t h, const double (&m)[18])
+__device__ __forceinline__ void store_link(double* __restrict__ blk, uint32_t h, const double (&m)[18])
 {
-    double2* p = reinterpret_cast<double2*>(blk) + h;
+    double2* p = reinterpret_cast<double2*>(blk) + (size_t)(h >> 5) * TileUnits<double, RECON>::value + (h & 31u);
 #pragma unroll
-    for (int c = 0; c < RECON / 2; ++c) p[(size_t)c * Vh] = make_double2(m[2 * c], m[2 * c + 1]);
+    for (int c = 0; c < RECON / 2; ++c) p[c * 32] = make_double2(m[2 * c], m[2 * c + 1]);
 }
 
 template <int RECON>
-__device__ __forceinline__ void store_link(float* __restrict__ blk, uint32_t Vh, uint32_t h, const float (&m)[18])
+__device__ __forceinline__ void store_link(float* __restrict__ blk, uint32_t h, const float (&m)[18])
 {
-    float4* p = reinterpret_cast<float4*>(blk) + h;
+    float4* p = reinterpret_cast<float4*>(blk) + (size_t)(h >> 6) * TileUnits<float, RECON>::value + (h & 63u);
 #pragma unroll
-    for (int c = 0; c < RECON / 4; ++c)
-        p[(size_t)c * Vh] = make_float4(m[4 * c], m[4 * c + 1], m[4 * c + 2], m[4 * c + 3]);
-    if (RECON == 18) reinterpret_cast<float2*>(blk + (size_t)16 * Vh)[h] = make_float2(m[16], m[17]);
+    for (int c = 0; c < RECON / 4; ++c) p[c * 64] = make_float4(m[4 * c], m[4 * c + 1], m[4 * c + 2], m[4 * c + 3]);
+    if (RECON == 18) *(reinterpret_cast<float2*>(p - (h & 63u) + 256) + (h & 63u)) = make_float2(m[16], m[17]);
+}
+
+// address of the first 16-byte chunk of the link of site h (the others follow at Tile<T>::W * 16 bytes)
+template <typename T, int RECON>
+__device__ __forceinline__ const char* link_address(const T* blk, uint32_t h)
+{
+    return reinterpret_cast<const char*>(blk) +
+           ((size_t)(h >> Tile<T>::SHIFT) * TileUnits<T, RECON>::value + (h & (Tile<T>::W - 1u))) * 16u;
 }
 
 // ------------------------------------------------------------------------- 3x3 complex algebra

@@ -29,6 +29,7 @@ struct SweepArgs {
 
 // the streamed sweep (gf_wave.cu): TMA bulk copies into a shared-memory ring, one thread per site
 struct WaveArgs {
+    int precision;                  // PREC_F32 | PREC_F64: storage type (tile width 64 | 32 sites)
     void* links;
     Geom G;
     uint32_t site_offset;
@@ -65,11 +66,12 @@ struct ReduceTail {
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);
 bool sweep_config_valid(int lanes, int block);
 
-bool wave_supported(const Geom& G);                       // the lattice can be tiled (32 sites = whole x-rows inside one plane)
+bool wave_supported(const Geom& G, int precision);        // a layout tile is whole x-rows inside one (z,t) plane
 uint32_t wave_stages(int precision, int recon);           // depth of the shared-memory ring of that variant
 unsigned long long wave_total_tiles(const WaveArgs& a);
 uint32_t wave_ticket_advance(const WaveArgs& a);          // by how much one launch moves the ticket counter
-uint32_t wave_tiles_per_plane(const Geom& G);             // parity-0 tiles of one plane: what one launch adds to every done[plane]
+uint32_t wave_tiles_per_plane(const Geom& G, int precision);   // layout tiles of one parity in a plane
+uint32_t wave_counts_per_plane(const Geom& G, int precision);  // what a fused launch adds to every done[plane]
 cudaError_t launch_wave(int precision, int solver_f64, int recon, const WaveArgs& a, cudaStream_t st);
 
 // prev_links / next_links: the fields of the slabs below / above in t (NULL = this field, periodic)

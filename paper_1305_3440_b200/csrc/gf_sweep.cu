@@ -90,11 +90,10 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
 
     if (MODE == MODE_ACC && j == 0) {
         // G(x) is only needed after the links have been written back: start moving it towards L2 now
-        const T* gp = P.gtrans + (size_t)parity * RECON * G.Vh;
+        const char* gp = link_address<T, RECON>(P.gtrans + (size_t)parity * RECON * padded_vh<T>(G), h);
         constexpr int CH = (RECON * (int)sizeof(T)) / 16;      // whole 16-byte chunks (the fp32/18 tail rides along)
 #pragma unroll
-        for (int c = 0; c < CH; ++c)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(gp) + ((size_t)c * G.Vh + h) * 16));
+        for (int c = 0; c < CH; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(gp + (size_t)c * Tile<T>::W * 16));
     }
 
     // a2: gather this lane's links
@@ -107,15 +106,15 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
         if (MODE == MODE_DEFER && d == 0 && j == 0) {
             // mu = 0: the temporal links stay where they are; their register slot carries G(x) instead,
             // loaded up front with the links (mu = 0 does not enter K in Coulomb gauge: mu0 = 1)
-            load_link<RECON>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, Uf[d]);
+            load_link<RECON>(P.gtrans + (size_t)parity * RECON * padded_vh<T>(G), h, Uf[d]);
 #pragma unroll
             for (int k = 0; k < 18; ++k) Ub[d][k] = T(0);
             continue;
         }
-        load_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, Uf[d]);
+        load_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G), h, Uf[d]);
         // the temporal link below the first local time slice belongs to the slab below
         const T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], Ub[d]);
+        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[d], Ub[d]);
     }
     // 12-real storage.  LAZY12: the third rows are never kept: they are formed for K(x) and dropped, and formed
     // again for the forward links in step a6 (U g^dagger does not need the third row of U at all) -- 24 flops per
@@ -194,7 +193,7 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
             T out[18];
             if (LAZY12) reconstruct_row2(Uf[d]);
             mul_g_U<ROWS>(g, Uf[d], out);
-            store_link<RECON>(P.gtrans + (size_t)parity * RECON * G.Vh, G.Vh, h, out);
+            store_link<RECON>(P.gtrans + (size_t)parity * RECON * padded_vh<T>(G), h, out);
             continue;
         }
         T out[18];
@@ -204,18 +203,18 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
             reconstruct_row2(Uf[d]);
         }
         mul_g_U<ROWS>(g, Uf[d], out);
-        store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, out);
+        store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G), h, out);
         mul_U_gdag<ROWS>(Ub[d], g, out);
         T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        store_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[d], out);
+        store_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[d], out);
     }
     if (MODE == MODE_ACC && j == 0) {
-        T* blk = P.gtrans + (size_t)parity * RECON * G.Vh;
+        T* blk = P.gtrans + (size_t)parity * RECON * padded_vh<T>(G);
         T Gt[18], out[18];
-        load_link<RECON>(blk, G.Vh, h, Gt);
+        load_link<RECON>(blk, h, Gt);
         if (RECON == 12) reconstruct_row2(Gt);
         mul_g_U<ROWS>(g, Gt, out);
-        store_link<RECON>(blk, G.Vh, h, out);
+        store_link<RECON>(blk, h, out);
     }
     }
 }

@@ -1,17 +1,18 @@
 // gf_wave.cu -- the streamed sweep: the same site update as gf_sweep.cu, organised for the
 // memory system instead of for the register file.
 //
-// * Persistent blocks.  One PRODUCER warp per block moves the links of a tile -- 32 consecutive sites of one parity:
-//   whole x-rows inside one (z,t) plane -- into a ring of shared-memory stages with 1-D TMA bulk copies
-//   (cp.async.bulk.shared.global, completion counted by an mbarrier): in the chunked layout block[c][h] every
-//   (link, 16-byte chunk) of a tile is ONE contiguous run, forward links and all four backward neighbours alike (the
-//   x-neighbour is the same run read with a shifted index, the y-neighbour the run one row down, z and t one plane /
-//   one time slice down, periodic wraps are a second run at most).  No tensor map is needed.
-// * CONSUMER warps, one thread per site: K(x) is accumulated out of shared memory, the three SU(2) solves run ONCE per
-//   site (the register kernel of gf_sweep.cu repeats them in each of the 2-4 lanes that share a site), the links are
-//   read from shared memory a second time for g U and U g^dagger and stored to global memory with 128-bit stores.
-//   Only K, g and one link are live in registers, so a handful of consumer warps saturates the arithmetic while the
-//   ring keeps ~100-200 KB of loads in flight per SM: load latency is decoupled from the arithmetic.
+// * Persistent blocks.  One PRODUCER warp per block moves the links of a tile -- the TW = 32 (fp64) or 64 (fp32)
+//   consecutive sites of one layout tile: whole x-rows inside one (z,t) plane -- into a ring of shared-memory stages
+//   with 1-D TMA bulk copies (cp.async.bulk.shared.global, completion counted by an mbarrier).  In the tiled layout
+//   (gf_device.cuh) all chunks of one link for one tile are ONE contiguous run of 4608 / 3072 bytes, so a stage is
+//   nine requests: the four forward links, and for the backward neighbours the tile itself (x: same run read with a
+//   shifted index; y: rows 1.. of the tile), the tile holding the row below (y), the tile one plane down (z) and one
+//   time slice down (t), periodic wraps included.  No tensor map is needed.  (Per-chunk runs of 512 bytes were
+//   measured first: a bulk copy costs ~35 ns of TMA time whatever its size, profiles/r2_tma_request_size.txt.)
+// * CONSUMER warps (two per stage) run the site update of the register kernel -- one lane per site in fp32, two in
+//   fp64 -- but take their links from shared memory instead of global memory and hand the stage back as soon as the
+//   links are in registers: the ring only covers the latency of the loads, ~200 KB in flight per SM whatever the
+//   arithmetic does, and a consumer never waits for DRAM.  Results go to global memory with 128-bit stores.
 // * Fused iteration (mode 2): ONE launch does both half-sweeps of an iteration in a wavefront over the
 //   (t,z) planes -- the parity-1 tiles of plane q are handed out `lag` planes behind the parity-0 tiles -- so that the
 //   second touch of every link finds it in the 126 MB L2 and the field crosses the DRAM interface once per iteration
@@ -22,12 +23,12 @@
 //   waits for a later ticket: no deadlock, whatever the hardware's dispatch order and however many streams share the GPU.
 // * Modes 0 / 1: one half-sweep (no dependencies) through the same pipeline.
 //
-// The links produced are bitwise those of two gf_sweep launches with one lane per site (same arithmetic, same order).
+// The links produced are bitwise those of two gf_sweep launches with one (fp32) / two (fp64) lanes per site.
 #include "gf_internal.h"
 
 namespace gf {
 
-constexpr uint32_t WAVE_TS = 32;        // sites per tile = one consumer warp
+constexpr uint32_t WAVE_SLOTS = 9;      // link tiles per stage
 constexpr uint32_t WAVE_BATCH = 4;      // tiles claimed per ticket
 constexpr uint32_t WAVE_HEADER = 1024;  // bytes of shared memory in front of the stages (barriers, tile descriptors)
 
@@ -48,6 +49,7 @@ template <typename T, typename TK> struct WaveConsts {
     uint32_t key0, key1, counter;
     uint32_t mode;                  // 0 / 1: half-sweep of that parity; 2: fused iteration
     uint32_t M;                     // tiles per plane and parity
+    uint32_t tiles_per_block;       // layout tiles in one field[parity][mu] block
     uint32_t planes;                // Nt * Nz
     uint32_t plane_sites;           // sites of one parity in a plane: (Nx/2) * Ny
     uint32_t lag;                   // fused iteration: parity-1 tiles of plane q follow the parity-0 tiles of plane q + lag
@@ -154,48 +156,20 @@ __device__ __forceinline__ WaveTile wave_schedule(const WaveConsts<T, TK>& P, un
 }
 
 // ------------------------------------------------------------------------ shared-memory stage
-// stage[slot 0..7][chunk][site]: slot mu = U_mu(x), slot 4 + mu = U_mu(x - mu); 16-byte chunks as in global memory
-// (fp32 / 18-real: four float4 chunks per link, then the float2 tails of all slots).  Thread i reads chunk c of its
-// site at ((slot * CH + c) * 32 + i) * 16: a warp reads 512 contiguous bytes, conflict free.
-template <typename T, int RECON> struct StageLayout;
-template <int RECON> struct StageLayout<double, RECON> {
-    static constexpr int CH16 = RECON / 2, TAIL = 0;
-};
-template <int RECON> struct StageLayout<float, RECON> {
-    static constexpr int CH16 = RECON / 4, TAIL = RECON == 18 ? 1 : 0;
+// A stage holds WAVE_SLOTS link tiles exactly as they lie in global memory ([chunk][site] inside the tile), so the
+// consumers read them with the same load_link as the register kernel (thread i reads chunk c at (c * TW + i) * 16:
+// a warp reads 512 contiguous bytes, conflict free).  Slots: mu = U_mu(x); 4 + mu = U_mu(x - mu) with 4 = the tile one
+// time slice down, 5 = this tile (x-neighbours), 6 = this tile (y-neighbours of rows 1..), 7 = one plane down,
+// 8 = the tile holding the row below this tile's first row.
+template <typename T, int RECON> struct StageLayout {
+    static constexpr uint32_t LINK_BYTES = TileUnits<T, RECON>::value * 16u;          // one link tile: 4608 or 3072 bytes
+    static constexpr uint32_t STAGE_BYTES = WAVE_SLOTS * LINK_BYTES;
 };
 
-template <int RECON>
-__device__ __forceinline__ void lds_link(const unsigned char* stage, int slot, uint32_t idx, double (&m)[18])
+template <typename T, int RECON>
+__device__ __forceinline__ const T* stage_slot(const unsigned char* stage, uint32_t slot)
 {
-    constexpr int CH = StageLayout<double, RECON>::CH16;
-    const double2* p = reinterpret_cast<const double2*>(stage) + (size_t)slot * CH * WAVE_TS + idx;
-#pragma unroll
-    for (int c = 0; c < CH; ++c) {
-        const double2 v = p[c * WAVE_TS];
-        m[2 * c] = v.x;
-        m[2 * c + 1] = v.y;
-    }
-}
-
-template <int RECON>
-__device__ __forceinline__ void lds_link(const unsigned char* stage, int slot, uint32_t idx, float (&m)[18])
-{
-    constexpr int CH = StageLayout<float, RECON>::CH16;
-    const float4* p = reinterpret_cast<const float4*>(stage) + (size_t)slot * CH * WAVE_TS + idx;
-#pragma unroll
-    for (int c = 0; c < CH; ++c) {
-        const float4 v = p[c * WAVE_TS];
-        m[4 * c] = v.x;
-        m[4 * c + 1] = v.y;
-        m[4 * c + 2] = v.z;
-        m[4 * c + 3] = v.w;
-    }
-    if (RECON == 18) {
-        const float2 v = reinterpret_cast<const float2*>(stage + (size_t)8 * CH * WAVE_TS * 16)[slot * WAVE_TS + idx];
-        m[16] = v.x;
-        m[17] = v.y;
-    }
+    return reinterpret_cast<const T*>(stage + (size_t)slot * StageLayout<T, RECON>::LINK_BYTES);
 }
 
 // ------------------------------------------------------------------------------ the producer
@@ -204,12 +178,12 @@ __device__ __forceinline__ void wave_producer(const WaveConsts<T, TK>& P, uint64
                                               unsigned char* stages, uint32_t lane)
 {
     using L = StageLayout<T, RECON>;
-    constexpr uint32_t CHT = L::CH16 + L::TAIL;                                    // runs per link
-    constexpr uint32_t STAGE_BYTES = WAVE_TS * 8u * RECON * (uint32_t)sizeof(T);
+    constexpr uint32_t TW = Tile<T>::W;
     const Geom& G = P.G;
-    const uint32_t Sh = G.stride[0];                                               // sites of one parity in a time slice
     const unsigned char* base = reinterpret_cast<const unsigned char*>(P.links);
+    const uint32_t tiles_slice = P.M * G.nz;                                        // tiles of one parity in a time slice
     uint32_t it = 0;
+    uint32_t verified = 0xffffffffu;                                               // plane whose dependencies this block has seen complete
     bool drain = false;                                                            // an error was seen: no more waiting, no more work
     for (;;) {
         unsigned long long b = 0;
@@ -222,9 +196,9 @@ __device__ __forceinline__ void wave_producer(const WaveConsts<T, TK>& P, uint64
             mbar_wait(empty + slot, ph ^ 1u);                                      // the consumers have released the slot
             const WaveTile w = wave_schedule(P, n);
             const uint32_t t = fdiv(w.plane, G.div_nz), z = w.plane - t * G.nz;
-            const uint32_t h0 = w.plane * P.plane_sites + w.m * WAVE_TS;
-            const uint32_t y0 = fdiv(w.m * WAVE_TS, G.div_nxh);
-            if (P.mode == 2u && w.parity == 1u && !drain) {
+            const uint32_t tile = w.plane * P.M + w.m;                             // layout tile inside a field block
+            const bool first_rows = w.m == 0u;                                     // the tile starts at y = 0
+            if (P.mode == 2u && w.parity == 1u && !drain && w.plane != verified) {
                 // the five planes whose parity-0 updates this tile's links have received
                 if (lane < 5u) {
                     uint32_t q = w.plane;
@@ -234,7 +208,7 @@ __device__ __forceinline__ void wave_producer(const WaveConsts<T, TK>& P, uint64
                     if (lane == 4u) q = t > 0u ? w.plane - G.nz : w.plane + (G.nt - 1u) * G.nz;
                     for (uint32_t spins = 0; (int32_t)(ld_acquire_gpu(P.done + q) - P.done_target) < 0; ++spins) {
                         __nanosleep(64);
-                        if (spins > (1u << 22) || (spins & 1023u) == 1023u && ld_volatile_u32(P.error) != 0u) {
+                        if (spins > (1u << 22) || ((spins & 1023u) == 1023u && ld_volatile_u32(P.error) != 0u)) {
                             *P.error = 1u;                                         // give up: nothing of this tile is stored
                             __threadfence();
                             break;
@@ -243,57 +217,41 @@ __device__ __forceinline__ void wave_producer(const WaveConsts<T, TK>& P, uint64
                 }
                 __syncwarp();
                 if (ld_volatile_u32(P.error) != 0u) drain = true;
+                verified = w.plane;                                                // the tiles of a plane share their five counters
                 // the other blocks' stores (generic proxy) are acquired; the bulk copies below read through the async proxy
                 asm volatile("fence.proxy.async;" ::: "memory");
             }
+            const bool own_y = G.nxh < TW;                                         // rows 1.. of the tile have their y-neighbours in it
             if (lane == 0) {
                 TileDesc d;
-                d.h0 = h0;
+                d.h0 = tile * TW;
                 d.plane = w.plane;
                 d.flags = 1u | (w.parity << 1) | ((P.mode == 2u && w.parity == 0u) ? 4u : 0u) | (drain ? 8u : 0u);
                 d.pad = 0;
                 desc[slot] = d;
                 if (drain) mbar_arrive(full + slot);
-                else mbar_expect_tx(full + slot, STAGE_BYTES);
+                else mbar_expect_tx(full + slot, (own_y ? 9u : 8u) * L::LINK_BYTES);
             }
             __syncwarp();
-            if (drain) continue;
-            unsigned char* stage = stages + (size_t)slot * STAGE_BYTES;
-            // runs: (link slot 0..7, chunk); a tile that starts at y = 0 takes its y-neighbours in two runs (slot 8)
-            const bool ywrap = y0 == 0u && WAVE_TS > G.nxh;
-            const uint32_t nruns = (ywrap ? 9u : 8u) * CHT;
-            for (uint32_t id = lane; id < nruns; id += 32u) {
-                const uint32_t ls = id / CHT, c = id - ls * CHT;
-                uint32_t sl = ls, par = w.parity, hsrc = h0, dst = 0, ns = WAVE_TS;
-                if (ls >= 4u) {
-                    par ^= 1u;
-                    const uint32_t mu = ls & 3u;
-                    if (ls == 8u) {                                  // rows 0 .. R-2 of the tile, shifted up by one row
-                        sl = 6u;
-                        dst = G.nxh;
-                        ns = WAVE_TS - G.nxh;
-                    } else if (mu == 2u) {
-                        if (y0 > 0u) hsrc = h0 - G.nxh;
-                        else {
-                            hsrc = h0 + G.nxh * (G.ny - 1u);                      // row Ny-1 of the same plane
-                            ns = G.nxh < WAVE_TS ? G.nxh : WAVE_TS;
-                        }
-                    } else if (mu == 3u) {
-                        hsrc = z > 0u ? h0 - P.plane_sites : h0 + P.plane_sites * (G.nz - 1u);
-                    } else if (mu == 0u) {
-                        hsrc = t > 0u ? h0 - Sh : h0 + Sh * (G.nt - 1u);
-                    }
-                }
-                const uint32_t mu = sl & 3u;
-                const unsigned char* blk = base + block_offset<T>(par, (int)mu, RECON, G.Vh) * sizeof(T);
-                if (c < (uint32_t)L::CH16) {
-                    bulk_g2s(stage + ((size_t)(sl * L::CH16 + c) * WAVE_TS + dst) * 16u, blk + ((size_t)c * G.Vh + hsrc) * 16u, ns * 16u,
-                             full + slot);
-                } else {
-                    bulk_g2s(stage + (size_t)8 * L::CH16 * WAVE_TS * 16u + ((size_t)sl * WAVE_TS + dst) * 8u,
-                             blk + (size_t)16 * G.Vh * sizeof(T) + (size_t)hsrc * 8u, ns * 8u, full + slot);
+            if (drain || lane >= WAVE_SLOTS || (lane == 6u && !own_y)) continue;
+            // lane = slot: one request per link tile
+            uint32_t par = w.parity, mu = lane & 3u, src = tile;
+            if (lane >= 4u) {
+                par ^= 1u;
+                if (lane == 4u) src = t > 0u ? tile - tiles_slice : tile + tiles_slice * (G.nt - 1u);
+                else if (lane == 7u) src = z > 0u ? tile - P.M : tile + P.M * (G.nz - 1u);
+                else if (lane == 8u) {
+                    mu = 2u;
+                    src = first_rows ? tile + P.M - 1u : tile - 1u;               // the tile whose last row lies below ours
                 }
             }
+#ifdef GF_WAVE_DEBUG_NOTMA
+            // bottleneck probe: the consumers alone (they compute on whatever the stage holds)
+            asm volatile("mbarrier.complete_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(full + slot)), "r"(L::LINK_BYTES) : "memory");
+#else
+            bulk_g2s(stages + (size_t)slot * L::STAGE_BYTES + (size_t)lane * L::LINK_BYTES,
+                     base + block_offset<T>(par, (int)mu, RECON, G) * sizeof(T) + (size_t)src * L::LINK_BYTES, L::LINK_BYTES, full + slot);
+#endif
         }
     }
     // one empty descriptor per consumer warp: consumer w takes the ring entries it = w (mod C)
@@ -309,24 +267,43 @@ __device__ __forceinline__ void wave_producer(const WaveConsts<T, TK>& P, uint64
 }
 
 // ------------------------------------------------------------------------------ the consumers
+// Lanes per site and warps per tile.  fp64: two lanes per site (each holds two directions, as in the register kernel),
+// 16 sites per warp, two warps per 32-site tile.  fp32: one lane per site, two warps per 64-site tile.
+template <typename T> struct WaveShape {
+    static constexpr int L = sizeof(T) == 8 ? 2 : 1;
+    static constexpr uint32_t SPW = 32u / L;                    // sites per warp
+    static constexpr uint32_t CW = Tile<T>::W / SPW;            // consumer warps per stage
+};
+
 template <typename T, typename TK, int RECON, int S, int C>
 __device__ __forceinline__ void wave_consumer(const WaveConsts<T, TK>& P, uint64_t* full, uint64_t* empty, const TileDesc* desc,
                                               const unsigned char* stages, uint32_t warp, uint32_t lane)
 {
-    constexpr uint32_t STAGE_BYTES = WAVE_TS * 8u * RECON * (uint32_t)sizeof(T);
+    using SL = StageLayout<T, RECON>;
+    constexpr uint32_t TW = Tile<T>::W;
+    constexpr int L = WaveShape<T>::L, ND = 4 / L;
+    constexpr uint32_t SPW = WaveShape<T>::SPW, CW = WaveShape<T>::CW;
     constexpr int ROWS = RECON == 12 ? 2 : 3;
     constexpr uint32_t NONE = 0xffffffffu;
     const Geom& G = P.G;
+    const uint32_t group = warp / CW, sub = warp % CW;
+    const uint32_t i = sub * SPW + lane % SPW;  // site of this lane inside a tile
+    const int j = lane / SPW;                   // which directions it holds: mu = j * ND ..
     uint32_t pending = NONE;                    // plane of a finished parity-0 tile whose completion is not published yet
-    for (uint32_t it = warp;; it += C) {
+    for (uint32_t it = group;; it += C) {
         const uint32_t slot = it % S, ph = (it / S) & 1u;
-        if (!mbar_try_wait(full + slot, ph)) {
+        // A parity wait may run at most one phase ahead of its barrier.  The previous fill of this slot may have been
+        // consumed by ANOTHER group (C does not divide S), and bulk copies complete out of order under load, so this
+        // warp first makes sure that fill was released -- which implies it landed -- before it waits for its own.
+        const bool ready = (it < (uint32_t)S || mbar_try_wait(empty + slot, ph ^ 1u)) && mbar_try_wait(full + slot, ph);
+        if (!ready) {
             // nothing to do yet: publish now (a producer, possibly this block's, may be waiting for exactly this count)
             if (pending != NONE) {
                 __syncwarp();
                 if (lane == 0) red_release_gpu_add(P.done + pending, 1u);
                 pending = NONE;
             }
+            if (it >= (uint32_t)S) mbar_wait(empty + slot, ph ^ 1u);
             mbar_wait(full + slot, ph);
         }
         const TileDesc d = desc[slot];
@@ -337,36 +314,65 @@ __device__ __forceinline__ void wave_consumer(const WaveConsts<T, TK>& P, uint64
             continue;
         }
         const uint32_t parity = (d.flags >> 1) & 1u;
-        const uint32_t h = d.h0 + lane;
-        const unsigned char* stage = stages + (size_t)slot * STAGE_BYTES;
+        const unsigned char* stage = stages + (size_t)slot * SL::STAGE_BYTES;
+        const uint32_t h = d.h0 + i;
         const Site s = decode_site(G, h, parity);
-        uint32_t hb[4];
-#pragma unroll
-        for (int mu = 0; mu < 4; ++mu) hb[mu] = backward_index(G, s, mu);
-        const uint32_t ixb = hb[1] - d.h0;      // the x-neighbour sits in the same row, hence in the same run
 
-        // a3: K(x) = sum_mu [U_mu(x) + U_mu(x-mu)^dagger]  (eq. 8)
+        // a2: this lane's links out of the stage into registers, then the stage goes back to the producer: the ring
+        // only has to cover the latency of the loads, not the arithmetic
+        T Uf[ND][18], Ub[ND][18];
+        uint32_t hb[ND];
+#pragma unroll
+        for (int dd = 0; dd < ND; ++dd) {
+            const int mu = j * ND + dd;
+            hb[dd] = backward_index(G, s, mu);
+            load_link<RECON>(stage_slot<T, RECON>(stage, mu), i, Uf[dd]);
+            // where the backward neighbour sits in the stage: x in the same row of this tile, y one row down
+            uint32_t bslot = 4u + (uint32_t)mu, bi = i;
+            if (mu == 1) bi = hb[dd] - d.h0;
+            if (mu == 2) {
+                bslot = i >= G.nxh ? 6u : 8u;
+                bi = i >= G.nxh ? i - G.nxh : TW - G.nxh + i;
+            }
+            load_link<RECON>(stage_slot<T, RECON>(stage, bslot), bi, Ub[dd]);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + slot);       // release: the loads above are performed before it
+#ifdef GF_WAVE_DEBUG_NOCOMPUTE
+        if (Uf[0][0] != T(12345.678)) continue;          // bottleneck probe: the producer / TMA path alone
+#endif
+
+        // a3: K(x) = sum_mu [U_mu(x) + U_mu(x-mu)^dagger]  (eq. 8); 12-real: the third rows are formed
+        // for K and dropped (as in the register kernel's lazy variant)
         TK K[18];
 #pragma unroll
         for (int k = 0; k < 18; ++k) K[k] = TK(0);
 #pragma unroll
-        for (int mu = 0; mu < 4; ++mu) {
+        for (int dd = 0; dd < ND; ++dd) {
+            const int mu = j * ND + dd;
             if (mu >= P.mu0) {
-                T Uf[18], Ub[18];
-                lds_link<RECON>(stage, mu, lane, Uf);
-                lds_link<RECON>(stage, 4 + mu, mu == 1 ? ixb : lane, Ub);
+                T rf[6], rb[6];
                 if (RECON == 12) {
-                    reconstruct_row2(Uf);
-                    reconstruct_row2(Ub);
+                    row2_of(Uf[dd], rf);
+                    row2_of(Ub[dd], rb);
                 }
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
                     for (int b = 0; b < 3; ++b) {
-                        GF_RE(K, a, b) += (TK)GF_RE(Uf, a, b) + (TK)GF_RE(Ub, b, a);
-                        GF_IM(K, a, b) += (TK)GF_IM(Uf, a, b) - (TK)GF_IM(Ub, b, a);
+                        const T fr = (RECON == 18 || a < 2) ? GF_RE(Uf[dd], a, b) : rf[2 * b];
+                        const T fi = (RECON == 18 || a < 2) ? GF_IM(Uf[dd], a, b) : rf[2 * b + 1];
+                        const T br = (RECON == 18 || b < 2) ? GF_RE(Ub[dd], b, a) : rb[2 * a];
+                        const T bi = (RECON == 18 || b < 2) ? GF_IM(Ub[dd], b, a) : rb[2 * a + 1];
+                        GF_RE(K, a, b) += (TK)fr + (TK)br;
+                        GF_IM(K, a, b) += (TK)fi - (TK)bi;
                     }
             }
+        }
+#pragma unroll
+        for (uint32_t off = SPW; off < 32u; off <<= 1) {
+#pragma unroll
+            for (int k = 0; k < 18; ++k) K[k] += __shfl_xor_sync(0xffffffffu, K[k], off);
         }
 
         // a5: the stochastic-relaxation draws
@@ -379,7 +385,7 @@ __device__ __forceinline__ void wave_consumer(const WaveConsts<T, TK>& P, uint64
             sq2 = (double)(w[2] >> 8) * (1.0 / 16777216.0) < P.p;
         }
 
-        // a4: the three SU(2) subgroups, once per site
+        // a4: the three SU(2) subgroups
         TK gk[18];
         solve_site(K, P.algo, P.omega, sq0, sq1, sq2, gk);
         T g[18];
@@ -395,18 +401,19 @@ __device__ __forceinline__ void wave_consumer(const WaveConsts<T, TK>& P, uint64
 
         // a6: U_mu(x) <- g U_mu(x),  U_mu(x-mu) <- U_mu(x-mu) g^dagger  (eq. 3)
 #pragma unroll
-        for (int mu = 0; mu < 4; ++mu) {
-            T U[18], out[18];
-            lds_link<RECON>(stage, mu, lane, U);
-            if (RECON == 12) reconstruct_row2(U);
-            mul_g_U<ROWS>(g, U, out);
-            store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G.Vh), G.Vh, h, out);
-            lds_link<RECON>(stage, 4 + mu, mu == 1 ? ixb : lane, U);
-            mul_U_gdag<ROWS>(U, g, out);
-            store_link<RECON>(P.links + block_offset<T>(parity ^ 1u, mu, RECON, G.Vh), G.Vh, hb[mu], out);
+        for (int dd = 0; dd < ND; ++dd) {
+            const int mu = j * ND + dd;
+            T out[18];
+            if (RECON == 12) {
+                forget(GF_RE(Uf[dd], 0, 1));
+                forget(GF_RE(Uf[dd], 0, 2));
+                reconstruct_row2(Uf[dd]);
+            }
+            mul_g_U<ROWS>(g, Uf[dd], out);
+            store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G), h, out);
+            mul_U_gdag<ROWS>(Ub[dd], g, out);
+            store_link<RECON>(P.links + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[dd], out);
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(empty + slot);                   // the stage may be refilled
         if (d.flags & 4u) pending = d.plane;
     }
     if (pending != NONE) {
@@ -416,7 +423,7 @@ __device__ __forceinline__ void wave_consumer(const WaveConsts<T, TK>& P, uint64
 }
 
 template <typename T, typename TK, int RECON, int S, int C>
-__global__ void __launch_bounds__(32 * (C + 1), 1) wave_kernel(const WaveConsts<T, TK> P)
+__global__ void __launch_bounds__(32 * (C * (int)WaveShape<T>::CW + 1), 1) wave_kernel(const WaveConsts<T, TK> P)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);
@@ -427,23 +434,25 @@ __global__ void __launch_bounds__(32 * (C + 1), 1) wave_kernel(const WaveConsts<
     if (threadIdx.x == 0) {
         for (int s = 0; s < S; ++s) {
             mbar_init(full + s, 1);
-            mbar_init(empty + s, 1);
+            mbar_init(empty + s, WaveShape<T>::CW);                 // every consumer warp of the stage releases it
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
-    if (warp == (uint32_t)C) wave_producer<T, TK, RECON, S, C>(P, full, empty, desc, stages, lane);
+    constexpr uint32_t CW = WaveShape<T>::CW;
+    if (warp == (uint32_t)C * CW) wave_producer<T, TK, RECON, S, C>(P, full, empty, desc, stages, lane);
     else wave_consumer<T, TK, RECON, S, C>(P, full, empty, desc, stages, warp, lane);
 }
 
 // --------------------------------------------------------------------------------- launching
 // stages x consumer warps per storage variant: the ring fills the shared memory of an SM (227 KB per block)
-#ifndef GF_WAVE_CFG
-#define GF_WAVE_CFG_F64_18 6, 4
-#define GF_WAVE_CFG_F64_12 8, 5
-#define GF_WAVE_CFG_F32_18 10, 6
-#define GF_WAVE_CFG_F32_12 12, 6
+#ifndef GF_WAVE_CFG_F64_18
+// (registers are allocated per four warps: 3 groups x 2 warps + the producer = 7 warps leave 255 registers per thread)
+#define GF_WAVE_CFG_F64_18 5, 3
+#define GF_WAVE_CFG_F64_12 8, 3
+#define GF_WAVE_CFG_F32_18 5, 3
+#define GF_WAVE_CFG_F32_12 8, 3
 #endif
 template <typename T, int RECON> struct WaveCfg;
 template <> struct WaveCfg<double, 18> { static constexpr int cfg[2] = {GF_WAVE_CFG_F64_18}; };
@@ -451,11 +460,11 @@ template <> struct WaveCfg<double, 12> { static constexpr int cfg[2] = {GF_WAVE_
 template <> struct WaveCfg<float, 18> { static constexpr int cfg[2] = {GF_WAVE_CFG_F32_18}; };
 template <> struct WaveCfg<float, 12> { static constexpr int cfg[2] = {GF_WAVE_CFG_F32_12}; };
 
-bool wave_supported(const Geom& G)
+bool wave_supported(const Geom& G, int precision)
 {
-    // a tile = 32 sites = whole x-rows inside one plane; runs of the fp32 tail array must stay 16-byte aligned
-    const uint32_t plane = G.nxh * G.ny;
-    return G.nxh >= 2 && G.nxh % 2u == 0 && WAVE_TS % G.nxh == 0 && plane % WAVE_TS == 0;
+    // a layout tile (32 sites in fp64, 64 in fp32) must be whole x-rows inside one (z,t) plane
+    const uint32_t plane = G.nxh * G.ny, TW = precision == PREC_F64 ? Tile<double>::W : Tile<float>::W;
+    return TW % G.nxh == 0 && plane % TW == 0;
 }
 
 uint32_t wave_stages(int precision, int recon)
@@ -464,7 +473,15 @@ uint32_t wave_stages(int precision, int recon)
     return recon == 12 ? WaveCfg<float, 12>::cfg[0] : WaveCfg<float, 18>::cfg[0];
 }
 
-uint32_t wave_tiles_per_plane(const Geom& G) { return G.nxh * G.ny / WAVE_TS; }
+uint32_t wave_tiles_per_plane(const Geom& G, int precision)
+{
+    return G.nxh * G.ny / (precision == PREC_F64 ? Tile<double>::W : Tile<float>::W);
+}
+
+// what a fused launch adds to every done[plane]: one count per consumer warp (two per tile) of its parity-0 tiles
+uint32_t wave_counts_per_plane(const Geom& G, int precision) { return 2u * wave_tiles_per_plane(G, precision); }
+
+
 
 uint32_t wave_ticket_advance(const WaveArgs& a)
 {
@@ -475,7 +492,7 @@ uint32_t wave_ticket_advance(const WaveArgs& a)
 
 unsigned long long wave_total_tiles(const WaveArgs& a)
 {
-    const unsigned long long per_parity = (unsigned long long)a.G.Vh / WAVE_TS;
+    const unsigned long long per_parity = (unsigned long long)a.G.Vh / (a.precision == PREC_F64 ? Tile<double>::W : Tile<float>::W);
     return a.mode == 2 ? 2ull * per_parity : per_parity;
 }
 
@@ -483,7 +500,7 @@ template <typename T, typename TK, int RECON>
 static cudaError_t launch_wave_t(const WaveArgs& a, cudaStream_t st)
 {
     constexpr int S = WaveCfg<T, RECON>::cfg[0], C = WaveCfg<T, RECON>::cfg[1];
-    constexpr size_t smem = WAVE_HEADER + (size_t)S * WAVE_TS * 8u * RECON * sizeof(T);
+    constexpr size_t smem = WAVE_HEADER + (size_t)S * StageLayout<T, RECON>::STAGE_BYTES;
     static_assert(smem <= 232448, "the ring does not fit the shared memory of an SM");
     WaveConsts<T, TK> P;
     P.links = static_cast<T*>(a.links);
@@ -498,7 +515,8 @@ static cudaError_t launch_wave_t(const WaveArgs& a, cudaStream_t st)
     P.counter = a.counter;
     P.mode = (uint32_t)a.mode;
     P.plane_sites = a.G.nxh * a.G.ny;
-    P.M = P.plane_sites / WAVE_TS;
+    P.M = P.plane_sites / Tile<T>::W;
+    P.tiles_per_block = a.G.Vh / Tile<T>::W;
     P.planes = a.G.nt * a.G.nz;
     P.lag = a.lag;
     P.total_tiles = wave_total_tiles(a);
@@ -511,13 +529,13 @@ static cudaError_t launch_wave_t(const WaveArgs& a, cudaStream_t st)
     auto kernel = wave_kernel<T, TK, RECON, S, C>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kernel<<<a.num_ctas, 32 * (C + 1), smem, st>>>(P);
+    kernel<<<a.num_ctas, 32 * (C * (int)WaveShape<T>::CW + 1), smem, st>>>(P);
     return cudaGetLastError();
 }
 
 cudaError_t launch_wave(int precision, int solver_f64, int recon, const WaveArgs& a, cudaStream_t st)
 {
-    if (!wave_supported(a.G) || a.num_ctas < 1) return cudaErrorInvalidValue;
+    if (!wave_supported(a.G, precision) || a.num_ctas < 1) return cudaErrorInvalidValue;
     if (precision == PREC_F64)
         return recon == 12 ? launch_wave_t<double, double, 12>(a, st) : launch_wave_t<double, double, 18>(a, st);
     if (solver_f64) return recon == 12 ? launch_wave_t<float, double, 12>(a, st) : launch_wave_t<float, double, 18>(a, st);

@@ -18,16 +18,17 @@ def _field(dims, prec, recon, dev, gauge=gf.GF_LANDAU, seed=0):
     return gf.GaugeField(dims, gauge=gauge, recon=recon, precisions=(prec,), seed=seed, device=dev)
 
 
-def streamed_ok(dims):
-    """include/gf.h: Nx/2 even and dividing 32, (Nx/2) * Ny a multiple of 32."""
-    nxh = dims[1] // 2
-    return nxh % 2 == 0 and 32 % nxh == 0 and (nxh * dims[2]) % 32 == 0
+def streamed_ok(dims, prec):
+    """include/gf.h: a layout tile (32 sites in fp64, 64 in fp32) is whole x-rows inside one plane."""
+    nxh, W = dims[1] // 2, 32 if prec == "f64" else 64
+    return W % nxh == 0 and (nxh * dims[2]) % W == 0
 
 
-# (8,8,8,8): 4 rows per tile, one tile per plane; (4,16,16,16): 4 tiles per plane; (6,4,16,4): rows of 2 sites;
-# (4,64,2,4): a whole row per tile (no second run for the y-neighbours); (4,4,4,4), (6,4,8,4), (8,12,8,8): not tileable
+# (8,8,8,8): fp64 one tile per plane (fp32: not tileable); (4,16,16,16): several tiles per plane; (6,4,16,4): rows of 2
+# sites; (4,64,2,4) / (4,128,2,4): a whole row per tile (the y-neighbours come from one other tile); (8,6,16,16): rows of
+# 3 sites, odd; (4,4,4,4), (6,4,8,4), (8,12,8,8): not tileable
 SHAPES = [(4, 4, 4, 4), (8, 8, 8, 8), (6, 4, 8, 4), (6, 4, 16, 4), (16, 8, 8, 8), (4, 16, 16, 16), (4, 64, 2, 4), (8, 12, 8, 8),
-          (4, 32, 4, 2), (2, 8, 8, 8)]
+          (4, 32, 4, 2), (2, 8, 8, 8), (4, 128, 2, 4), (6, 4, 32, 2), (4, 8, 16, 6)]
 
 
 @pytest.mark.parametrize("dims", SHAPES)
@@ -35,19 +36,19 @@ SHAPES = [(4, 4, 4, 4), (8, 8, 8, 8), (6, 4, 8, 4), (6, 4, 16, 4), (16, 8, 8, 8)
 @pytest.mark.parametrize("recon", [18, 12])
 @pytest.mark.parametrize("algo,omega,p", [(gf.GF_STOCHASTIC, 1.0, 0.6), (gf.GF_OVERRELAX, 1.7, 0.0)])
 def test_fused_iterations_are_the_half_sweeps(cuda_device, dims, prec, recon, algo, omega, p):
-    """gf_iterate with the fused launch against 2n gf_sweep launches of the register kernel with one lane per site:
-    same arithmetic in the same order, so the links are compared bit for bit."""
+    """gf_iterate with the fused launch against 2n gf_sweep launches of the register kernel with the same lanes per
+    site (one in fp32, two in fp64): same arithmetic in the same order, so the links are compared bit for bit."""
     U = torch.from_numpy(gi.smooth_random_gauge(dims, 0.5, 23)).to(cuda_device).to(CDTYPE[prec]).contiguous()
     a = _field(dims, prec, recon, cuda_device, seed=5)
     b = _field(dims, prec, recon, cuda_device, seed=5)
     for f in (a, b):
         f.pack(U, PREC[prec])
-        f.set_tuning(PREC[prec], 1, 64)
+        f.set_tuning(PREC[prec], 1 if prec == "f32" else 2, 64)
     a.set_wavefront(2)
     l0 = gf.gf_launch_count(a.ctx)
     a.iterate(7, algo, omega, p, PREC[prec])
     fused = gf.gf_launch_count(a.ctx) - l0 == 7
-    assert fused == (streamed_ok(dims) and dims[0] >= 4)              # otherwise it fell back to 14 half-sweeps
+    assert fused == (streamed_ok(dims, prec) and dims[0] >= 4)              # otherwise it fell back to 14 half-sweeps
     for it in range(7):
         b.sweep(0, algo, omega, p, PREC[prec])
         b.sweep(1, algo, omega, p, PREC[prec])
@@ -60,7 +61,7 @@ def test_fused_iterations_are_the_half_sweeps(cuda_device, dims, prec, recon, al
     b.close()
 
 
-@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (4, 16, 16, 16), (2, 8, 8, 8), (4, 64, 2, 4)])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (4, 16, 16, 16), (2, 8, 16, 8), (4, 64, 2, 4), (4, 128, 2, 2)])
 @pytest.mark.parametrize("prec,recon", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
 def test_streamed_half_sweeps_are_the_register_kernel(cuda_device, dims, prec, recon):
     """Mode 3: gf_sweep itself through the streamed kernel (one parity per launch, no dependencies)."""
@@ -69,7 +70,7 @@ def test_streamed_half_sweeps_are_the_register_kernel(cuda_device, dims, prec, r
     b = _field(dims, prec, recon, cuda_device, seed=9)
     for f in (a, b):
         f.pack(U, PREC[prec])
-        f.set_tuning(PREC[prec], 1, 64)
+        f.set_tuning(PREC[prec], 1 if prec == "f32" else 2, 64)
     a.set_wavefront(3)
     for k in range(3):
         for parity in (1, 0, 0):                                  # any order of parities, as gf_sweep allows
@@ -91,7 +92,7 @@ def test_fused_iteration_for_any_lag_and_block_count(cuda_device, lag, blocks):
     b = _field(dims, "f64", 18, cuda_device, seed=4)
     for f in (a, b):
         f.pack(U, gf.GF_F64)
-        f.set_tuning(gf.GF_F64, 1, 64)
+        f.set_tuning(gf.GF_F64, 2, 64)
     a.set_wavefront(2)
     a.set_wave_tuning(lag, blocks)
     a.iterate(4, gf.GF_STOCHASTIC, 1.0, 0.5, gf.GF_F64)
@@ -134,7 +135,7 @@ def test_fused_iteration_eligibility_and_modes(cuda_device):
     b = _field(dims, "f64", 18, cuda_device, gauge=gf.GF_COULOMB)
     for f in (a, b):
         f.pack(U, gf.GF_F64)
-        f.set_tuning(gf.GF_F64, 1, 64)
+        f.set_tuning(gf.GF_F64, 2, 64)
     a.set_wavefront(2)
     b.set_wavefront(0)
     l0, l1 = gf.gf_launch_count(a.ctx), gf.gf_launch_count(b.ctx)
