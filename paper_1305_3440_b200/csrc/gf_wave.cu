@@ -447,13 +447,19 @@ __global__ void __launch_bounds__(32 * (C * (int)WaveShape<T>::CW + 1), 1) wave_
 
 // --------------------------------------------------------------------------------- launching
 // stages x consumer warps per storage variant: the ring fills the shared memory of an SM (227 KB per block)
-#ifndef GF_WAVE_CFG_F64_18
-// (registers are allocated per four warps: 3 groups x 2 warps + the producer = 7 warps leave 255 registers per thread)
-#define GF_WAVE_CFG_F64_18 5, 3
-#define GF_WAVE_CFG_F64_12 8, 3
-#define GF_WAVE_CFG_F32_18 5, 3
-#define GF_WAVE_CFG_F32_12 8, 3
+#ifndef GF_WAVE_S18
+#define GF_WAVE_S18 5
 #endif
+#ifndef GF_WAVE_S12
+#define GF_WAVE_S12 8
+#endif
+#ifndef GF_WAVE_C
+#define GF_WAVE_C 3      // registers are allocated per four warps: 3 groups x 2 warps + the producer = 7 warps leave 255 registers per thread
+#endif
+#define GF_WAVE_CFG_F64_18 GF_WAVE_S18, GF_WAVE_C
+#define GF_WAVE_CFG_F64_12 GF_WAVE_S12, GF_WAVE_C
+#define GF_WAVE_CFG_F32_18 GF_WAVE_S18, GF_WAVE_C
+#define GF_WAVE_CFG_F32_12 GF_WAVE_S12, GF_WAVE_C
 template <typename T, int RECON> struct WaveCfg;
 template <> struct WaveCfg<double, 18> { static constexpr int cfg[2] = {GF_WAVE_CFG_F64_18}; };
 template <> struct WaveCfg<double, 12> { static constexpr int cfg[2] = {GF_WAVE_CFG_F64_12}; };
