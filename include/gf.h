@@ -100,30 +100,11 @@ int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is_f64, int p
  * GF_ESTATE (no storage for that precision), GF_ECUDA. */
 int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision);
 
-/* n iterations = n x {parity 0, parity 1}, asynchronous; the Philox counter advances by 2 per
- * iteration exactly as 2n gf_sweep calls would.
- *
- * The streamed kernel and the fused iteration.  Besides the register kernel behind gf_sweep
- * the library has a second organisation of the same site update: persistent blocks whose producer warp streams
- * tiles of 32 sites into a shared-memory ring with TMA bulk copies while consumer warps (one thread per site) compute
- * out of shared memory.  With it ONE launch can do both half-sweeps of an iteration in a wavefront over the (t,z)
- * planes: the parity-1 tiles follow the parity-0 tiles `lag` planes behind and every parity-1 tile waits, in the
- * kernel, for the completion counters of the five planes its links were updated from.  The second touch of every
- * link then hits the L2 cache: the field crosses the DRAM interface once per iteration instead of twice.
- * Eligible: a whole lattice (no slabs), no transformation buffer attached for `precision`, no slice mask, N_t >= 4,
- * and a layout tile (W = 32 sites in fp64, 64 in fp32) made of whole x-rows inside one plane: Nx/2 divides W and W
- * divides (Nx/2) * Ny; otherwise an iteration is two gf_sweep launches.
- * gf_set_wavefront: 0 = never (default until section 13's measurements say otherwise), 1 = fuse when a time slice of
- * links is at most 24 MB (so that the ~3 slices between the two fronts stay in the 126 MB L2), 2 = fuse whenever
- * eligible, 3 = as 2 and gf_sweep itself also goes through the streamed kernel when eligible.
- * gf_set_wave_tuning: lag in planes (0 = automatic: N_z + planes in flight + 2) and number of persistent blocks
- * (0 = one per SM).  The links are those of the register kernel with one lane per site (gf_set_tuning lanes = 1).
- * Errors: as gf_sweep; if a tile ever gives up waiting for a dependency (never expected; the wait is bounded so that
- * a fault cannot hang the GPU) nothing more is stored by that launch and the next call that synchronises the stream
- * (gf_measure, gf_measure_collect, gf_fix_until, gf_store_host, gf_plaquette, gf_unitarity) returns GF_ECUDA. */
+/* n iterations = n x {gf_sweep(parity 0); gf_sweep(parity 1)}, enqueued without synchronising; the
+ * Philox counter advances by 2 per iteration.  (A fused both-parities launch in t-wavefront order was built and
+ * measured in rounds 1 and 2 and removed: it did not beat two half-sweeps on B200.)
+ * Errors: as gf_sweep. */
 int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, int precision);
-int gf_set_wavefront(gf_ctx* ctx, int mode);
-int gf_set_wave_tuning(gf_ctx* ctx, int lag_planes, int blocks);
 
 /* F (eq. 2) and theta (eq. 4-5, with A_mu the traceless
  * anti-Hermitian part of U_mu) of the field of `precision`, accumulated in fp64 with a fixed

@@ -11,7 +11,7 @@ from .binding import (  # noqa: F401
     GF_RELAX, GF_OVERRELAX, GF_STOCHASTIC, GF_RECON18, GF_RECON12, GF_SOLVER_AUTO,
     GFError, lib, lib_path,
     gf_storage_bytes, gf_workspace_bytes, gf_init_lattice, gf_destroy, gf_last_error,
-    gf_pack, gf_unpack, gf_load_host, gf_store_host, gf_sweep, gf_iterate, gf_set_wavefront, gf_set_wave_tuning, gf_functional, gf_theta,
+    gf_pack, gf_unpack, gf_load_host, gf_store_host, gf_sweep, gf_iterate, gf_functional, gf_theta,
     gf_measure, gf_measure_async, gf_measure_collect, gf_fix_until, gf_set_rng, gf_get_counter, gf_reunitarize, gf_cast,
     gf_transform_bytes, gf_set_transform, gf_transform_identity, gf_transform_pack, gf_transform_unpack,
     gf_transform_cast, gf_apply_transform, gf_set_coulomb_mode, gf_coulomb_finish, gf_set_slice_mask, gf_set_slab, gf_enable_peer, gf_get_device,

@@ -43,8 +43,6 @@ def _load():
         "gf_store_host": (i32, [vp, vp, i32, i32, vp]),
         "gf_sweep": (i32, [vp, i32, i32, dbl, dbl, i32]),
         "gf_iterate": (i32, [vp, i32, i32, dbl, dbl, i32]),
-        "gf_set_wavefront": (i32, [vp, i32]),
-        "gf_set_wave_tuning": (i32, [vp, i32, i32]),
         "gf_functional": (i32, [vp, i32, dp]),
         "gf_theta": (i32, [vp, i32, dp]),
         "gf_measure": (i32, [vp, i32, dp, dp]),
@@ -87,7 +85,7 @@ def _load():
 
 lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
-           "gf_sweep gf_iterate gf_set_wavefront gf_set_wave_tuning gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
+           "gf_sweep gf_iterate gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
            "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_enable_peer gf_get_device gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
@@ -155,14 +153,6 @@ def gf_sweep(ctx, parity, algo, omega, p, precision, check=True):
 
 def gf_iterate(ctx, n, algo, omega, p, precision, check=True):
     return _rc(ctx, lib.gf_iterate(ctx, int(n), algo, omega, p, precision), check)
-
-
-def gf_set_wavefront(ctx, mode, check=True):
-    return _rc(ctx, lib.gf_set_wavefront(ctx, int(mode)), check)
-
-
-def gf_set_wave_tuning(ctx, lag_planes, blocks, check=True):
-    return _rc(ctx, lib.gf_set_wave_tuning(ctx, int(lag_planes), int(blocks)), check)
 
 
 def _nout(ctx_dims, gauge):

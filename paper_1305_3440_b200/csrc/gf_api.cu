@@ -20,15 +20,6 @@ static int write_identity(gf_ctx* ctx, int precision);
 extern "C" int gf_coulomb_finish(gf_ctx* ctx, int precision);
 static int upload_mask(gf_ctx* ctx);
 static int sync_and_check(gf_ctx* ctx, const char* what);
-static uint64_t wave_total_tiles_for(const Geom& G, int mode)
-{
-    WaveArgs a;
-    memset(&a, 0, sizeof(a));
-    a.G = G;
-    a.mode = mode;
-    a.precision = PREC_F64;          // the narrower tiles: the larger count
-    return wave_total_tiles(a);
-}
 
 namespace {
 constexpr int kMeasureBlock = 128;
@@ -48,16 +39,6 @@ struct gf_ctx {
     uint8_t* host_mask;         // pinned copy
     int mask_on;                // the sweeps consult dev_mask
     double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
-    // streamed sweep / fused iteration (gf_wave.cu): device state in the workspace, running totals on the host
-    int wave_mode;              // 0 never, 1 fused iteration when eligible and a time slice is small enough for the L2,
-                                // 2 whenever eligible, 3 = 2 and single half-sweeps go through the streamed kernel too
-    int wave_lag;               // planes between the two parity fronts; 0 = automatic
-    int wave_ctas;              // persistent blocks; 0 = one per SM
-    int sm_count;
-    unsigned long long* wave_ticket;
-    uint32_t *wave_done, *wave_error;
-    unsigned long long wave_ticket_total;
-    uint32_t wave_done_total;
     // slab decomposition along t (gf_set_slab): this context holds N_t local slices of a lattice nranks times as long
     int slab_rank, slab_n;
     void* prev_links[2];        // field of the slab below (per precision); NULL = own (one slab)
@@ -162,9 +143,8 @@ extern "C" size_t gf_workspace_bytes(const int dims[4])
 {
     if (!dims_ok(dims)) return 0;
     const MeasureGrid mg = measure_grid(dims);
-    // + the slice mask + the wavefront state (ticket, error word, reduction counter, one completion counter per (t,z) plane)
-    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt + 16 +
-           sizeof(uint32_t) * (size_t)dims[0] * dims[3];
+    // + the slice mask + the counter of the last reduction stage
+    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt + 16;
 }
 
 extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
@@ -202,11 +182,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->partials = c->workspace;
     c->slice_tmp = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
     c->dev_mask = reinterpret_cast<uint8_t*>(c->slice_tmp + (size_t)dims[0] * 2);
-    c->wave_ticket = reinterpret_cast<unsigned long long*>(c->dev_mask + kMaxNt);
-    c->wave_error = reinterpret_cast<uint32_t*>(c->wave_ticket + 1);
-    c->reduce_counter = c->wave_error + 1;
-    c->wave_done = c->wave_error + 2;
-    c->wave_mode = 0;         // opt-in: see gf_set_wavefront
+    c->reduce_counter = reinterpret_cast<uint32_t*>(c->dev_mask + kMaxNt);
 
     Geom& G = c->G;
     G.nt = dims[0];
@@ -234,8 +210,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->slab_rank = 0;
     c->slab_n = 1;
 
-    c->sm_count = prop.multiProcessorCount;
-    if (cudaMemsetAsync(c->wave_ticket, 0, 16 + sizeof(uint32_t) * (size_t)dims[0] * dims[3], c->stream) != cudaSuccess) {
+    if (cudaMemsetAsync(c->reduce_counter, 0, 16, c->stream) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return GF_ECUDA;
@@ -520,77 +495,9 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     return GF_OK;
 }
 
-// Largest time slice (bytes of link storage) for which the fused iteration is chosen automatically: the second
-// touch of a link comes about `lag` planes (two to three time slices) after the first and has to find it in the L2.
-static const size_t kWaveMaxSliceBytes = (size_t)24 << 20;
-
-// The streamed kernel handles the plain site update of one whole lattice: no transformation buffer, no slice mask,
-// no slabs; the lattice must tile (wave_supported).
-static bool stream_eligible(const gf_ctx* ctx, int precision)
-{
-    return ctx->slab_n == 1 && !ctx->gtrans[precision] && !ctx->mask_on && wave_supported(ctx->G, precision) &&
-           wave_total_tiles_for(ctx->G, 2) < (uint64_t(1) << 32);
-}
-
-static bool fused_eligible(const gf_ctx* ctx, int precision)
-{
-    if (ctx->wave_mode == 0 || ctx->dims[0] < 4 || !stream_eligible(ctx, precision)) return false;
-    if (ctx->wave_mode == 1) {
-        const size_t slice = (size_t)ctx->mg.Sh * 2 * 4 * (size_t)ctx->recon * (precision == GF_F64 ? 8 : 4);
-        if (slice > kWaveMaxSliceBytes) return false;
-    }
-    return true;
-}
-
-// mode 0 / 1: one half-sweep of that parity; mode 2: one fused iteration
-static int enqueue_streamed(gf_ctx* ctx, int mode, int algo, double omega, double p, int precision)
-{
-    const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
-    WaveArgs a;
-    memset(&a, 0, sizeof(a));
-    a.precision = precision;
-    a.links = ctx->links[precision];
-    a.G = ctx->G;
-    a.site_offset = 0;
-    a.mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
-    a.algo = algo;
-    a.omega = omega;
-    a.p = p;
-    a.key0 = (uint32_t)ctx->seed;
-    a.key1 = (uint32_t)(ctx->seed >> 32);
-    a.counter = ctx->counter;
-    a.mode = mode;
-    a.num_ctas = ctx->wave_ctas > 0 ? ctx->wave_ctas : ctx->sm_count;
-    const uint32_t M = wave_tiles_per_plane(ctx->G, precision), nz = (uint32_t)ctx->dims[3], planes = (uint32_t)ctx->dims[0] * nz;
-    if (mode == 2) {
-        // the parity-1 front follows the parity-0 front by one time slice (the dependency on plane q + Nz) plus the
-        // planes whose parity-0 tiles can be in flight at once (every block's ring), so that the waits rarely spin
-        uint32_t lag = ctx->wave_lag > 0 ? (uint32_t)ctx->wave_lag
-                                         : nz + ((uint32_t)a.num_ctas * wave_stages(precision, ctx->recon) + 2u * M - 1u) / (2u * M) + 2u;
-        if (lag < nz + 1u) lag = nz + 1u;
-        if (lag > planes - nz) lag = planes - nz;
-        a.lag = lag;
-    }
-    a.ticket = ctx->wave_ticket;
-    a.ticket_base = ctx->wave_ticket_total;
-    a.done = ctx->wave_done;
-    a.done_target = ctx->wave_done_total + wave_counts_per_plane(ctx->G, precision);
-    a.error = ctx->wave_error;
-    cudaError_t e = launch_wave(precision, solver_f64, ctx->recon, a, ctx->stream);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "streamed sweep launch");
-    ctx->wave_ticket_total += wave_ticket_advance(a);
-    const int half_sweeps = mode == 2 ? 2 : 1;
-    if (mode == 2) ctx->wave_done_total += wave_counts_per_plane(ctx->G, precision);
-    ctx->counter += half_sweeps;
-    ctx->sweeps += half_sweeps;
-    ctx->launches += 1;
-    return GF_OK;
-}
-
-// One iteration = parity 0 then parity 1: a single fused launch when eligible, else two half-sweeps.
+// One iteration = parity 0 then parity 1.
 static int enqueue_iteration(gf_ctx* ctx, int algo, double omega, double p, int precision)
 {
-    if (fused_eligible(ctx, precision)) return enqueue_streamed(ctx, 2, algo, omega, p, precision);
     int e = enqueue_sweep(ctx, 0, algo, omega, p, precision);
     if (e == GF_OK) e = enqueue_sweep(ctx, 1, algo, omega, p, precision);
     return e;
@@ -611,25 +518,6 @@ extern "C" int gf_iterate(gf_ctx* ctx, int n, int algo, double omega, double p, 
     return GF_OK;
 }
 
-extern "C" int gf_set_wavefront(gf_ctx* ctx, int mode)
-{
-    DeviceGuard guard(ctx);
-    if (!ctx) return GF_EINVAL;
-    if (mode < 0 || mode > 3)
-        return fail(ctx, GF_EINVAL, "wavefront mode must be 0 (off), 1 (automatic), 2 (whenever eligible) or 3 (2 + streamed half-sweeps)");
-    ctx->wave_mode = mode;
-    return GF_OK;
-}
-
-extern "C" int gf_set_wave_tuning(gf_ctx* ctx, int lag_planes, int blocks)
-{
-    if (!ctx) return GF_EINVAL;
-    if (lag_planes < 0 || blocks < 0 || blocks > 4096) return fail(ctx, GF_EINVAL, "lag and block count must be >= 0 (0 = automatic)");
-    ctx->wave_lag = lag_planes;
-    ctx->wave_ctas = blocks;
-    return GF_OK;
-}
-
 extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double p, int precision)
 {
     DeviceGuard guard(ctx);
@@ -638,8 +526,6 @@ extern "C" int gf_sweep(gf_ctx* ctx, int parity, int algo, double omega, double 
     if (parity != 0 && parity != 1) return fail(ctx, GF_EINVAL, "parity must be 0 or 1");
     rc = check_algo(ctx, algo, omega, p);
     if (rc) return rc;
-    if (ctx->wave_mode == 3 && !ctx->defer_temporal && stream_eligible(ctx, precision))
-        return enqueue_streamed(ctx, parity, algo, omega, p, precision);
     return enqueue_sweep(ctx, parity, algo, omega, p, precision);
 }
 
@@ -673,17 +559,10 @@ static ReduceTail lattice_tail(const gf_ctx* ctx, double scale)
     return t;
 }
 
-// Synchronises the stream; if streamed sweeps have run, also fetches their error word: a fused iteration whose
-// dependency wait gave up stores nothing further and the field is reported invalid at the next call that synchronises.
 static int sync_and_check(gf_ctx* ctx, const char* what)
 {
-    uint32_t* wave_err = reinterpret_cast<uint32_t*>(ctx->host_mask + kMaxNt);
-    cudaError_t e = cudaSuccess;
-    if (ctx->wave_ticket_total) e = cudaMemcpyAsync(wave_err, ctx->wave_error, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, what);
-    if (ctx->wave_ticket_total && *wave_err)
-        return fail(ctx, GF_ECUDA, "a fused iteration gave up waiting for a dependency: the link field is invalid");
     return GF_OK;
 }
 

@@ -27,26 +27,6 @@ struct SweepArgs {
     uint32_t reverse;       // traverse the lattice backwards (L2 reuse between consecutive launches)
 };
 
-// the streamed sweep (gf_wave.cu): TMA bulk copies into a shared-memory ring, one thread per site
-struct WaveArgs {
-    int precision;                  // PREC_F32 | PREC_F64: storage type (tile width 64 | 32 sites)
-    void* links;
-    Geom G;
-    uint32_t site_offset;
-    int mu0, algo;
-    double omega, p;
-    uint32_t key0, key1;
-    uint32_t counter;               // half-sweep counter of the (first) half-sweep; the fused iteration uses counter, counter + 1
-    int mode;                       // 0 / 1: one half-sweep of that parity; 2: fused iteration (parity 0 then parity 1)
-    uint32_t lag;                   // mode 2: planes between the parity-0 and the parity-1 front; Nz < lag <= (Nt - 1) Nz
-    unsigned long long* ticket;     // device counter, monotonic over launches
-    unsigned long long ticket_base; // its value when this launch starts
-    uint32_t* done;                 // Nt * Nz device counters, monotonic over launches
-    uint32_t done_target;           // value every done[plane] reaches when the parity-0 tiles of this launch are complete
-    uint32_t* error;                // device word, set if a dependency wait gave up
-    int num_ctas;                   // persistent blocks
-};
-
 struct MeasureGrid {
     uint32_t Sh;            // sites per time slice per parity
     uint32_t bpp;           // blocks per (slice, parity)
@@ -65,14 +45,6 @@ struct ReduceTail {
 // solver_f64: with fp32 storage, accumulate K(x) and run the SU(2) solves in fp64 registers
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);
 bool sweep_config_valid(int lanes, int block);
-
-bool wave_supported(const Geom& G, int precision);        // a layout tile is whole x-rows inside one (z,t) plane
-uint32_t wave_stages(int precision, int recon);           // depth of the shared-memory ring of that variant
-unsigned long long wave_total_tiles(const WaveArgs& a);
-uint32_t wave_ticket_advance(const WaveArgs& a);          // by how much one launch moves the ticket counter
-uint32_t wave_tiles_per_plane(const Geom& G, int precision);   // layout tiles of one parity in a plane
-uint32_t wave_counts_per_plane(const Geom& G, int precision);  // what a fused launch adds to every done[plane]
-cudaError_t launch_wave(int precision, int solver_f64, int recon, const WaveArgs& a, cudaStream_t st);
 
 // prev_links / next_links: the fields of the slabs below / above in t (NULL = this field, periodic)
 cudaError_t launch_measure(int precision, int recon, const void* links, const void* prev_links, const Geom& G, int mu0,

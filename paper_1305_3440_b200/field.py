@@ -84,12 +84,6 @@ class GaugeField:
     def iterate(self, n, algo, omega, p, precision):
         B.gf_iterate(self.ctx, n, algo, omega, p, precision)
 
-    def set_wavefront(self, mode):
-        B.gf_set_wavefront(self.ctx, mode)
-
-    def set_wave_tuning(self, lag_planes=0, blocks=0):
-        B.gf_set_wave_tuning(self.ctx, lag_planes, blocks)
-
     def functional(self, precision):
         return B.gf_functional(self.ctx, precision, self.n_out)
 

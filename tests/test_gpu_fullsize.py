@@ -34,18 +34,36 @@ def held_by_device(fld, prec):
 
 @pytest.mark.parametrize("prec,recon", [("f64", 18), ("f64", 12), ("f32", 18), ("f32", 12)])
 def test_32_4_full_field_against_oracle(cuda_device, prec, recon):
-    """configs[2]: 32^4, eps 0.6 smooth field + Haar gauge transform, overrelaxation omega = 1.7."""
+    """configs[2]: 32^4, eps 0.6 smooth field + Haar gauge transform, overrelaxation omega = 1.7.
+
+    fp64: every link within 1e-12 of the oracle after each of the two half-sweeps, the oracle running on from its own
+    field.  fp32 (default solver: K(x) and the SU(2) solves in fp32): every link within 1e-5 after EACH half-sweep
+    judged from the field the device held before it -- the error of a site update is eps32 |K| / |v| (DESIGN.md,
+    "Tolerances"), and among the 524 288 sites of a half-sweep of this field there is one whose SU(2) projection |v| is
+    45 times smaller than its block of K: 8.8e-6 there, 1.2e-7 in the median.  Carried through the second half-sweep
+    without re-synchronising, that site's links end 1.08e-5 from the oracle's, which is why the fp32 links are
+    re-synchronised between the half-sweeps while F and theta after 10 iterations are compared with an oracle that
+    never is.  The same kernels with the solves in fp64 registers (gf_set_solver_precision) stay within 1e-6
+    cumulatively; that is checked too."""
     dims = (32, 32, 32, 32)
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device).to(CDTYPE[prec])
     fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)     # default tuning = what bench.py times
     fld.pack(U, PREC[prec])
-    del U
-    Uo = held_by_device(fld, prec)
+    Uo = held_by_device(fld, prec)                # the oracle that runs on freely (F / theta after 10 iterations)
+    Us = Uo.copy() if prec == "f32" else Uo       # fp32: re-synchronised before every half-sweep (links)
     for parity in (0, 1):
         fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
         oracle.sweep(Uo, dims, parity, oracle.LANDAU, oracle.OVERRELAX, 1.7)
-        err = float(np.abs(held_by_device(fld, prec) - Uo).max())              # all 4 194 304 links
+        if prec == "f32":
+            oracle.sweep(Us, dims, parity, oracle.LANDAU, oracle.OVERRELAX, 1.7)
+        got = held_by_device(fld, prec)
+        err = float(np.abs(got - Us).max())                                    # all 4 194 304 links
         assert err < LINK_TOL[prec], (prec, recon, parity, err)
+        if prec == "f32":
+            assert float(np.median(np.abs(got - Us))) < 2e-7
+            assert float(np.abs(got - Uo).max()) < 3e-5                         # never re-synchronised: still an fp32-sized error
+            Us = got
+    del Us
     fld.iterate(9, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])                       # the call bench.py's step uses
     for it in range(9):
         for parity in (0, 1):
@@ -58,6 +76,15 @@ def test_32_4_full_field_against_oracle(cuda_device, prec, recon):
     assert du < (1e-12 if prec == "f64" else 1e-5) and dd < (1e-12 if prec == "f64" else 1e-5)
     gdu, gdd = fld.unitarity(PREC[prec])
     assert abs(gdu - du) < (1e-13 if prec == "f64" else 1e-6) and abs(gdd - dd) < (1e-13 if prec == "f64" else 1e-6)
+    if prec == "f32":
+        # fp32 storage, solves in fp64 registers: one whole iteration, no re-synchronisation
+        fld.set_solver_precision(gf.GF_F64)
+        fld.pack(U, PREC[prec])
+        Uo = held_by_device(fld, prec)
+        for parity in (0, 1):
+            fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+            oracle.sweep(Uo, dims, parity, oracle.LANDAU, oracle.OVERRELAX, 1.7)
+        assert float(np.abs(held_by_device(fld, prec) - Uo).max()) < 1e-6
     fld.close()
 
 
@@ -155,6 +182,7 @@ def test_32_4_accumulated_transformation_full_field(cuda_device, prec, recon):
         fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
         oracle.sweep_accumulate(Uo, Go, dims, parity, oracle.LANDAU, oracle.OVERRELAX, 1.7)
     G = fld.transform(PREC[prec], torch.complex128).cpu().numpy()
-    assert np.abs(G - Go).max() < LINK_TOL[prec]
-    assert np.abs(held_by_device(fld, prec) - Uo).max() < LINK_TOL[prec]
+    assert np.abs(G - Go).max() < LINK_TOL[prec]                     # every G(x) is the product of ONE site update so far
+    # the links have been through both half-sweeps (fp32: see test_32_4_full_field_against_oracle on the ill-conditioned site)
+    assert np.abs(held_by_device(fld, prec) - Uo).max() < (LINK_TOL[prec] if prec == "f64" else 3e-5)
     fld.close()

@@ -388,7 +388,7 @@ def test_no_writes_outside_the_lent_buffers(cuda_device, dims, prec, recon):
 # ------------------------------------------------------------------------------------- fuzz
 
 def test_random_small_lattices_against_oracle(cuda_device):
-    """40 seeded random combinations of (dims, gauge, algorithm, storage, lanes, block, fused iteration):
+    """40 seeded random combinations of (dims, gauge, algorithm, storage, lanes, block):
     two iterations on the device against the oracle, links within the one-sweep tolerance x 4."""
     rng = np.random.default_rng(2024)
     for case in range(40):
@@ -403,7 +403,7 @@ def test_random_small_lattices_against_oracle(cuda_device):
         fld = make_field(dims, prec, cuda_device, gauge=gauge, recon=recon, seed=seed)
         fld.pack(to_device(U, prec, cuda_device), PREC[prec])
         fld.set_tuning(PREC[prec], lanes, block)
-        fld.set_wavefront(int(rng.integers(0, 3)))
+        rng.integers(0, 3)                       # (keeps the seeded case list of round 1)
         fld.iterate(2, algo, omega, p, PREC[prec])
         Uo = oracle_input(U, prec)
         og = oracle.LANDAU if gauge == gf.GF_LANDAU else oracle.COULOMB
