@@ -318,47 +318,80 @@ cudaError_t launch_unitarity(int precision, int recon, const void* links, const 
 }
 
 // ---------------------------------------------------------------------- pack / unpack / cast
-// a11: canonical AoS (site s, mu, 3x3 row-major complex) <-> the private chunked layout.
-// One thread per site; the AoS side is strided (16 of every 32-byte sector per instruction).  A
-// version that transposes through a shared-memory tile is 3.6x faster in isolation (unpack 0.81 ->
-// 0.23 ms at 32^4) but was measured to slow the pipelined end-to-end step from 41 to 50 ms: kernels
-// that need shared memory do not share SMs smoothly with the register-bound sweep kernels of the
-// other lattices in flight.  These conversions run once per field, so the simple form stays.
-template <typename T, int RECON, typename TC>
-__global__ void pack_kernel(T* __restrict__ links, const Geom G, const TC* __restrict__ canonical)
+// a11: canonical AoS (site s, mu, 3x3 row-major complex) <-> the private tiled layout, transposed through a small
+// shared-memory tile so that BOTH sides move whole 16-byte vectors to consecutive addresses.  A block takes a
+// segment of PACK_TH consecutive half-indices of one x-row: with both parities that is 2 * PACK_TH consecutive
+// canonical sites (x = 2 xh + xodd, the two parities interleave along x), i.e. one contiguous canonical range of
+// 2 * PACK_TH * 72 reals = 9216 bytes in fp64.  One thread per link does the private-layout side (load_link /
+// store_link: 16-byte chunks, consecutive lanes consecutive sites; reconstruction of row 2 for 12-real storage), all
+// threads stream the canonical side.  64 threads and at most 9 KB of static shared memory per block: such blocks
+// co-reside with the register-bound sweep blocks of other lattices in flight (the round-1 transpose, with large
+// dynamic tiles, did not: it was 3.6x faster alone and slowed the pipelined end-to-end step).
+constexpr uint32_t PACK_TH = 8;                       // half-indices per segment
+constexpr uint32_t PACK_THREADS = 2 * 4 * PACK_TH;    // one thread per (parity, mu, site) link
+
+struct PackSegment {
+    uint32_t h0, len;       // first half-index and number of sites (<= PACK_TH; the last segment of a row may be short)
+    uint32_t xodd0;         // x & 1 of the parity-0 sites of this row
+    size_t site0;           // canonical index of the first site of the range: 2 * h0
+};
+
+__device__ __forceinline__ PackSegment pack_segment(const Geom& G, uint32_t segs_per_row)
 {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= 2u * G.Vh) return;
-    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
-    const Site s = decode_site(G, h, parity);
-    const size_t site = 2u * (size_t)h + s.xodd;
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
-        const TC* src = canonical + (site * 4 + mu) * 18;
-        T m[18];
-#pragma unroll
-        for (int k = 0; k < 18; ++k) m[k] = (T)src[k];
-        store_link<RECON>(links + block_offset<T>(parity, mu, RECON, G), h, m);
-    }
+    PackSegment p;
+    const uint32_t row = blockIdx.x / segs_per_row, seg = blockIdx.x - row * segs_per_row;
+    p.h0 = row * G.nxh + seg * PACK_TH;
+    p.len = min(PACK_TH, G.nxh - seg * PACK_TH);
+    const Site s = decode_site(G, p.h0, 0u);
+    p.xodd0 = s.xodd;
+    p.site0 = 2u * (size_t)p.h0;
+    return p;
 }
 
 template <typename T, int RECON, typename TC>
-__global__ void unpack_kernel(const T* __restrict__ links, const Geom G, TC* __restrict__ canonical)
+__global__ void __launch_bounds__(PACK_THREADS) pack_kernel(T* __restrict__ links, const Geom G, const uint32_t segs_per_row,
+                                                            const TC* __restrict__ canonical)
 {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= 2u * G.Vh) return;
-    const uint32_t parity = i >= G.Vh ? 1u : 0u, h = i - parity * G.Vh;
-    const Site s = decode_site(G, h, parity);
-    const size_t site = 2u * (size_t)h + s.xodd;
+    __shared__ __align__(16) TC tile[2 * PACK_TH * 72];
+    const PackSegment p = pack_segment(G, segs_per_row);
+    // canonical -> shared: one contiguous range, 16-byte vectors (72 reals per site: always whole vectors)
+    using V = typename Vec16<TC>::type;
+    constexpr uint32_t PER = 16u / (uint32_t)sizeof(TC);
+    const uint32_t nvec = 2u * p.len * 72u / PER;
+    const V* src = reinterpret_cast<const V*>(canonical + p.site0 * 72u);
+    for (uint32_t i = threadIdx.x; i < nvec; i += PACK_THREADS) reinterpret_cast<V*>(tile)[i] = src[i];
+    __syncthreads();
+    // shared -> private layout: thread = (parity, mu, k)
+    const uint32_t k = threadIdx.x % PACK_TH, mu = (threadIdx.x / PACK_TH) & 3u, parity = threadIdx.x / (4u * PACK_TH);
+    if (k >= p.len) return;
+    const uint32_t local = 2u * k + (p.xodd0 ^ parity);          // site of this parity inside the canonical range
+    T m[18];
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
+    for (int q = 0; q < 18; ++q) m[q] = (T)tile[(local * 4u + mu) * 18u + q];
+    store_link<RECON>(links + block_offset<T>(parity, (int)mu, RECON, G), p.h0 + k, m);
+}
+
+template <typename T, int RECON, typename TC>
+__global__ void __launch_bounds__(PACK_THREADS) unpack_kernel(const T* __restrict__ links, const Geom G, const uint32_t segs_per_row,
+                                                              TC* __restrict__ canonical)
+{
+    __shared__ __align__(16) TC tile[2 * PACK_TH * 72];
+    const PackSegment p = pack_segment(G, segs_per_row);
+    const uint32_t k = threadIdx.x % PACK_TH, mu = (threadIdx.x / PACK_TH) & 3u, parity = threadIdx.x / (4u * PACK_TH);
+    if (k < p.len) {
+        const uint32_t local = 2u * k + (p.xodd0 ^ parity);
         T m[18];
-        load_link<RECON>(links + block_offset<T>(parity, mu, RECON, G), h, m);
+        load_link<RECON>(links + block_offset<T>(parity, (int)mu, RECON, G), p.h0 + k, m);
         if (RECON == 12) reconstruct_row2(m);
-        TC* dst = canonical + (site * 4 + mu) * 18;
 #pragma unroll
-        for (int k = 0; k < 18; ++k) dst[k] = (TC)m[k];
+        for (int q = 0; q < 18; ++q) tile[(local * 4u + mu) * 18u + q] = (TC)m[q];
     }
+    __syncthreads();
+    using V = typename Vec16<TC>::type;
+    constexpr uint32_t PER = 16u / (uint32_t)sizeof(TC);
+    const uint32_t nvec = 2u * p.len * 72u / PER;
+    V* dst = reinterpret_cast<V*>(canonical + p.site0 * 72u);
+    for (uint32_t i = threadIdx.x; i < nvec; i += PACK_THREADS) dst[i] = reinterpret_cast<const V*>(tile)[i];
 }
 
 // Gram-Schmidt on rows 0 and 1, row 2 = conj(row 0 x row 1)
@@ -409,25 +442,27 @@ __global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int repr
     store_link<RECON>(dst + (size_t)pm * RECON * padded_vh<TD>(G), h, o);
 }
 
+static uint32_t pack_segments_per_row(const Geom& G) { return (G.nxh + PACK_TH - 1u) / PACK_TH; }
+
 template <typename T, int RECON>
 static cudaError_t pack_run(void* links, const Geom& G, const void* canonical, int canonical_is_f64, cudaStream_t st)
 {
-    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    const uint32_t spr = pack_segments_per_row(G), grid = G.Vh / G.nxh * spr;
     if (canonical_is_f64)
-        pack_kernel<T, RECON, double><<<grid, block, 0, st>>>(static_cast<T*>(links), G, static_cast<const double*>(canonical));
+        pack_kernel<T, RECON, double><<<grid, PACK_THREADS, 0, st>>>(static_cast<T*>(links), G, spr, static_cast<const double*>(canonical));
     else
-        pack_kernel<T, RECON, float><<<grid, block, 0, st>>>(static_cast<T*>(links), G, static_cast<const float*>(canonical));
+        pack_kernel<T, RECON, float><<<grid, PACK_THREADS, 0, st>>>(static_cast<T*>(links), G, spr, static_cast<const float*>(canonical));
     return cudaGetLastError();
 }
 
 template <typename T, int RECON>
 static cudaError_t unpack_run(const void* links, const Geom& G, void* canonical, int canonical_is_f64, cudaStream_t st)
 {
-    const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
+    const uint32_t spr = pack_segments_per_row(G), grid = G.Vh / G.nxh * spr;
     if (canonical_is_f64)
-        unpack_kernel<T, RECON, double><<<grid, block, 0, st>>>(static_cast<const T*>(links), G, static_cast<double*>(canonical));
+        unpack_kernel<T, RECON, double><<<grid, PACK_THREADS, 0, st>>>(static_cast<const T*>(links), G, spr, static_cast<double*>(canonical));
     else
-        unpack_kernel<T, RECON, float><<<grid, block, 0, st>>>(static_cast<const T*>(links), G, static_cast<float*>(canonical));
+        unpack_kernel<T, RECON, float><<<grid, PACK_THREADS, 0, st>>>(static_cast<const T*>(links), G, spr, static_cast<float*>(canonical));
     return cudaGetLastError();
 }
 
