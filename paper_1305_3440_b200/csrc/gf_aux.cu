@@ -271,8 +271,10 @@ template <typename T, int RECON> struct MeasureLauncher {
     static cudaError_t run(const void* links, const void* prev_links, const Geom& G, int mu0, const MeasureGrid& mg, double* partials,
                            const ReduceTail& tail, double* slice_out, cudaStream_t st)
     {
+        uniform_carveout(measure_kernel<T, RECON>);
         measure_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
                                                                            static_cast<const T*>(prev_links ? prev_links : links), G, mu0, mg, partials);
+        uniform_carveout(reduce_slices_kernel<OpSum>);
         reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
         return cudaGetLastError();
     }
@@ -282,8 +284,10 @@ template <typename T, int RECON> struct PlaquetteLauncher {
     static cudaError_t run(const void* links, const void* next_links, const Geom& G, const MeasureGrid& mg, double* partials,
                            const ReduceTail& tail, double* slice_out, cudaStream_t st)
     {
+        uniform_carveout(plaquette_kernel<T, RECON>);
         plaquette_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
                                                                              static_cast<const T*>(next_links ? next_links : links), G, mg, partials);
+        uniform_carveout(reduce_slices_kernel<OpSum>);
         reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
         return cudaGetLastError();
     }
@@ -293,7 +297,9 @@ template <typename T, int RECON> struct UnitarityLauncher {
     static cudaError_t run(const void* links, const Geom& G, const MeasureGrid& mg, double* partials,
                            const ReduceTail& tail, double* slice_out, cudaStream_t st)
     {
+        uniform_carveout(unitarity_kernel<T, RECON>);
         unitarity_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mg, partials);
+        uniform_carveout(reduce_slices_kernel<OpMax>);
         reduce_slices_kernel<OpMax><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
         return cudaGetLastError();
     }
@@ -448,10 +454,13 @@ template <typename T, int RECON>
 static cudaError_t pack_run(void* links, const Geom& G, const void* canonical, int canonical_is_f64, cudaStream_t st)
 {
     const uint32_t spr = pack_segments_per_row(G), grid = G.Vh / G.nxh * spr;
-    if (canonical_is_f64)
+    if (canonical_is_f64) {
+        uniform_carveout(pack_kernel<T, RECON, double>);
         pack_kernel<T, RECON, double><<<grid, PACK_THREADS, 0, st>>>(static_cast<T*>(links), G, spr, static_cast<const double*>(canonical));
-    else
+    } else {
+        uniform_carveout(pack_kernel<T, RECON, float>);
         pack_kernel<T, RECON, float><<<grid, PACK_THREADS, 0, st>>>(static_cast<T*>(links), G, spr, static_cast<const float*>(canonical));
+    }
     return cudaGetLastError();
 }
 
@@ -459,10 +468,13 @@ template <typename T, int RECON>
 static cudaError_t unpack_run(const void* links, const Geom& G, void* canonical, int canonical_is_f64, cudaStream_t st)
 {
     const uint32_t spr = pack_segments_per_row(G), grid = G.Vh / G.nxh * spr;
-    if (canonical_is_f64)
+    if (canonical_is_f64) {
+        uniform_carveout(unpack_kernel<T, RECON, double>);
         unpack_kernel<T, RECON, double><<<grid, PACK_THREADS, 0, st>>>(static_cast<const T*>(links), G, spr, static_cast<double*>(canonical));
-    else
+    } else {
+        uniform_carveout(unpack_kernel<T, RECON, float>);
         unpack_kernel<T, RECON, float><<<grid, PACK_THREADS, 0, st>>>(static_cast<const T*>(links), G, spr, static_cast<float*>(canonical));
+    }
     return cudaGetLastError();
 }
 
@@ -491,10 +503,13 @@ static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G
 {
     const uint32_t block = 128;
     const dim3 grid((G.Vh + block - 1) / block, (uint32_t)nblocks, 1);
-    if (recon == 12)
+    if (recon == 12) {
+        uniform_carveout(cast_kernel<TS, TD, 12>);
         cast_kernel<TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
-    else
+    } else {
+        uniform_carveout(cast_kernel<TS, TD, 18>);
         cast_kernel<TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
+    }
     return cudaGetLastError();
 }
 
@@ -548,10 +563,13 @@ template <typename T, int RECON, bool TO_INTERNAL>
 static cudaError_t transform_convert_run(void* gtrans, const Geom& G, void* canonical, int canonical_is_f64, cudaStream_t st)
 {
     const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
-    if (canonical_is_f64)
+    if (canonical_is_f64) {
+        uniform_carveout(transform_convert_kernel<T, RECON, double, TO_INTERNAL>);
         transform_convert_kernel<T, RECON, double, TO_INTERNAL><<<grid, block, 0, st>>>(static_cast<T*>(gtrans), G, static_cast<double*>(canonical));
-    else
+    } else {
+        uniform_carveout(transform_convert_kernel<T, RECON, float, TO_INTERNAL>);
         transform_convert_kernel<T, RECON, float, TO_INTERNAL><<<grid, block, 0, st>>>(static_cast<T*>(gtrans), G, static_cast<float*>(canonical));
+    }
     return cudaGetLastError();
 }
 
@@ -581,11 +599,11 @@ cudaError_t launch_transform_identity(int precision, int recon, void* gtrans, co
 {
     const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
     if (precision == PREC_F64) {
-        if (recon == 12) transform_identity_kernel<double, 12><<<grid, block, 0, st>>>(static_cast<double*>(gtrans), G);
-        else transform_identity_kernel<double, 18><<<grid, block, 0, st>>>(static_cast<double*>(gtrans), G);
+        if (recon == 12) { uniform_carveout(transform_identity_kernel<double, 12>); transform_identity_kernel<double, 12><<<grid, block, 0, st>>>(static_cast<double*>(gtrans), G); }
+        else { uniform_carveout(transform_identity_kernel<double, 18>); transform_identity_kernel<double, 18><<<grid, block, 0, st>>>(static_cast<double*>(gtrans), G); }
     } else {
-        if (recon == 12) transform_identity_kernel<float, 12><<<grid, block, 0, st>>>(static_cast<float*>(gtrans), G);
-        else transform_identity_kernel<float, 18><<<grid, block, 0, st>>>(static_cast<float*>(gtrans), G);
+        if (recon == 12) { uniform_carveout(transform_identity_kernel<float, 12>); transform_identity_kernel<float, 12><<<grid, block, 0, st>>>(static_cast<float*>(gtrans), G); }
+        else { uniform_carveout(transform_identity_kernel<float, 18>); transform_identity_kernel<float, 18><<<grid, block, 0, st>>>(static_cast<float*>(gtrans), G); }
     }
     return cudaGetLastError();
 }
@@ -633,10 +651,13 @@ static cudaError_t apply_run(int recon, const void* gtrans, const void* src, voi
                              cudaStream_t st)
 {
     const uint32_t n = 2u * G.Vh, block = 128, grid = (n + block - 1) / block;
-    if (recon == 12)
+    if (recon == 12) {
+        uniform_carveout(apply_transform_kernel<TG, TS, TD, 12>);
         apply_transform_kernel<TG, TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G, mu_begin, mu_end);
-    else
+    } else {
+        uniform_carveout(apply_transform_kernel<TG, TS, TD, 18>);
         apply_transform_kernel<TG, TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TG*>(gtrans), static_cast<const TS*>(src), static_cast<TD*>(dst), G, mu_begin, mu_end);
+    }
     return cudaGetLastError();
 }
 
@@ -673,6 +694,7 @@ __global__ void philox_kernel(int n, const uint32_t* __restrict__ ctr, const uin
 
 cudaError_t launch_philox(int n, const uint32_t* ctr, const uint32_t* key, uint32_t* out, cudaStream_t st)
 {
+    uniform_carveout(philox_kernel);
     philox_kernel<<<(n + 127) / 128, 128, 0, st>>>(n, ctr, key, out);
     return cudaGetLastError();
 }

@@ -41,6 +41,21 @@ struct ReduceTail {
     double scale0, scale1;  // normalisations applied to the two sums on the device
 };
 
+// All kernels of the library ask for the same shared-memory carveout (a hint).  The pack / unpack kernels need a few
+// KB of shared memory per block, the sweep kernels none; blocks of kernels with different carveouts do not share an
+// SM, so with several lattices in flight (one stream each) a conversion kernel would otherwise force SMs to drain and
+// switch configuration in the middle of the other lattices' sweeps.
+constexpr int kCarveoutPercent = 25;
+template <typename Kernel>
+inline void uniform_carveout(Kernel kernel)
+{
+    static bool done = false;          // per kernel instantiation; a benign race at worst sets it twice
+    if (!done) {
+        cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, kCarveoutPercent);
+        done = true;
+    }
+}
+
 // every launcher returns cudaGetLastError() after the launch
 // solver_f64: with fp32 storage, accumulate K(x) and run the SU(2) solves in fp64 registers
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);

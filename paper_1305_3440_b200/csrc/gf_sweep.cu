@@ -254,13 +254,21 @@ __global__ void __launch_bounds__(GF_CAP_MAXT, GF_CAP_MINB) sweep_kernel_cap(con
 template <typename T, typename TK, int RECON, int L, int MODE>
 static void launch_kernel(uint32_t grid, int block, cudaStream_t st, const SweepConsts<T, TK>& P)
 {
-    if constexpr (UseR128<T, RECON, L>::value)
+    if constexpr (UseR128<T, RECON, L>::value) {
+        uniform_carveout(sweep_kernel_r128<T, TK, RECON, L, MODE>);
         sweep_kernel_r128<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
-    else if constexpr (sizeof(T) == 8 && RECON == 12 && L == GF_CAP_L) {
-        if (block <= GF_CAP_MAXT) sweep_kernel_cap<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
-        else sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
-    } else
+    } else if constexpr (sizeof(T) == 8 && RECON == 12 && L == GF_CAP_L) {
+        if (block <= GF_CAP_MAXT) {
+            uniform_carveout(sweep_kernel_cap<T, TK, RECON, L, MODE>);
+            sweep_kernel_cap<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+        } else {
+            uniform_carveout(sweep_kernel<T, TK, RECON, L, MODE>);
+            sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+        }
+    } else {
+        uniform_carveout(sweep_kernel<T, TK, RECON, L, MODE>);
         sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+    }
 }
 
 template <typename T, typename TK, int RECON, int L>
