@@ -78,7 +78,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
@@ -251,6 +251,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
         return out
 
+    U64_host = U64.cpu().numpy() if (rank == 0 and world == 1 and not args.no_cpu_baseline) else None
     main = bench_variant(args.variant, args.steps, args.warmup, True)
     variants = {}
     if not args.no_variants:
@@ -292,9 +293,13 @@ def run_ours(args):
             del fld
             torch.cuda.empty_cache()
 
+    others = None
+    if args.all_configs and world == 1:
+        others = other_configs(gf, gi, torch, dev)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(U64.cpu().numpy(), budget_s=12.0)
+        cpu = cpu_baseline(U64_host, budget_s=12.0)
 
     if rank == 0:
         pkey, recon, _ = VARIANTS[args.variant]
@@ -310,10 +315,97 @@ def run_ours(args):
             "gflops_nominal": main["value"] * FLOP_PER_SITE_UPDATE / 1e9,
             "gpu_launches": main["gpu_launches"], "clocks": main["clocks"], "e2e": main["e2e"],
             "roofline": main["roofline"], "cpu_baseline": cpu, "variants": variants, "fix_until_theta_1e-12": fixes,
+            "other_configs": others,
             "final_F": main["final_F"], "final_theta": main["final_theta"],
         }
         print(json.dumps(line), flush=True)
     rep.close()
+
+
+def other_configs(gf, gi, torch, dev):
+    """BASELINE.json's other workloads at full size (context for BASELINE.md section 4; parity for them is in tests/):
+    configs[1] 16^4, configs[3] 64^4 (omega 1.8, 200 iterations, F / theta every 10), configs[4] 32^3 x 64 Coulomb
+    gauge with stochastic relaxation (iteration rate, and gf_fix_until to max theta_t < 1e-12 with the Coulomb
+    options of DESIGN.md section 12), and the per-time-slice times Tab. 1 of the paper lists."""
+    out = {}
+
+    def timed(fn):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        r = fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b), r
+
+    def fixed_iterations(fld, prec, n, omega, check):
+        for k in range(n // check):
+            fld.iterate(check, gf.GF_OVERRELAX, omega, 0.0, prec)
+            fld.measure_async(prec, k % 16)
+            if k % 16 == 15 or k == n // check - 1:
+                last = [fld.measure_collect(j % 16) for j in range(k - k % 16, k + 1)][-1]
+        return last
+
+    for name, dims, eps, omega, n in (("configs[1] 16^4", (16, 16, 16, 16), 0.5, 1.7, 500),
+                                      ("configs[3] 64^4", (64, 64, 64, 64), 0.6, 1.8, 200)):
+        vol = dims[0] * dims[1] * dims[2] * dims[3]
+        U = gi.torch_smooth_random_gauge(dims, eps, SEED, device=dev)
+        for pkey, prec, cd in (("f32", gf.GF_F32, torch.complex64), ("f64", gf.GF_F64, torch.complex128)):
+            Uc = U.to(cd).contiguous() if pkey == "f32" else U
+            for recon in (18, 12):
+                fld = gf.GaugeField(dims, recon=recon, precisions=(pkey,), device=dev)
+                fld.pack(Uc, prec)
+                fixed_iterations(fld, prec, 20, omega, 10)
+                fld.pack(Uc, prec)
+                ms, (F, th) = timed(lambda: fixed_iterations(fld, prec, n, omega, 10))
+                B = 8 if pkey == "f64" else 4
+                out["%s %s-%d" % (name, pkey, recon)] = {
+                    "iterations": n, "theta_F_every": 10, "seconds": ms * 1e-3, "site_updates_per_s": vol * n / (ms * 1e-3),
+                    "algorithmic_GBs": vol * n * 16 * recon * B / (ms * 1e-3) / 1e9, "final_F": F[0], "final_theta": th[0]}
+                fld.close()
+                del fld
+            del Uc
+        del U
+        torch.cuda.empty_cache()
+
+    dims = (64, 32, 32, 32)
+    vol = 64 * 32 ** 3
+    U = gi.torch_smooth_random_gauge(dims, EPS, SEED, device=dev)
+    for recon in (18, 12):
+        for defer, freeze in ((0, 0), (1, 0), (1, 1)):
+            fld = gf.GaugeField(dims, gauge=gf.GF_COULOMB, recon=recon, precisions=("f64",), seed=2013, device=dev)
+            fld.attach_transform(("f64",) if defer else ())
+            fld.pack(U, gf.GF_F64)
+            fld.set_coulomb_mode(defer, freeze)
+            fld.iterate(5, gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64)
+            ms_it, _ = timed(lambda: fld.iterate(50, gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64))
+            fld.pack(U, gf.GF_F64)
+            gf.gf_set_rng(fld.ctx, 2013, 0)
+            ms, (rc, it, th) = timed(lambda: fld.fix_until(gf.GF_STOCHASTIC, 1.0, 0.8, gf.GF_F64, 1e-12, 100000, 20))
+            out["configs[4] 32^3x64 Coulomb stochastic p=0.8 f64-%d defer_temporal=%d freeze_slices=%d" % (recon, defer, freeze)] = {
+                "site_updates_per_s": vol * 50 / (ms_it * 1e-3), "ms_per_iteration": ms_it / 50,
+                "fix_converged": rc == gf.GF_OK, "fix_iterations": it, "fix_max_theta_t": th, "fix_seconds": ms * 1e-3}
+            fld.close()
+            del fld
+    del U
+    torch.cuda.empty_cache()
+
+    tab1 = {}
+    for ns, nt in ((16, 64), (32, 32), (64, 8), (128, 4)):
+        dims = (nt, ns, ns, ns)
+        U = gi.torch_hot_links(dims, 3, device=dev)
+        for pkey, prec, cd in (("f32", gf.GF_F32, torch.complex64), ("f64", gf.GF_F64, torch.complex128)):
+            fld = gf.GaugeField(dims, precisions=(pkey,), device=dev)
+            fld.pack(U.to(cd).contiguous(), prec)
+            n = max(5, int(2e9 / (nt * ns ** 3) / 3))
+            fld.iterate(3, gf.GF_OVERRELAX, OMEGA, 0.0, prec)
+            ms, _ = timed(lambda: fld.iterate(n, gf.GF_OVERRELAX, OMEGA, 0.0, prec))
+            tab1["Ns=%d Nt=%d %s-18" % (ns, nt, pkey)] = {"ms_per_time_slice_both_parities": ms / n / nt}
+            fld.close()
+            del fld
+        del U
+        torch.cuda.empty_cache()
+    out["PAPER.md Tab. 1 'kernel' column re-measured"] = tab1
+    return out
 
 
 def cpu_baseline(U, budget_s):
@@ -387,6 +479,8 @@ def main():
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-fix", action="store_true", help="skip the time-to-solution runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="also time BASELINE.json configs[1], [3], [4] and the Tab. 1 slice sizes (adds about two minutes)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

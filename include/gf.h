@@ -193,7 +193,10 @@ int gf_apply_transform(gf_ctx* ctx, int g_precision, int src_precision, int dst_
  *
  * gf_set_slice_mask: explicit control for gf_sweep: host_active[t] != 0 means the sites of slice t
  * are visited (N_t bytes, HOST pointer, copied before returning); NULL = all slices.  gf_fix_until
- * with freeze_slices manages the mask itself and leaves it off.
+ * with freeze_slices manages the mask itself and leaves it off.  The library turns the mask into the
+ * list of active slices and a half-sweep is launched over the sites of those slices only, so slices
+ * that converge at different times cost nothing once frozen (the time of a half-sweep is proportional
+ * to the number of active slices); with no active slice nothing is launched.
  * While a deferred update is outstanding the transformation buffer of that precision holds the only copy of
  * what still has to be applied to U_0: gf_transform_identity, gf_transform_pack, gf_transform_cast INTO it and
  * gf_set_transform replacing it return GF_ESTATE until gf_coulomb_finish (or a call that finishes implicitly)

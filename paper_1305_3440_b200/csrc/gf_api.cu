@@ -35,9 +35,11 @@ struct gf_ctx {
     int defer_temporal;         // Coulomb: sweeps record G(x) and leave the temporal links to gf_coulomb_finish
     int freeze_slices;          // Coulomb: gf_fix_until stops sweeping slices whose theta_t is below the target
     int pending[2];             // deferred temporal update outstanding for the field of that precision
-    uint8_t* dev_mask;          // workspace: one byte per time slice, 0 = frozen
-    uint8_t* host_mask;         // pinned copy
-    int mask_on;                // the sweeps consult dev_mask
+    uint16_t* dev_list;         // workspace: the time slices still being swept (ascending)
+    uint16_t* host_list;        // pinned staging copy of it
+    uint8_t* host_mask;         // one byte per time slice, 0 = frozen: what the list is built from
+    int n_active;               // entries of the list
+    int mask_on;                // the sweeps cover the listed slices only
     double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
     // slab decomposition along t (gf_set_slab): this context holds N_t local slices of a lattice nranks times as long
     int slab_rank, slab_n;
@@ -143,8 +145,8 @@ extern "C" size_t gf_workspace_bytes(const int dims[4])
 {
     if (!dims_ok(dims)) return 0;
     const MeasureGrid mg = measure_grid(dims);
-    // + the slice mask + the counter of the last reduction stage
-    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt + 16;
+    // + the list of active slices + the counter of the last reduction stage
+    return ((size_t)dims[0] * 2 * mg.bpp * 2 + (size_t)dims[0] * 2) * sizeof(double) + kMaxNt * sizeof(uint16_t) + 16;
 }
 
 extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void* dev_links_f64,
@@ -181,8 +183,8 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->mg = measure_grid(dims);
     c->partials = c->workspace;
     c->slice_tmp = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
-    c->dev_mask = reinterpret_cast<uint8_t*>(c->slice_tmp + (size_t)dims[0] * 2);
-    c->reduce_counter = reinterpret_cast<uint32_t*>(c->dev_mask + kMaxNt);
+    c->dev_list = reinterpret_cast<uint16_t*>(c->slice_tmp + (size_t)dims[0] * 2);
+    c->reduce_counter = reinterpret_cast<uint32_t*>(c->dev_list + kMaxNt);
 
     Geom& G = c->G;
     G.nt = dims[0];
@@ -200,6 +202,8 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     G.div_nxh = make_fastdiv(G.nxh);
     G.div_ny = make_fastdiv(G.ny);
     G.div_nz = make_fastdiv(G.nz);
+    G.sh = G.Vh / G.nt;
+    G.div_sh = make_fastdiv(G.sh);
 
     // 0 = automatic (default_tuning below); gf_set_tuning overrides
     c->lanes[PREC_F32] = c->lanes[PREC_F64] = 0;
@@ -215,12 +219,13 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
         delete c;
         return GF_ECUDA;
     }
-    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt + 16) != cudaSuccess) {
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_pinned), sizeof(double) * 2 * kMaxNt + kMaxNt * (1 + sizeof(uint16_t)) + 16) != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return GF_ENOMEM;
     }
-    c->host_mask = reinterpret_cast<uint8_t*>(c->host_pinned + 2 * kMaxNt);
+    c->host_list = reinterpret_cast<uint16_t*>(c->host_pinned + 2 * kMaxNt);
+    c->host_mask = reinterpret_cast<uint8_t*>(c->host_list + kMaxNt);
     for (int k = 0; k < kAsyncSlots; ++k) c->slot_precision[k] = -1;
     if (cudaMallocHost(reinterpret_cast<void**>(&c->host_slots), sizeof(double) * 2 * dims[0] * kAsyncSlots) != cudaSuccess ||
         cudaHostGetDevicePointer(reinterpret_cast<void**>(&c->slots_dev), c->host_slots, 0) != cudaSuccess) {
@@ -435,8 +440,21 @@ static int check_algo(gf_ctx* ctx, int algo, double omega, double p)
 // Launch configuration chosen by measurement on B200 at 32^4 (profiles/r1_tune_32x32x32x32.txt, profiles/r2_tune_f64_12.txt,
 // DESIGN.md "Kernels"): two lanes per site everywhere except fp64 / 12-real, where one lane per site (no redundant
 // solve, third rows never held in registers) is the variant that stays bandwidth-bound under the power cap.
-static void default_tuning(int precision, int recon, int solver_f64, int accumulate, int defer, int* lanes, int* block)
+static void default_tuning(int precision, int recon, int solver_f64, int accumulate, int defer, uint32_t Vh, int* lanes, int* block)
 {
+    // Lattices of less than one wave of blocks are bound by the latency of a single site update, not by bandwidth: more
+    // lanes per site shorten it (8^4: 9.2 instead of 12.3 us per fp64 / 12-real iteration; 16^4 fp32 / 12-real: 12.3
+    // instead of 16.4 us with two lanes).
+    if (Vh <= 4096u) {
+        *lanes = 4;
+        *block = 64;
+        return;
+    }
+    if (Vh <= 65536u && precision == GF_F32 && recon == GF_RECON12 && !solver_f64 && !defer) {
+        *lanes = 2;
+        *block = 64;
+        return;
+    }
     if (defer && precision == GF_F32) {      // 6 links + G: one lane per site is balanced and fits the registers
         *lanes = 1;
         *block = 64;
@@ -468,7 +486,8 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.links = ctx->links[precision];
     a.gtrans = ctx->gtrans[precision];
     a.defer_temporal = ctx->defer_temporal;
-    a.slice_active = ctx->mask_on ? ctx->dev_mask : nullptr;
+    a.slice_list = ctx->mask_on ? ctx->dev_list : nullptr;
+    a.n_listed = (uint32_t)ctx->n_active;
     a.prev_links = ctx->prev_links[precision];
     a.site_offset = (uint32_t)((uint64_t)ctx->slab_rank * ctx->V);
     a.G = ctx->G;
@@ -483,9 +502,13 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.reverse = ctx->zigzag ? (uint32_t)(ctx->sweeps & 1u) : 0u;
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
     int lanes, block;
-    default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, a.gtrans != nullptr && a.defer_temporal, &lanes, &block);
+    default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, a.gtrans != nullptr && a.defer_temporal, ctx->G.Vh, &lanes, &block);
     if (ctx->lanes[precision]) lanes = ctx->lanes[precision];
     if (ctx->block[precision]) block = ctx->block[precision];
+    if (a.slice_list && a.n_listed == 0) {   // every slice frozen: the half-sweep is empty, the Philox counter still advances
+        ctx->counter += 1;
+        return GF_OK;
+    }
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_sweep(precision, solver_f64, ctx->recon, lanes, block, a, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_sweep launch");
@@ -966,10 +989,16 @@ extern "C" int gf_set_coulomb_mode(gf_ctx* ctx, int defer_temporal, int freeze_s
     return GF_OK;
 }
 
-// uploads ctx->host_mask (pinned) to the device; the copy is ordered on the stream between the sweeps
+// Turns ctx->host_mask into the ascending list of active slices and uploads it; the copy is ordered on the stream
+// between the sweeps.  The callers have drained the stream, so the pinned staging copy is not in flight.
 static int upload_mask(gf_ctx* ctx)
 {
-    cudaError_t e = cudaMemcpyAsync(ctx->dev_mask, ctx->host_mask, (size_t)ctx->dims[0], cudaMemcpyHostToDevice, ctx->stream);
+    int n = 0;
+    for (int t = 0; t < ctx->dims[0]; ++t)
+        if (ctx->host_mask[t]) ctx->host_list[n++] = (uint16_t)t;
+    ctx->n_active = n;
+    if (n == 0) return GF_OK;
+    cudaError_t e = cudaMemcpyAsync(ctx->dev_list, ctx->host_list, (size_t)n * sizeof(uint16_t), cudaMemcpyHostToDevice, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "slice mask copy");
     return GF_OK;
 }

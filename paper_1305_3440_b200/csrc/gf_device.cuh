@@ -44,6 +44,8 @@ struct Geom {
     uint32_t stride[4];         // distance in h of one step in mu (mu=1: unused)
     uint32_t extent[4];         // N_mu
     FastDiv div_nxh, div_ny, div_nz;
+    uint32_t sh;                // sites per time slice per parity = Vh / Nt
+    FastDiv div_sh;
 };
 
 struct Site {

@@ -14,7 +14,8 @@ struct SweepArgs {
     void* links;            // internal field of the chosen precision
     void* gtrans;           // accumulated transformation of the same precision, or NULL
     int defer_temporal;     // Coulomb: with gtrans, leave the temporal links to gf_coulomb_finish
-    const uint8_t* slice_active;   // per time slice, 0 = frozen; NULL = all active
+    const uint16_t* slice_list;    // Coulomb slice freezing: the time slices still being swept, ascending; NULL = all
+    uint32_t n_listed;             // entries of slice_list
     void* prev_links;       // slab below (same precision and layout), or NULL = this field (periodic)
     uint32_t site_offset;   // global site index of the slab's first site
     Geom G;

@@ -20,7 +20,8 @@ namespace gf {
 template <typename T, typename TK> struct SweepConsts {
     T* links;
     T* gtrans;              // MODE > 0: the accumulated transformation G[parity][chunk][h], else unused
-    const uint8_t* slice_active;   // Coulomb slice freezing: sites of slices with 0 are skipped; NULL = all active
+    const uint16_t* slice_list;    // Coulomb slice freezing: the launch covers only the listed time slices; NULL = all
+    uint32_t n_sites;              // sites of the active parity the launch covers: Vh, or entries of slice_list x G.sh
     T* prev_links;          // slab decomposition in t: field holding U_0(x-0) of the sites with local t = 0 (the rank
                             // below; this rank's own field when there is one slab, which is the periodic wrap)
     uint32_t site_offset;   // global index of this slab's first site (Philox counter word 0)
@@ -77,16 +78,18 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     const uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
     const uint32_t parity = P.parity, counter = P.counter;
     const uint32_t warp = (bid * blockDim.x + threadIdx.x) >> 5;
-    if (warp * S >= G.Vh) return;                       // warp-uniform
+    if (warp * S >= P.n_sites) return;                  // warp-uniform
     uint32_t h = warp * S + (lane % S);
     const int j = lane / S;
-    bool live = h < G.Vh;
-    if (!live) h = G.Vh - 1u;                           // keeps the lane in the shuffles; no store
-    const Site s = decode_site(G, h, parity);
-    if (P.slice_active != nullptr) {                    // warp-uniform branch
-        live = live && P.slice_active[s.c[0]] != 0;
-        if (!__any_sync(0xffffffffu, live)) return;     // the whole warp sits in frozen slices
+    const bool live = h < P.n_sites;
+    if (!live) h = P.n_sites - 1u;                      // keeps the lane in the shuffles; no store
+    if (P.slice_list != nullptr) {
+        // frozen time slices (reading A17b) are not part of the launch at all: the grid covers the listed slices only,
+        // position i of the list standing for slice slice_list[i]
+        const uint32_t i = fdiv(h, G.div_sh);
+        h = (uint32_t)P.slice_list[i] * G.sh + (h - i * G.sh);
     }
+    const Site s = decode_site(G, h, parity);
 
     if (MODE == MODE_ACC && j == 0) {
         // G(x) is only needed after the links have been written back: start moving it towards L2 now
@@ -96,25 +99,29 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
         for (int c = 0; c < CH; ++c) asm volatile("prefetch.global.L2 [%0];" ::"l"(gp + (size_t)c * Tile<T>::W * 16));
     }
 
-    // a2: gather this lane's links
+    // a2: gather this lane's links.  MODE_DEFER: the temporal links stay where they are; the lane that owns mu = 0
+    // carries G(x) in that register slot instead (loaded up front with the links; mu = 0 does not enter K in Coulomb
+    // gauge, mu0 = 1) and has no backward link there.  The lanes of a warp run the same instruction stream -- G(x) is
+    // a forward link read from another base pointer, the missing backward link a masked-off load and product -- so
+    // with two or four lanes per site the warp issues no more than the plain kernel does.
     T Uf[ND][18], Ub[ND][18];
     uint32_t hb[ND];
+    T* const gblock = MODE == MODE_PLAIN ? nullptr : P.gtrans + (size_t)parity * RECON * padded_vh<T>(G);
+    const bool gslot = MODE == MODE_DEFER && j == 0;
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
         hb[d] = backward_index(G, s, mu);
-        if (MODE == MODE_DEFER && d == 0 && j == 0) {
-            // mu = 0: the temporal links stay where they are; their register slot carries G(x) instead,
-            // loaded up front with the links (mu = 0 does not enter K in Coulomb gauge: mu0 = 1)
-            load_link<RECON>(P.gtrans + (size_t)parity * RECON * padded_vh<T>(G), h, Uf[d]);
+        const bool is_g = d == 0 && gslot;
+        load_link<RECON>(is_g ? gblock : P.links + block_offset<T>(parity, mu, RECON, G), h, Uf[d]);
+        if (is_g) {
 #pragma unroll
             for (int k = 0; k < 18; ++k) Ub[d][k] = T(0);
-            continue;
+        } else {
+            // the temporal link below the first local time slice belongs to the slab below
+            const T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
+            load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[d], Ub[d]);
         }
-        load_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G), h, Uf[d]);
-        // the temporal link below the first local time slice belongs to the slab below
-        const T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        load_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[d], Ub[d]);
     }
     // 12-real storage.  LAZY12: the third rows are never kept: they are formed for K(x) and dropped, and formed
     // again for the forward links in step a6 (U g^dagger does not need the third row of U at all) -- 24 flops per
@@ -189,13 +196,7 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
 #pragma unroll
     for (int d = 0; d < ND; ++d) {
         const int mu = j * ND + d;
-        if (MODE == MODE_DEFER && d == 0 && j == 0) {   // G(x) <- g(x) G(x)
-            T out[18];
-            if (LAZY12) reconstruct_row2(Uf[d]);
-            mul_g_U<ROWS>(g, Uf[d], out);
-            store_link<RECON>(P.gtrans + (size_t)parity * RECON * padded_vh<T>(G), h, out);
-            continue;
-        }
+        const bool is_g = d == 0 && gslot;              // this slot holds G(x): G(x) <- g(x) G(x), no backward link
         T out[18];
         if (LAZY12) {                                   // the third row of the forward link again, not merged with a3's
             forget(GF_RE(Uf[d], 0, 1));
@@ -203,13 +204,15 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
             reconstruct_row2(Uf[d]);
         }
         mul_g_U<ROWS>(g, Uf[d], out);
-        store_link<RECON>(P.links + block_offset<T>(parity, mu, RECON, G), h, out);
-        mul_U_gdag<ROWS>(Ub[d], g, out);
-        T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
-        store_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[d], out);
+        store_link<RECON>(is_g ? gblock : P.links + block_offset<T>(parity, mu, RECON, G), h, out);
+        if (!is_g) {
+            mul_U_gdag<ROWS>(Ub[d], g, out);
+            T* back = (mu == 0 && s.c[0] == 0) ? P.prev_links : P.links;
+            store_link<RECON>(back + block_offset<T>(parity ^ 1u, mu, RECON, G), hb[d], out);
+        }
     }
     if (MODE == MODE_ACC && j == 0) {
-        T* blk = P.gtrans + (size_t)parity * RECON * padded_vh<T>(G);
+        T* blk = gblock;
         T Gt[18], out[18];
         load_link<RECON>(blk, h, Gt);
         if (RECON == 12) reconstruct_row2(Gt);
@@ -277,7 +280,8 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     SweepConsts<T, TK> P;
     P.links = static_cast<T*>(a.links);
     P.gtrans = static_cast<T*>(a.gtrans);
-    P.slice_active = a.slice_active;
+    P.slice_list = a.slice_list;
+    P.n_sites = a.slice_list ? a.n_listed * a.G.sh : a.G.Vh;
     P.prev_links = a.prev_links ? static_cast<T*>(a.prev_links) : P.links;
     P.site_offset = a.site_offset;
     P.G = a.G;
@@ -290,7 +294,8 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     P.key1 = a.key1;
     P.counter = a.counter;
     P.reverse = a.reverse;
-    const uint64_t threads = (uint64_t)a.G.Vh * L;
+    if (P.n_sites == 0) return cudaSuccess;             // every slice frozen: nothing to launch
+    const uint64_t threads = (uint64_t)P.n_sites * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);
     if (a.gtrans && a.defer_temporal)
         launch_kernel<T, TK, RECON, L, MODE_DEFER>(grid, block, st, P);

@@ -148,6 +148,84 @@ def test_fix_until_with_freezing_matches_oracle(cuda_device, defer):
     fld.close()
 
 
+def mixed_smoothness_field(dims, seed):
+    """Time slices of very different smoothness (eps 0.05 ... 0.6), hence very different convergence times in Coulomb
+    gauge: slice t of the input is slice t of one of four seeded smooth fields.  Any SU(3) link field is a valid input."""
+    fields = [gi.smooth_random_gauge(dims, eps, seed + k) for k, eps in enumerate((0.05, 0.2, 0.4, 0.6))]
+    U = np.empty_like(fields[0])
+    for t in range(dims[0]):
+        U[t] = fields[(t * 7 + t // 3) % 4][t]
+    return U
+
+
+@pytest.mark.parametrize("defer", [False, True])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_slices_converging_at_different_times(cuda_device, defer, recon):
+    """NEXT-2, "batching slices with different convergence": with freeze_slices the half-sweeps cover the list of
+    still-active slices only.  On an input whose slices converge at very different iterations the run stops at the
+    oracle's iteration, every slice on the oracle's (frozen) trajectory."""
+    dims = (12, 6, 4, 6)
+    U = mixed_smoothness_field(dims, 40)
+    Uo = U.copy()
+    it_o, th_o, frozen_at, conv = oracle.fix_until_freeze(Uo, dims, algo=oracle.OVERRELAX, omega=1.5, theta_target=1e-12,
+                                                          max_iter=5000, check_every=5)
+    assert conv and frozen_at.max() > 2 * frozen_at.min() and len(set(frozen_at.tolist())) >= 4    # really staggered
+    fld = coulomb_field(dims, "f64", cuda_device, recon=recon)
+    fld.pack(to_device(U, "f64", cuda_device), gf.GF_F64)
+    fld.set_coulomb_mode(defer_temporal=defer, freeze_slices=True)
+    launches0 = gf.gf_launch_count(fld.ctx)
+    rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.5, 0.0, gf.GF_F64, 1e-12, 5000, 5)
+    assert rc == gf.GF_OK and th < 1e-12 and abs(it - it_o) <= 5
+    got = fld.unpack(gf.GF_F64, torch.complex128).cpu().numpy()
+    if it == it_o:
+        assert np.abs(got[..., 1:, :, :] - Uo[..., 1:, :, :]).max() < 1e-10
+    assert oracle.theta(np.ascontiguousarray(got), dims, oracle.COULOMB).max() < 1.1e-12
+    assert abs(oracle.plaquette(np.ascontiguousarray(got), dims) - oracle.plaquette(U, dims)) < 1e-12
+    fld.close()
+
+
+def test_all_slices_frozen_launches_nothing_and_keeps_the_philox_counter(cuda_device):
+    dims = (4, 4, 4, 4)
+    U = gi.smooth_random_gauge(dims, 0.5, 3)
+    fld = coulomb_field(dims, "f64", cuda_device, seed=9, transform=False)
+    fld.pack(to_device(U, "f64", cuda_device), gf.GF_F64)
+    fld.set_slice_mask([0, 0, 0, 0])
+    n0 = gf.gf_launch_count(fld.ctx)
+    fld.iterate(2, gf.GF_STOCHASTIC, 1.0, 0.5, gf.GF_F64)
+    assert gf.gf_launch_count(fld.ctx) == n0 and gf.gf_get_counter(fld.ctx) == 4
+    assert np.array_equal(fld.unpack(gf.GF_F64, torch.complex128).cpu().numpy(), U)
+    fld.set_slice_mask([0, 0, 1, 0])                       # one slice, the last position of a one-entry list
+    fld.sweep(0, gf.GF_STOCHASTIC, 1.0, 0.5, gf.GF_F64)
+    Uo = U.copy()
+    oracle.sweep_masked(Uo, dims, 0, [0, 0, 1, 0], algo=oracle.STOCHASTIC, p=0.5, seed=9, half_sweep_counter=4)
+    assert np.abs(fld.unpack(gf.GF_F64, torch.complex128).cpu().numpy() - Uo).max() < 1e-12
+    fld.close()
+
+
+def test_half_sweep_time_follows_the_number_of_active_slices(cuda_device):
+    """configs[4] size: with 4 of 64 slices active a half-sweep costs a small fraction of the full one (the launch covers
+    the listed slices only; a byte mask consulted by every warp of a full grid took 0.12 of the full time)."""
+    dims = (64, 32, 32, 32)
+    fld = coulomb_field(dims, "f64", cuda_device, transform=False)
+    fld.pack(gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device), gf.GF_F64)
+
+    def ms(mask, n=20):
+        fld.set_slice_mask(mask)
+        fld.iterate(3, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fld.iterate(n, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    full = ms(None)
+    few = ms([1 if t % 16 == 5 else 0 for t in range(64)])
+    print("32^3 x 64 fp64: %.4f ms per iteration with 64 active slices, %.4f ms with 4" % (full, few))
+    assert few < 0.09 * full                                # 4 / 64 = 0.0625 of the sites
+    fld.close()
+
+
 def test_coulomb_mode_errors(cuda_device):
     dims = (4, 4, 4, 4)
     B = gf.binding.lib
