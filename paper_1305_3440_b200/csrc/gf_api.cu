@@ -125,6 +125,8 @@ static MeasureGrid measure_grid(const int dims[4])
     mg.Sh = (uint32_t)((uint64_t)dims[1] * dims[2] * dims[3] / 2);
     mg.block = kMeasureBlock;
     mg.bpp = (mg.Sh + mg.block - 1) / mg.block;
+    mg.slice_list = nullptr;
+    mg.n_listed = 0;
     return mg;
 }
 
@@ -591,11 +593,19 @@ static int sync_and_check(gf_ctx* ctx, const char* what)
 }
 
 // Runs the measurement kernels and leaves F and theta (Coulomb: per slice, interleaved) in ctx->host_pinned.
-static int measure_to_host(gf_ctx* ctx, int precision)
+// active_only (the fix loop with slice freezing): only the slices still being swept are measured; the frozen ones keep
+// the F_t, theta_t of their last evaluation in host_pinned -- nothing that enters them has changed since.
+static int measure_to_host(gf_ctx* ctx, int precision, bool active_only = false)
 {
     const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
+    MeasureGrid mg = ctx->mg;
+    if (active_only && ctx->mask_on && ctx->gauge == GF_COULOMB) {
+        if (ctx->n_active == 0) return GF_OK;
+        mg.slice_list = ctx->dev_list;
+        mg.n_listed = (uint32_t)ctx->n_active;
+    }
     GF_SLAB_BEGIN(ctx);
-    cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0, ctx->mg,
+    cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0, mg,
                                    ctx->partials, measure_tail(ctx), ctx->slice_out, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "measure launch");
     GF_SLAB_END(ctx);
@@ -700,7 +710,7 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
             if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         }
         it += n;
-        int e = measure_to_host(ctx, precision);
+        int e = measure_to_host(ctx, precision, freeze);
         if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         *theta_out = finish_measure(ctx, nullptr, nullptr);
         if (*theta_out < target) { rc = GF_OK; break; }

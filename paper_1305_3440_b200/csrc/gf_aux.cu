@@ -57,11 +57,13 @@ __device__ __forceinline__ void block_reduce2(double a, double b, double* out)
 
 template <typename Op>
 __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32_t per_slice, const ReduceTail tail,
-                                     double* __restrict__ out)
+                                     double* __restrict__ out, const uint16_t* __restrict__ slice_list)
 {
     __shared__ double res[2];
     __shared__ uint32_t last;
-    const double* p = partials + (size_t)blockIdx.x * per_slice * 2;
+    // block -> time slice; with a list (per-slice results only, tail.combine == 0) the listed slices
+    const uint32_t slice = slice_list ? slice_list[blockIdx.x] : blockIdx.x;
+    const double* p = partials + (size_t)slice * per_slice * 2;
     double a = 0.0, b = 0.0;
     for (uint32_t i = threadIdx.x; i < per_slice; i += blockDim.x) {
         a = Op::apply(a, p[2 * i]);
@@ -70,8 +72,8 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
     block_reduce2<Op>(a, b, res);
     if (!tail.combine) {
         if (threadIdx.x == 0) {
-            out[2 * blockIdx.x] = res[0] * tail.scale0;
-            out[2 * blockIdx.x + 1] = res[1] * tail.scale1;
+            out[2 * slice] = res[0] * tail.scale0;
+            out[2 * slice + 1] = res[1] * tail.scale1;
         }
         return;
     }
@@ -98,20 +100,26 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
     }
 }
 
-// thread -> (slice t, parity, site) of the measurement grids: blockIdx.y = t, blockIdx.x = 2*chunk + parity
+// blockIdx.y -> time slice: all of them, or the listed ones (Coulomb slice freezing: frozen slices keep their results)
+__device__ __forceinline__ uint32_t measure_slice(const MeasureGrid& mg)
+{
+    return mg.slice_list ? mg.slice_list[blockIdx.y] : blockIdx.y;
+}
+
+// thread -> (slice t, parity, site) of the measurement grids: blockIdx.y -> t, blockIdx.x = 2*chunk + parity
 __device__ __forceinline__ bool measure_site(const Geom& G, const MeasureGrid& mg, uint32_t& parity, Site& s)
 {
     parity = blockIdx.x & 1u;
     const uint32_t i = (blockIdx.x >> 1) * blockDim.x + threadIdx.x;
     const bool live = i < mg.Sh;
-    const uint32_t h = blockIdx.y * mg.Sh + (live ? i : mg.Sh - 1u);
+    const uint32_t h = measure_slice(mg) * mg.Sh + (live ? i : mg.Sh - 1u);
     s = decode_site(G, h, parity);
     return live;
 }
 
 __device__ __forceinline__ size_t partial_slot(const MeasureGrid& mg)
 {
-    return ((size_t)blockIdx.y * (2u * mg.bpp) + blockIdx.x) * 2;
+    return ((size_t)measure_slice(mg) * (2u * mg.bpp) + blockIdx.x) * 2;
 }
 
 // a7 + a8: per-block partial sums of  sum_mu Re tr U_mu(x)  and  tr[Delta(x) Delta(x)^dagger].
@@ -265,7 +273,7 @@ static cudaError_t dispatch(int precision, int recon, Args... args)
     return recon == 12 ? Launcher<float, 12>::run(args...) : Launcher<float, 18>::run(args...);
 }
 
-static dim3 measure_dims(const Geom& G, const MeasureGrid& mg) { return dim3(2u * mg.bpp, G.nt, 1); }
+static dim3 measure_dims(const Geom& G, const MeasureGrid& mg) { return dim3(2u * mg.bpp, mg.slice_list ? mg.n_listed : G.nt, 1); }
 
 template <typename T, int RECON> struct MeasureLauncher {
     static cudaError_t run(const void* links, const void* prev_links, const Geom& G, int mu0, const MeasureGrid& mg, double* partials,
@@ -275,7 +283,7 @@ template <typename T, int RECON> struct MeasureLauncher {
         measure_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
                                                                            static_cast<const T*>(prev_links ? prev_links : links), G, mu0, mg, partials);
         uniform_carveout(reduce_slices_kernel<OpSum>);
-        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
+        reduce_slices_kernel<OpSum><<<measure_dims(G, mg).y, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out, mg.slice_list);
         return cudaGetLastError();
     }
 };
@@ -288,7 +296,7 @@ template <typename T, int RECON> struct PlaquetteLauncher {
         plaquette_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links),
                                                                              static_cast<const T*>(next_links ? next_links : links), G, mg, partials);
         uniform_carveout(reduce_slices_kernel<OpSum>);
-        reduce_slices_kernel<OpSum><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
+        reduce_slices_kernel<OpSum><<<measure_dims(G, mg).y, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out, mg.slice_list);
         return cudaGetLastError();
     }
 };
@@ -300,7 +308,7 @@ template <typename T, int RECON> struct UnitarityLauncher {
         uniform_carveout(unitarity_kernel<T, RECON>);
         unitarity_kernel<T, RECON><<<measure_dims(G, mg), mg.block, 0, st>>>(static_cast<const T*>(links), G, mg, partials);
         uniform_carveout(reduce_slices_kernel<OpMax>);
-        reduce_slices_kernel<OpMax><<<G.nt, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out);
+        reduce_slices_kernel<OpMax><<<measure_dims(G, mg).y, 256, 0, st>>>(partials, 2u * mg.bpp, tail, slice_out, mg.slice_list);
         return cudaGetLastError();
     }
 };

@@ -32,6 +32,8 @@ struct MeasureGrid {
     uint32_t Sh;            // sites per time slice per parity
     uint32_t bpp;           // blocks per (slice, parity)
     uint32_t block;         // threads per block
+    const uint16_t* slice_list;   // measure only these time slices (the others keep their previous results); NULL = all
+    uint32_t n_listed;
 };
 
 // last stage of a reduction (gf_aux.cu, reduce_slices_kernel)

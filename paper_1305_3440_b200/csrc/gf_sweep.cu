@@ -50,6 +50,11 @@ __device__ __forceinline__ T shfl_xor_T(T v, int mask)
 // traffic; U_0(x) <- G(x) U_0(x) G(x+0)^dagger is applied once at the end (gf_coulomb_finish).
 enum { MODE_PLAIN = 0, MODE_ACC = 1, MODE_DEFER = 2 };
 
+// 1: half-sweeps are launched with programmatic stream serialisation (see sweep_body); 0: plain stream order
+#ifndef GF_PDL
+#define GF_PDL 1
+#endif
+
 // bit L set: the L-lanes-per-site kernel of that storage type is "lazy".  Measured at 32^4 (sustained runs under the
 // power cap, profiles/r2_tune_f64_12.txt): fp64 with one or two lanes per site goes from 226 to 166 registers (L = 2) and
 // from 81 % to 100 % of the HBM peak; with four lanes it changes nothing.
@@ -75,6 +80,12 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     // Alternate half-sweeps walk the lattice in opposite directions (blocks are dispatched in
     // ascending blockIdx order): the launch starts on the sites the previous one finished with,
     // whose links are still in the 126 MB L2.  The result does not depend on the order.
+#if GF_PDL
+    // Programmatic dependent launch: the next half-sweep of the stream may be scheduled onto SMs as the blocks of this
+    // one drain; its blocks wait below, before their first access to global memory, until this grid has completed and
+    // its stores are visible.  What overlaps is launch latency and block start-up, never two half-sweeps' accesses.
+    asm volatile("griddepcontrol.launch_dependents;");
+#endif
     const uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
     const uint32_t parity = P.parity, counter = P.counter;
     const uint32_t warp = (bid * blockDim.x + threadIdx.x) >> 5;
@@ -83,6 +94,9 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     const int j = lane / S;
     const bool live = h < P.n_sites;
     if (!live) h = P.n_sites - 1u;                      // keeps the lane in the shuffles; no store
+#if GF_PDL
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
     if (P.slice_list != nullptr) {
         // frozen time slices (reading A17b) are not part of the launch at all: the grid covers the listed slices only,
         // position i of the list standing for slice slice_list[i]
@@ -254,23 +268,35 @@ __global__ void __launch_bounds__(GF_CAP_MAXT, GF_CAP_MINB) sweep_kernel_cap(con
     sweep_body<T, TK, RECON, L, MODE>(P);
 }
 
+template <typename Kernel, typename Consts>
+static void launch_pdl(Kernel kernel, uint32_t grid, int block, cudaStream_t st, const Consts& P)
+{
+    uniform_carveout(kernel);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3((unsigned)block, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = GF_PDL;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, P);
+}
+
 template <typename T, typename TK, int RECON, int L, int MODE>
 static void launch_kernel(uint32_t grid, int block, cudaStream_t st, const SweepConsts<T, TK>& P)
 {
     if constexpr (UseR128<T, RECON, L>::value) {
-        uniform_carveout(sweep_kernel_r128<T, TK, RECON, L, MODE>);
-        sweep_kernel_r128<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+        launch_pdl(sweep_kernel_r128<T, TK, RECON, L, MODE>, grid, block, st, P);
     } else if constexpr (sizeof(T) == 8 && RECON == 12 && L == GF_CAP_L) {
-        if (block <= GF_CAP_MAXT) {
-            uniform_carveout(sweep_kernel_cap<T, TK, RECON, L, MODE>);
-            sweep_kernel_cap<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
-        } else {
-            uniform_carveout(sweep_kernel<T, TK, RECON, L, MODE>);
-            sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
-        }
+        if (block <= GF_CAP_MAXT)
+            launch_pdl(sweep_kernel_cap<T, TK, RECON, L, MODE>, grid, block, st, P);
+        else
+            launch_pdl(sweep_kernel<T, TK, RECON, L, MODE>, grid, block, st, P);
     } else {
-        uniform_carveout(sweep_kernel<T, TK, RECON, L, MODE>);
-        sweep_kernel<T, TK, RECON, L, MODE><<<grid, block, 0, st>>>(P);
+        launch_pdl(sweep_kernel<T, TK, RECON, L, MODE>, grid, block, st, P);
     }
 }
 
