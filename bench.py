@@ -46,15 +46,18 @@ TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.json")
 def ncu_traffic(variant):
     """dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 32^4 from the committed `ncu --set full`
     summary (written by paper_1305_3440_b200/profile_traffic.py; command in profiles/r2_sweep_variants_ncu.md).
-    Valid only for the kernel sources it was captured at: returns (None, why) when they have changed since."""
+    Valid only for the kernel sources it was captured at: returns (None, why, None) when they have changed since.
+    Third value: the same sum from the single-pass capture of consecutive launches without ncu's L2 flush, if on record."""
     try:
         from paper_1305_3440_b200.build import source_hash
         doc = json.load(open(TRAFFIC_FILE))
         if doc.get("source_hash") != source_hash():
-            return None, "profiles/r2_traffic.json was captured at sources %s, the library is at %s" % (doc.get("source_hash"), source_hash())
-        return float(doc["variants"][variant]["traffic_bytes"]), "profiles/r2_traffic.json (ncu --set full, sources %s)" % doc["source_hash"]
+            return None, "profiles/r2_traffic.json was captured at sources %s, the library is at %s" % (doc.get("source_hash"), source_hash()), None
+        v = doc["variants"][variant]
+        warm = v.get("in_run", {}).get("traffic_bytes")
+        return float(v["traffic_bytes"]), "profiles/r2_traffic.json (ncu --set full, sources %s)" % doc["source_hash"], warm
     except Exception as e:                                      # missing file or variant: no claim
-        return None, "no ncu capture on record (%s)" % type(e).__name__
+        return None, "no ncu capture on record (%s)" % type(e).__name__, None
 
 
 def measured_peaks():
@@ -73,12 +76,17 @@ class ClockSampler:
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.first = index, [], None, 0
+
+    def mark(self):
+        """The timed region starts here: only rows sampled from now on are reported (nvidia-smi is started
+        earlier, during the warm-up, because it takes a few hundred ms to deliver its first row)."""
+        self.first = len(self.rows)
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
@@ -92,10 +100,11 @@ class ClockSampler:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        rows = self.rows[self.first:] or self.rows[-1:]
+        sm = [float(r[0]) for r in rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in self.rows)]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i] == "Active" for r in rows)]
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": reasons, "samples": len(sm)}
 
@@ -144,12 +153,13 @@ def run_ours(args):
                     history = [fld.measure_collect(j % 16) for j in range(k - k % 16, k + 1)]
             return history
 
+        sampler = ClockSampler(local_rank)
+        sampler.start()
         for _ in range(warmup):
             step(False)
         launches0 = gf.gf_launch_count(fld.ctx)
-        sampler = ClockSampler(local_rank)
         barrier()
-        sampler.start()
+        sampler.mark()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         for _ in range(steps):
@@ -163,7 +173,7 @@ def run_ours(args):
         kern_ms = sum(a.elapsed_time(b) for a, b in sweep_ms) / (len(sweep_ms) * 2 * args.check)
         bytes_per_launch = (V // 2) * 16 * recon * B
         achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
-        traffic, traffic_src = ncu_traffic(name)
+        traffic, traffic_src, traffic_warm = ncu_traffic(name)
         out = {
             "value": world * V * args.iters * steps / (ms_total * 1e-3),
             "ms_per_step": ms_total / steps,
@@ -176,6 +186,10 @@ def run_ours(args):
                          "traffic": traffic, "traffic_source": traffic_src,
                          "dram_achieved": (traffic / (kern_ms * 1e-3) / 1e9) if traffic else None,
                          "dram_frac": (traffic / (kern_ms * 1e-3) / 1e9 / peak) if traffic else None,
+                         # ncu flushes the L2 before a profiled launch; traffic_in_run is a single-pass capture of
+                         # consecutive launches without the flush: what crosses the DRAM interface inside a step
+                         "traffic_in_run": traffic_warm,
+                         "dram_frac_in_run": (traffic_warm / (kern_ms * 1e-3) / 1e9 / peak) if traffic_warm else None,
                          "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
                          "bytes_per_launch": bytes_per_launch, "avg_launch_ms": kern_ms, "peak_source": peak_src,
                          "frac_of_8TBs_nominal": achieved / 8000.0},

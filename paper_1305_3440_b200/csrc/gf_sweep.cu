@@ -256,18 +256,6 @@ template <typename T, int RECON, int L> struct UseR128 {
     static constexpr bool value = sizeof(T) == 4 && RECON == 18 && L == 2;
 };
 
-// exploration hook: a register cap for one (fp64, 12-real, L) variant, chosen at compile time
-#ifndef GF_CAP_L
-#define GF_CAP_L 0
-#define GF_CAP_MAXT 64
-#define GF_CAP_MINB 1
-#endif
-template <typename T, typename TK, int RECON, int L, int MODE>
-__global__ void __launch_bounds__(GF_CAP_MAXT, GF_CAP_MINB) sweep_kernel_cap(const SweepConsts<T, TK> P)
-{
-    sweep_body<T, TK, RECON, L, MODE>(P);
-}
-
 template <typename Kernel, typename Consts>
 static void launch_pdl(Kernel kernel, uint32_t grid, int block, cudaStream_t st, const Consts& P)
 {
@@ -290,11 +278,6 @@ static void launch_kernel(uint32_t grid, int block, cudaStream_t st, const Sweep
 {
     if constexpr (UseR128<T, RECON, L>::value) {
         launch_pdl(sweep_kernel_r128<T, TK, RECON, L, MODE>, grid, block, st, P);
-    } else if constexpr (sizeof(T) == 8 && RECON == 12 && L == GF_CAP_L) {
-        if (block <= GF_CAP_MAXT)
-            launch_pdl(sweep_kernel_cap<T, TK, RECON, L, MODE>, grid, block, st, P);
-        else
-            launch_pdl(sweep_kernel<T, TK, RECON, L, MODE>, grid, block, st, P);
     } else {
         launch_pdl(sweep_kernel<T, TK, RECON, L, MODE>, grid, block, st, P);
     }

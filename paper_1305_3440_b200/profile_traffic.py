@@ -1,8 +1,12 @@
 """Reads `ncu --set full` captures of the sweep kernels and writes the per-launch DRAM traffic bench.py reports.
 
     python -m paper_1305_3440_b200.profile_traffic OUT.json NAME=REPORT.ncu-rep [NAME=REPORT.ncu-rep ...]
+    (REPORT may also be the .csv written by `ncu -i REPORT.ncu-rep --page raw --csv`)
 
-NAME is a bench.py variant (f64-18, f64-12, f32-18, f32-12).  For every report the launches whose kernel name
+NAME is a bench.py variant (f64-18, f64-12, f32-18, f32-12); NAME@run marks a single-pass capture of consecutive
+launches taken with ``--cache-control none`` and only the DRAM byte and duration metrics (no replay, no L2 flush:
+the traffic of a launch as it runs inside a step, with the L2 reuse between consecutive half-sweeps), stored under
+the variant's "in_run" key.  For every report the launches whose kernel name
 contains "sweep" are read with `ncu -i REPORT --page raw --csv` (works without a GPU) and
 dram__bytes_read.sum + dram__bytes_write.sum, gpu__time_duration.sum and a few evidence counters are averaged
 over them.  The JSON records the hash of the kernel sources (build.source_hash) the library had when this
@@ -35,7 +39,10 @@ SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "us": 1.0, "ms":
 
 
 def read_report(path, pattern="sweep"):
-    out = subprocess.run([NCU, "-i", path, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    if path.endswith(".csv"):               # already exported with `ncu -i REPORT --page raw --csv > path`
+        out = open(path).read()
+    else:
+        out = subprocess.run([NCU, "-i", path, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
     rows = list(csv.reader(io.StringIO(out)))
     header, units, data = rows[0], rows[1], rows[2:]
     col = {name: i for i, name in enumerate(header)}
@@ -58,9 +65,12 @@ def main(argv):
         raise SystemExit(__doc__)
     doc = {"source_hash": source_hash(), "how": "ncu --set full --clock-control none, averaged over the captured sweep launches "
            "(see the .md beside this file for the command)", "variants": {}}
-    for a in argv[2:]:
+    for a in sorted(argv[2:], key=lambda a: "@run" in a):
         name, path = a.split("=", 1)
-        doc["variants"][name] = read_report(path)
+        if name.endswith("@run"):
+            doc["variants"].setdefault(name[:-4], {})["in_run"] = read_report(path)
+        else:
+            doc["variants"][name] = read_report(path)
     json.dump(doc, open(argv[1], "w"), indent=1, sort_keys=True)
     print(json.dumps(doc, indent=1, sort_keys=True))
 
