@@ -196,70 +196,57 @@ def run_ours(args):
             "final_F": F[0], "final_theta": th[0],
         }
         if with_e2e:
-            # End to end through the public API with HOST buffers.  Two lattices are in flight, each with
-            # its own context, CUDA stream, pinned host buffer and host thread (the library calls release
-            # the GIL): while one lattice sweeps, the other's fixed field goes device->host and its next
-            # input host->device, so PCIe transfers overlap the kernels as in a production pipeline.  Every
-            # step still copies its whole input from pinned host memory and its whole result back.
-            extra = []
-            for _ in range(args.e2e_lanes - 1):
-                with torch.cuda.stream(torch.cuda.Stream(device=dev)):
-                    extra.append(gf.GaugeField(DIMS, recon=recon, precisions=(pkey,), device=dev, staging=True))
-            lanes = [(f, torch.empty(fld.shape, dtype=cdtype).pin_memory()) for f in [fld] + extra]
+            # End to end through the public API with HOST buffers (paper_1305_3440_b200.pipeline.HostPipeline): a few
+            # lattices are in flight, each with its own context, CUDA stream, staging buffer and host thread (the library
+            # calls release the GIL): while one lattice sweeps, another's fixed field goes device->host and its next
+            # input host->device, so the PCIe transfers overlap the kernels; the sweep phases take turns on the GPU.
+            # Every step still copies its whole input from pinned host memory and its whole result back.
+            from paper_1305_3440_b200.pipeline import HostPipeline
+            pipe = HostPipeline(DIMS, recon=recon, precisions=(pkey,), lanes=args.e2e_lanes, device=dev,
+                                gate=bool(args.e2e_gate), first_field=fld)
+            bufs = [torch.empty(fld.shape, dtype=cdtype).pin_memory() for _ in pipe.fields]
             sys.setswitchinterval(1e-4)                 # the worker threads hand the GIL over quickly
-            for _, host in lanes:
-                host.copy_(Uc)
 
-            def e2e_step(f, host):
-                f.load_host(host, prec)
+            def enqueue(f):                             # one step's sweeps and reductions; nothing here waits for the GPU
                 for k in range(n_blocks):
                     f.iterate(args.check, gf.GF_OVERRELAX, OMEGA, 0.0, prec)
                     f.measure_async(prec, k % 16)
-                    if k % 16 == 15 or k == n_blocks - 1:
-                        for j in range(k - k % 16, k + 1):
-                            f.measure_collect(j % 16)
-                f.store_host(host, prec)                # synchronises its stream: the fixed field is on the host
+                    if k % 16 == 15 and k != n_blocks - 1:
+                        [f.measure_collect(j) for j in range(16)]
 
-            def worker(f, host, n):
-                torch.cuda.set_device(dev)
-                for _ in range(n):
-                    e2e_step(f, host)
+            def collect(f):
+                return [f.measure_collect(j % 16) for j in range(n_blocks - 1 - (n_blocks - 1) % 16, n_blocks)]
 
-            def run_pipeline(n_steps, use=None):
-                use = lanes if use is None else use
-                counts = [n_steps // len(use) + (1 if i < n_steps % len(use) else 0) for i in range(len(use))]
-                threads = [threading.Thread(target=worker, args=(f, h, c)) for (f, h), c in zip(use, counts) if c]
-                for t in threads:
-                    t.start()
-                for t in threads:
-                    t.join()
-                torch.cuda.synchronize()
+            def run_pipeline(n_steps, lanes=None):
+                for h in bufs:
+                    h.copy_(Uc)
+                n = len(bufs) if lanes is None else lanes
+                barrier()
+                t0 = time.perf_counter()
+                pipe.process([bufs[i % n] for i in range(n_steps)], enqueue, prec, collect=collect, lanes=lanes)
+                return max_over_ranks(time.perf_counter() - t0)
 
-            run_pipeline(len(lanes) * max(1, warmup // 2))
-            for _, host in lanes:
-                host.copy_(Uc)
-            barrier()
-            t0 = time.perf_counter()
-            run_pipeline(steps)
-            dt = max_over_ranks(time.perf_counter() - t0)
+            run_pipeline(len(bufs) * max(1, warmup // 2))
+            dt = run_pipeline(steps)
+            steady = pipe.steady_seconds_per_item()
+            steady = max_over_ranks(steady) if steady else None
             # the same step with ONE lattice in flight: nothing overlaps the copies -- the latency a single caller sees
-            run_pipeline(1, lanes[:1])
+            run_pipeline(1, 1)
             n_single = max(2, steps // 3)
-            barrier()
-            t0 = time.perf_counter()
-            run_pipeline(n_single, lanes[:1])
-            dt_single = max_over_ranks(time.perf_counter() - t0)
-            nbytes = lanes[0][1].numel() * lanes[0][1].element_size()
+            dt_single = run_pipeline(n_single, 1)
+            nbytes = bufs[0].numel() * bufs[0].element_size()
             out["e2e"] = {"value": world * V * args.iters * steps / dt, "unit": "site-updates/s",
                           "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 16 * n_blocks,
                           "ms_per_step": 1e3 * dt / steps,
+                          "steady_ms_per_step": 1e3 * steady if steady else None,
                           "single_lattice_ms_per_step": 1e3 * dt_single / n_single,
                           "single_lattice_value": world * V * args.iters * n_single / dt_single,
-                          "pipeline": "%d lattices in flight (one context, stream, pinned buffer and host thread each): "
-                                      "copies overlap sweeps" % len(lanes)}
-            for f in extra:
-                f.close()
-            del lanes, extra
+                          "pipeline": "%d lattices in flight (one context, stream, pinned buffer and host thread each): copies "
+                                      "overlap sweeps%s; value and ms_per_step are wall clock over all K steps including the "
+                                      "pipeline's fill and drain, steady_ms_per_step is the time per step between the first and "
+                                      "the last completed step" % (len(bufs), ", sweep phases take turns" if args.e2e_gate else "")}
+            pipe.close()
+            del pipe, bufs
         fld.close()
         del fld, Uc
         torch.cuda.empty_cache()
@@ -490,6 +477,7 @@ def main():
     ap.add_argument("--iters", type=int, default=100, help="iterations per step")
     ap.add_argument("--check", type=int, default=10, help="F/theta reduction every CHECK iterations")
     ap.add_argument("--e2e-lanes", type=int, default=4, help="lattices in flight in the end-to-end pipeline")
+    ap.add_argument("--e2e-gate", type=int, default=1, help="1: the sweep phases of the lattices in flight take turns on the GPU")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-fix", action="store_true", help="skip the time-to-solution runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")

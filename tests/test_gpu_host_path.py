@@ -78,3 +78,60 @@ def test_pipelined_lattices_do_not_disturb_each_other(cuda_device):
         assert torch.equal(o, w)
     for f in fields:
         f.close()
+
+
+@pytest.mark.parametrize("gate", [True, False])
+def test_host_pipeline_ensemble_matches_lone_runs_and_the_oracle(cuda_device, gate):
+    """HostPipeline (the form bench.py's e2e leg uses): seven configurations in host memory through three lanes;
+    every fixed field is bitwise the one a lone GaugeField produces, the iteration counts are the same, and one
+    of them is followed by the oracle (same count within one check interval, F and theta to 1e-10)."""
+    from paper_1305_3440_b200.pipeline import HostPipeline
+    dims = (4, 6, 4, 8)
+    inputs = [torch.from_numpy(gi.smooth_random_gauge(dims, 0.4, 900 + i)) for i in range(7)]
+
+    def work(f):
+        return f.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64, 1e-12, 4000, 5)
+
+    want, want_res = [], []
+    lone = gf.GaugeField(dims, precisions=("f64",), device=cuda_device, staging=True)
+    for h in inputs:
+        b = h.clone().pin_memory()
+        lone.load_host(b, gf.GF_F64)
+        want_res.append(work(lone))
+        lone.store_host(b, gf.GF_F64)
+        want.append(b.clone())
+    lone.close()
+
+    pipe = HostPipeline(dims, precisions=("f64",), lanes=3, device=cuda_device, gate=gate)
+    bufs = [h.clone().pin_memory() for h in inputs]
+    res = pipe.process(bufs, work, gf.GF_F64)
+    assert len(pipe.done_at) == 7 and pipe.steady_seconds_per_item() > 0
+    for b, w, r, wr in zip(bufs, want, res, want_res):
+        assert torch.equal(b, w)
+        assert r[0] == gf.GF_OK and r[1] == wr[1] and r[2] == wr[2]
+    # a second batch through the same lanes (fewer items than lanes)
+    bufs2 = [h.clone().pin_memory() for h in inputs[:2]]
+    pipe.process(bufs2, work, gf.GF_F64)
+    assert torch.equal(bufs2[0], want[0]) and torch.equal(bufs2[1], want[1])
+    pipe.close()
+
+    Uo = np.ascontiguousarray(inputs[3].numpy())
+    it, th, conv = oracle.fix_until(Uo, dims, algo=oracle.OVERRELAX, omega=1.7, theta_target=1e-12, max_iter=4000, check_every=5)
+    assert conv
+    assert abs(it - res[3][1]) <= 5
+    got = np.ascontiguousarray(bufs[3].numpy())
+    assert oracle.theta(got, dims) < 1e-12                       # fixed, as judged by the oracle
+    assert abs(oracle.plaquette(got, dims) - oracle.plaquette(np.ascontiguousarray(inputs[3].numpy()), dims)) < 1e-12
+    if it == res[3][1]:
+        assert abs(oracle.functional(got, dims) / oracle.functional(Uo, dims) - 1) < 1e-10
+        assert np.abs(got - Uo).max() < 1e-9
+
+
+def test_host_pipeline_surfaces_errors(cuda_device):
+    from paper_1305_3440_b200.pipeline import HostPipeline
+    dims = (4, 4, 4, 4)
+    pipe = HostPipeline(dims, precisions=("f64",), lanes=2, device=cuda_device)
+    bufs = [torch.from_numpy(gi.smooth_random_gauge(dims, 0.4, 5)).pin_memory() for _ in range(3)]
+    with pytest.raises(gf.GFError):
+        pipe.process(bufs, lambda f: f.iterate(1, gf.GF_OVERRELAX, 2.5, 0.0, gf.GF_F64), gf.GF_F64)   # omega out of range
+    pipe.close()
