@@ -406,6 +406,27 @@ def other_configs(gf, gi, torch, dev):
         del U
         torch.cuda.empty_cache()
     out["PAPER.md Tab. 1 'kernel' column re-measured"] = tab1
+
+    # the per-GPU lattices of the paper's weak-scaling figure (Fig. 3): 64^3 x 32 and 48^4
+    fig3 = {}
+    for dims in ((32, 64, 64, 64), (48, 48, 48, 48)):
+        vol = dims[0] * dims[1] * dims[2] * dims[3]
+        U = gi.torch_smooth_random_gauge(dims, EPS, SEED, device=dev)
+        for pkey, prec, cd, B in (("f32", gf.GF_F32, torch.complex64, 4), ("f64", gf.GF_F64, torch.complex128, 8)):
+            for recon in (18, 12):
+                fld = gf.GaugeField(dims, recon=recon, precisions=(pkey,), device=dev)
+                fld.pack(U.to(cd).contiguous(), prec)
+                n = max(20, int(4e9 / vol))
+                fld.iterate(5, gf.GF_OVERRELAX, OMEGA, 0.0, prec)
+                ms, _ = timed(lambda: fld.iterate(n, gf.GF_OVERRELAX, OMEGA, 0.0, prec))
+                fig3["%dx%d^3 %s-%d" % (dims[0], dims[1], pkey, recon)] = {
+                    "site_updates_per_s": vol * n / (ms * 1e-3), "gflops_nominal": vol * n * FLOP_PER_SITE_UPDATE / (ms * 1e-3) / 1e9,
+                    "algorithmic_GBs": vol * n * 16 * recon * B / (ms * 1e-3) / 1e9}
+                fld.close()
+                del fld
+        del U
+        torch.cuda.empty_cache()
+    out["PAPER.md Fig. 3 per-GPU lattices, overrelaxation sweeps only"] = fig3
     return out
 
 

@@ -261,3 +261,30 @@ def test_32_4_as_two_slabs_equals_the_undivided_lattice(cuda_device):
     assert torch.equal(got, want)                     # same kernels, same order of operations per site: bitwise
     assert abs(F[0] - Fw[0]) < 1e-13 and abs(th[0] / thw[0] - 1) < 1e-12
     lat.close()
+
+
+# ------------------------------------------------------------------------------ the paper's own per-GPU lattices
+
+@pytest.mark.parametrize("dims,prec,recon", [((48, 48, 48, 48), "f64", 18), ((48, 48, 48, 48), "f32", 12),
+                                             ((32, 64, 64, 64), "f64", 12), ((32, 64, 64, 64), "f32", 18)])
+def test_fig3_lattices_sampled_against_oracle(cuda_device, dims, prec, recon):
+    """48^4 and 64^3 x 32, the per-GPU lattices of the paper's weak-scaling figure: extents that are
+    not powers of two at a size of several GB, default launch configuration.  One iteration with sampled sites
+    recomputed by the oracle, then invariants after 20 more."""
+    U = gi.torch_smooth_random_gauge(dims, 0.6, 48, device=cuda_device).to(CDTYPE[prec])
+    fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
+    fld.pack(U, PREC[prec])
+    del U
+    torch.cuda.empty_cache()
+    P0 = fld.plaquette(PREC[prec])
+    F0, th0 = fld.measure(PREC[prec])
+    rng = np.random.default_rng(dims[0] + recon)
+    sampled_sweep_check(fld, dims, prec, gf.GF_LANDAU, oracle.LANDAU, gf.GF_OVERRELAX, oracle.OVERRELAX, 1.7, 0.0, 0, 24, rng)
+    torch.cuda.empty_cache()
+    fld.iterate(20, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
+    F1, th1 = fld.measure(PREC[prec])
+    assert F1[0] > F0[0] and th1[0] < th0[0]
+    assert abs(fld.plaquette(PREC[prec]) - P0) < (1e-12 if prec == "f64" else 1e-5)
+    du, dd = fld.unitarity(PREC[prec])
+    assert du < (1e-12 if prec == "f64" else 1e-4) and dd < (1e-12 if prec == "f64" else 1e-4)
+    fld.close()
