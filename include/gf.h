@@ -280,6 +280,17 @@ int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff);
  * The links produced are bitwise the same (sites of one parity are independent). */
 int gf_set_traversal(gf_ctx* ctx, int zigzag);
 
+/* How gf_fix_until follows theta ("iterated until the requested gauge precision theta has
+ * been reached").  blocks = 0: after every evaluation the host waits for theta before it enqueues the
+ * next check_every iterations.  blocks = 1..8 (default 4): up to that many blocks of {iterations;
+ * F / theta reduction} are enqueued ahead of the one whose result the host waits for; the last
+ * reduction kernel compares theta (Coulomb gauge: every theta_t) with theta_target on the device and,
+ * once it is below, the half-sweeps already enqueued behind it leave the field alone.  Links,
+ * iteration count, theta and the Philox stream are exactly those of blocks = 0; the GPU never idles
+ * for a host round trip.  With Coulomb slice freezing (gf_set_coulomb_mode) the loop always waits,
+ * because the list of active slices changes between evaluations.  Errors: GF_EINVAL. */
+int gf_set_fix_runahead(gf_ctx* ctx, int blocks);
+
 /* Arithmetic of the per-site solver when the STORAGE is fp32 (gf_sweep with GF_F32): K(x) is
  * accumulated and the three SU(2) solves run in solver_precision: GF_F32 (everything in fp32),
  * GF_F64 (fp64 registers: no extra memory traffic, ~15 % more time, removes the amplification of

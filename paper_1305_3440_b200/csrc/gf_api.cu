@@ -25,6 +25,7 @@ namespace {
 constexpr int kMeasureBlock = 128;
 constexpr int kMaxNt = 4096;
 constexpr int kAsyncSlots = 16;
+constexpr int kRunAhead = 8;          // most evaluation blocks the fix loop keeps enqueued ahead of the one it reads
 }
 
 struct gf_ctx {
@@ -54,10 +55,14 @@ struct gf_ctx {
     double* partials;           // workspace: per-block partial sums
     double* slice_tmp;          // workspace: 2 doubles per time slice (reduce_slices_kernel, whole-lattice sums)
     uint32_t* reduce_counter;   // workspace: blocks of the last reduction stage that have finished (zero between launches)
+    uint32_t* stop_dev;         // workspace: zero except while a run-ahead fix loop has reached its target on the device
+    int runahead;               // evaluation blocks gf_fix_until keeps in flight (0 = wait for every theta before going on)
+    cudaEvent_t fix_events[8];  // one per block in flight
     double* slice_out;          // 2 doubles per time slice, written by the last reduction kernel: the DEVICE ADDRESS OF
                                 // host_pinned (zero-copy: the result is in host memory when the stream has drained)
     double* host_pinned;        // 2 * Nt doubles
-    double* host_slots;         // kAsyncSlots x 2 * Nt doubles (pinned): results of gf_measure_async
+    double* host_slots;         // (kAsyncSlots + kRunAhead) x 2 * Nt doubles (pinned): results of gf_measure_async, then
+                                // the ring the run-ahead fix loop reads its evaluations from
     double* slots_dev;          // device address of host_slots
     int slot_precision[16];     // precision measured into the slot, or -1 when empty
     cudaStream_t stream;
@@ -187,6 +192,8 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->slice_tmp = c->workspace + (size_t)dims[0] * 2 * c->mg.bpp * 2;
     c->dev_list = reinterpret_cast<uint16_t*>(c->slice_tmp + (size_t)dims[0] * 2);
     c->reduce_counter = reinterpret_cast<uint32_t*>(c->dev_list + kMaxNt);
+    c->stop_dev = c->reduce_counter + 1;                 // both zeroed below
+    c->runahead = 4;
 
     Geom& G = c->G;
     G.nt = dims[0];
@@ -229,7 +236,7 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
     c->host_list = reinterpret_cast<uint16_t*>(c->host_pinned + 2 * kMaxNt);
     c->host_mask = reinterpret_cast<uint8_t*>(c->host_list + kMaxNt);
     for (int k = 0; k < kAsyncSlots; ++k) c->slot_precision[k] = -1;
-    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_slots), sizeof(double) * 2 * dims[0] * kAsyncSlots) != cudaSuccess ||
+    if (cudaMallocHost(reinterpret_cast<void**>(&c->host_slots), sizeof(double) * 2 * dims[0] * (kAsyncSlots + kRunAhead)) != cudaSuccess ||
         cudaHostGetDevicePointer(reinterpret_cast<void**>(&c->slots_dev), c->host_slots, 0) != cudaSuccess) {
         cudaGetLastError();
         if (c->host_slots) cudaFreeHost(c->host_slots);
@@ -244,6 +251,15 @@ extern "C" int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int r
         delete c;
         return GF_ECUDA;
     }
+    for (int k = 0; k < kRunAhead; ++k)
+        if (cudaEventCreateWithFlags(&c->fix_events[k], cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            for (int j = 0; j < k; ++j) cudaEventDestroy(c->fix_events[j]);
+            cudaFreeHost(c->host_slots);
+            cudaFreeHost(c->host_pinned);
+            delete c;
+            return GF_ECUDA;
+        }
     *out = c;
     return GF_OK;
 }
@@ -252,6 +268,7 @@ extern "C" void gf_destroy(gf_ctx* ctx)
 {
     if (!ctx) return;
     DeviceGuard guard(ctx);
+    for (int k = 0; k < kRunAhead; ++k) cudaEventDestroy(ctx->fix_events[k]);
     if (ctx->host_pinned) cudaFreeHost(ctx->host_pinned);
     if (ctx->host_slots) cudaFreeHost(ctx->host_slots);
     delete ctx;
@@ -502,6 +519,7 @@ static int enqueue_sweep(gf_ctx* ctx, int parity, int algo, double omega, double
     a.key1 = (uint32_t)(ctx->seed >> 32);
     a.counter = ctx->counter;
     a.reverse = ctx->zigzag ? (uint32_t)(ctx->sweeps & 1u) : 0u;
+    a.stop = ctx->stop_dev;
     const int solver_f64 = ctx->solver_mode == GF_SOLVER_AUTO ? algo == GF_STOCHASTIC : ctx->solver_mode == GF_F64;
     int lanes, block;
     default_tuning(precision, ctx->recon, solver_f64, a.gtrans != nullptr, a.gtrans != nullptr && a.defer_temporal, ctx->G.Vh, &lanes, &block);
@@ -562,6 +580,8 @@ static ReduceTail measure_tail(const gf_ctx* ctx)
     ReduceTail t;
     t.slice_tmp = ctx->slice_tmp;
     t.counter = ctx->reduce_counter;
+    t.stop = nullptr;
+    t.target = 0.0;
     if (ctx->gauge == GF_COULOMB) {
         const double Vs = (double)(ctx->V / ctx->dims[0]);
         t.combine = 0;
@@ -582,6 +602,8 @@ static ReduceTail lattice_tail(const gf_ctx* ctx, double scale)
     t.counter = ctx->reduce_counter;
     t.combine = 1;
     t.scale0 = t.scale1 = scale;
+    t.stop = nullptr;
+    t.target = 0.0;
     return t;
 }
 
@@ -687,6 +709,64 @@ extern "C" int gf_theta(gf_ctx* ctx, int precision, double* host_out)
     return gf_measure(ctx, precision, nullptr, host_out);
 }
 
+// The fix loop without a host round trip per evaluation.  Blocks of {iterations up to the next evaluation; F / theta
+// reduction} are enqueued up to ctx->runahead ahead of the block whose result the host is waiting for.  The last
+// reduction kernel of a block compares theta with the target ON THE DEVICE (the same double, the same comparison the
+// host makes when it reads the value from pinned memory) and sets ctx->stop_dev; the half-sweeps already enqueued
+// behind it then leave the field alone.  The host reads the blocks in order, stops at the first one below the target
+// and rewinds its half-sweep counter to that block: field, iteration count and Philox stream are those of the loop
+// that waits for every theta (fix_phase below with runahead = 0).
+static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
+                              int check_every, int* it_io, double* theta_out)
+{
+    struct Block { int it_end; uint32_t counter_end; uint64_t sweeps_end; } meta[kRunAhead];
+    const int depth = ctx->runahead < kRunAhead ? ctx->runahead : kRunAhead;
+    const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
+    const size_t slot_len = (size_t)2 * ctx->dims[0];
+    int it_enq = *it_io, rc = GF_NOT_CONVERGED, err = GF_OK;
+    long head = 0, tail = 0;
+    ReduceTail rt = measure_tail(ctx);
+    rt.stop = ctx->stop_dev;
+    rt.target = target;
+    while (true) {
+        while (err == GF_OK && head - tail < depth && it_enq < max_iter) {
+            int n = check_every - (it_enq % check_every);
+            if (n > max_iter - it_enq) n = max_iter - it_enq;
+            for (int k = 0; k < n && err == GF_OK; ++k) err = enqueue_iteration(ctx, algo, omega, p, precision);
+            if (err != GF_OK) break;
+            it_enq += n;
+            const int s = (int)(head % depth);
+            cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0,
+                                           ctx->mg, ctx->partials, rt, ctx->slots_dev + (size_t)(kAsyncSlots + s) * slot_len, ctx->stream);
+            if (e == cudaSuccess) e = cudaEventRecord(ctx->fix_events[s], ctx->stream);
+            if (e != cudaSuccess) { err = cuda_fail(ctx, e, "fix loop"); break; }
+            ctx->launches += 2;
+            meta[s].it_end = it_enq;
+            meta[s].counter_end = ctx->counter;
+            meta[s].sweeps_end = ctx->sweeps;
+            ++head;
+        }
+        if (tail == head) break;                        // nothing in flight: max_iter reached (or an error before any block)
+        const int s = (int)(tail % depth);
+        cudaError_t e = cudaEventSynchronize(ctx->fix_events[s]);
+        if (e != cudaSuccess) { err = cuda_fail(ctx, e, "fix loop"); break; }
+        *theta_out = finish_measure(ctx, nullptr, nullptr, ctx->host_slots + (size_t)(kAsyncSlots + s) * slot_len);
+        *it_io = meta[s].it_end;
+        ++tail;
+        if (*theta_out < target) {
+            // the device took the same decision after this block: what is enqueued behind it is a no-op there
+            ctx->counter = meta[s].counter_end;
+            ctx->sweeps = meta[s].sweeps_end;
+            rc = GF_OK;
+            break;
+        }
+    }
+    // behind everything enqueued so far: later sweeps of this context act again
+    cudaError_t e = cudaMemsetAsync(ctx->stop_dev, 0, sizeof(uint32_t), ctx->stream);
+    if (e != cudaSuccess && err == GF_OK) err = cuda_fail(ctx, e, "fix loop");
+    return err != GF_OK ? err : rc;
+}
+
 // One phase of the fix loop in one precision.  Returns GF_OK when theta < target was seen.
 static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
                      int check_every, int* it_io, double* theta_out)
@@ -694,6 +774,8 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
     int it = *it_io;
     int rc = GF_NOT_CONVERGED;
     const bool freeze = ctx->freeze_slices && ctx->gauge == GF_COULOMB;
+    // slice freezing changes the launch list between evaluations on the host: that loop waits for every theta
+    if (!freeze && ctx->runahead > 0) return fix_phase_runahead(ctx, algo, omega, p, precision, target, max_iter, check_every, it_io, theta_out);
     if (freeze) {                            // every slice starts active (the stream is idle or ordered: pinned copy is free)
         cudaError_t e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "fix loop");
@@ -1111,6 +1193,14 @@ extern "C" int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff)
     if (!ctx) return GF_EINVAL;
     if (!(theta_handoff > 0.0)) return fail(ctx, GF_EINVAL, "the hand-off theta must be positive");
     ctx->handoff = theta_handoff;
+    return GF_OK;
+}
+
+extern "C" int gf_set_fix_runahead(gf_ctx* ctx, int blocks)
+{
+    if (!ctx) return GF_EINVAL;
+    if (blocks < 0 || blocks > kRunAhead) return fail(ctx, GF_EINVAL, "run-ahead must be 0..%d evaluation blocks", kRunAhead);
+    ctx->runahead = blocks;
     return GF_OK;
 }
 

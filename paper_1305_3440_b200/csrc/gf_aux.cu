@@ -75,6 +75,24 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
             out[2 * slice] = res[0] * tail.scale0;
             out[2 * slice + 1] = res[1] * tail.scale1;
         }
+        if (tail.stop == nullptr) return;
+        // run-ahead fix loop, Coulomb gauge: the block that finishes last decides max_t theta_t < target
+        if (threadIdx.x == 0) {
+            tail.slice_tmp[blockIdx.x] = res[1] * tail.scale1;
+            __threadfence();
+            last = atomicAdd(tail.counter, 1u) == gridDim.x - 1u ? 1u : 0u;
+        }
+        __syncthreads();
+        if (!last) return;
+        __threadfence();
+        a = b = 0.0;
+        for (uint32_t t = threadIdx.x; t < gridDim.x; t += blockDim.x) a = fmax(a, __ldcg(tail.slice_tmp + t));
+        __syncthreads();
+        block_reduce2<OpMax>(a, b, res);
+        if (threadIdx.x == 0) {
+            if (res[0] < tail.target) *tail.stop = 1u;
+            *tail.counter = 0u;
+        }
         return;
     }
     if (threadIdx.x == 0) {
@@ -94,8 +112,10 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
     __syncthreads();                                    // block_reduce2's scratch is reused
     block_reduce2<Op>(a, b, res);
     if (threadIdx.x == 0) {
+        const double th = res[1] * tail.scale1;
         out[0] = res[0] * tail.scale0;
-        out[1] = res[1] * tail.scale1;
+        out[1] = th;
+        if (tail.stop != nullptr && th < tail.target) *tail.stop = 1u;    // the value the host compares, same comparison
         *tail.counter = 0u;
     }
 }

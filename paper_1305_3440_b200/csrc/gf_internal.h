@@ -26,6 +26,8 @@ struct SweepArgs {
     uint32_t key0, key1;    // Philox key = seed
     uint32_t counter;       // half-sweep counter (Philox counter word 2)
     uint32_t reverse;       // traverse the lattice backwards (L2 reuse between consecutive launches)
+    const uint32_t* stop;   // device word, never NULL: non-zero = the run-ahead fix loop has reached its target on the
+                            // device and this half-sweep, enqueued before the host knew, must leave the field alone
 };
 
 struct MeasureGrid {
@@ -42,6 +44,8 @@ struct ReduceTail {
     uint32_t* counter;      // device word, zero between launches
     int combine;            // 0: one (scaled) pair per time slice; 1: one pair for the whole lattice in out[0], out[1]
     double scale0, scale1;  // normalisations applied to the two sums on the device
+    uint32_t* stop;         // run-ahead fix loop: set *stop = 1 when theta (Coulomb: every theta_t) < target; NULL = no decision
+    double target;
 };
 
 // All kernels of the library ask for the same shared-memory carveout (a hint).  The pack / unpack kernels need a few

@@ -32,6 +32,7 @@ template <typename T, typename TK> struct SweepConsts {
     double p;
     uint32_t key0, key1, counter;
     uint32_t reverse;       // 1: blocks walk the lattice from the last site to the first
+    const uint32_t* stop;   // see SweepArgs
 };
 
 template <typename T>
@@ -53,6 +54,12 @@ enum { MODE_PLAIN = 0, MODE_ACC = 1, MODE_DEFER = 2 };
 // 1: half-sweeps are launched with programmatic stream serialisation (see sweep_body); 0: plain stream order
 #ifndef GF_PDL
 #define GF_PDL 1
+#endif
+
+// 0: the half-sweeps ignore the stop word of the run-ahead fix loop (for A/B timing of the sweeps only: gf_fix_until
+// then needs gf_set_fix_runahead(ctx, 0))
+#ifndef GF_STOP_CHECK
+#define GF_STOP_CHECK 1
 #endif
 
 // bit L set: the L-lanes-per-site kernel of that storage type is "lazy".  Measured at 32^4 (sustained runs under the
@@ -96,6 +103,17 @@ __device__ __forceinline__ void sweep_body(const SweepConsts<T, TK>& P)
     if (!live) h = P.n_sites - 1u;                      // keeps the lane in the shuffles; no store
 #if GF_PDL
     asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+    // Run-ahead fix loop (gf_api.cu, fix_phase_runahead): the reduction that found theta below the target set this word;
+    // the half-sweeps that were already enqueued behind it do nothing.  The word was written by an earlier grid of the
+    // stream, which the wait above has awaited; after the first warp of an SM the load is an L1 hit.  Tested at once: a
+    // value held across the solve costs the one-lane fp32 / 12-real kernel 21 registers.
+#if GF_STOP_CHECK
+    {
+        uint32_t stopped;
+        asm volatile("ld.global.ca.u32 %0, [%1];" : "=r"(stopped) : "l"(P.stop) : "memory");
+        if (stopped != 0u) return;
+    }
 #endif
     if (P.slice_list != nullptr) {
         // frozen time slices (reading A17b) are not part of the launch at all: the grid covers the listed slices only,
@@ -303,6 +321,7 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     P.key1 = a.key1;
     P.counter = a.counter;
     P.reverse = a.reverse;
+    P.stop = a.stop;
     if (P.n_sites == 0) return cudaSuccess;             // every slice frozen: nothing to launch
     const uint64_t threads = (uint64_t)P.n_sites * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);

@@ -168,3 +168,6 @@ class GaugeField:
 
     def set_traversal(self, zigzag):
         B.gf_set_traversal(self.ctx, zigzag)
+
+    def set_fix_runahead(self, blocks):
+        B.gf_set_fix_runahead(self.ctx, blocks)

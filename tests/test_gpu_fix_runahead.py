@@ -1,0 +1,146 @@
+"""The fix loop without a host round trip per evaluation (gf_set_fix_runahead, include/gf.h): evaluation blocks
+are enqueued ahead, the reduction kernel takes the stopping decision on the device and the half-sweeps enqueued
+behind it leave the field alone.  Required: links, iteration count, theta and the Philox stream bitwise those of
+the loop that waits for every theta (run-ahead 0) -- which the other test files compare with the oracle -- and,
+directly, the oracle's iteration count and field."""
+import numpy as np
+import pytest
+import torch
+
+import gf_inputs as gi
+import oracle
+import paper_1305_3440_b200 as gf
+
+pytestmark = pytest.mark.gpu
+
+
+def run_fix(cuda_device, U, dims, runahead, *, gauge=gf.GF_LANDAU, algo=gf.GF_OVERRELAX, omega=1.7, p=0.0, mode=gf.GF_F64,
+            recon=18, target=1e-12, max_iter=3000, check_every=5, seed=7, defer=False, after=0):
+    """Returns (rc, iterations, theta, Philox counter after the call, launches, fixed fp field, [G])."""
+    mixed = mode in (gf.GF_MIXED, gf.GF_MIXED_EXACT)
+    precs = ("f64", "f32") if mixed else (("f64",) if mode == gf.GF_F64 else ("f32",))
+    fld = gf.GaugeField(dims, gauge=gauge, recon=recon, precisions=precs, seed=seed, device=cuda_device)
+    Ud = torch.from_numpy(U).to(cuda_device)
+    if mode in (gf.GF_F64, gf.GF_MIXED_EXACT):
+        fld.pack(Ud, gf.GF_F64)
+    if mode in (gf.GF_F32, gf.GF_MIXED):
+        fld.pack(Ud.to(torch.complex64), gf.GF_F32)
+    if mode == gf.GF_MIXED_EXACT:
+        fld.attach_transform(("f64", "f32"))
+    if defer:
+        fld.attach_transform(("f64",))
+        fld.set_coulomb_mode(True, False)
+    fld.set_fix_runahead(runahead)
+    n0 = gf.gf_launch_count(fld.ctx)
+    rc, it, th = fld.fix_until(algo, omega, p, mode, target, max_iter, check_every)
+    launches = gf.gf_launch_count(fld.ctx) - n0
+    counter = gf.gf_get_counter(fld.ctx)
+    out_prec = gf.GF_F32 if mode == gf.GF_F32 else gf.GF_F64
+    if after:            # the stop word is clear again: sweeps that follow the loop act on the field
+        fld.iterate(after, algo, omega, p, out_prec)
+    res = fld.unpack(out_prec, torch.complex128).cpu().numpy()
+    F, ths = fld.measure(out_prec)
+    fld.close()
+    return rc, it, th, counter, launches, res, ths
+
+
+@pytest.mark.parametrize("depth", [1, 4, 8])
+@pytest.mark.parametrize("mode,recon", [(gf.GF_F64, 18), (gf.GF_F64, 12), (gf.GF_F32, 18), (gf.GF_MIXED, 18), (gf.GF_MIXED_EXACT, 12)])
+def test_runahead_equals_the_waiting_loop_landau(cuda_device, depth, mode, recon):
+    dims = (6, 4, 8, 6)
+    U = gi.smooth_random_gauge(dims, 0.4, 314)
+    target = 1e-6 if mode == gf.GF_F32 else 1e-12
+    a = run_fix(cuda_device, U, dims, 0, mode=mode, recon=recon, target=target)
+    b = run_fix(cuda_device, U, dims, depth, mode=mode, recon=recon, target=target)
+    assert a[0] == b[0] == gf.GF_OK
+    assert a[1] == b[1] and a[2] == b[2] and a[3] == b[3]          # iterations, theta, Philox counter
+    assert np.array_equal(a[5], b[5])                                # the fixed field, bitwise
+    assert b[4] >= a[4]                                              # the blocks enqueued ahead were launched (and did nothing)
+
+
+@pytest.mark.parametrize("check_every,max_iter", [(1, 3000), (7, 3000), (10, 23), (4, 8), (5, 0)])
+def test_runahead_iteration_accounting(cuda_device, check_every, max_iter):
+    """Evaluation points (multiples of check_every and the last iteration), max_iter reached without convergence,
+    max_iter that is not a multiple of check_every, and sweeps after the loop (the stop word is clear again)."""
+    dims = (4, 6, 4, 4)
+    U = gi.smooth_random_gauge(dims, 0.4, 2718)
+    a = run_fix(cuda_device, U, dims, 0, check_every=check_every, max_iter=max_iter, after=2)
+    b = run_fix(cuda_device, U, dims, 4, check_every=check_every, max_iter=max_iter, after=2)
+    assert a[:4] == b[:4]
+    assert a[0] == (gf.GF_OK if max_iter == 3000 else gf.GF_NOT_CONVERGED)
+    assert np.array_equal(a[5], b[5]) and np.array_equal(a[6], b[6])
+    if max_iter == 3000:                                             # and the oracle agrees on where the loop stops
+        Uo = U.copy()
+        it, th, conv = oracle.fix_until(Uo, dims, algo=oracle.OVERRELAX, omega=1.7, theta_target=1e-12, max_iter=3000, check_every=check_every)
+        assert conv and abs(it - b[1]) <= check_every
+        if it == b[1]:
+            for _ in range(2):
+                for parity in (0, 1):
+                    oracle.sweep(Uo, dims, parity, algo=oracle.OVERRELAX, omega=1.7)
+            assert np.abs(b[5] - Uo).max() < 1e-9
+
+
+@pytest.mark.parametrize("defer", [False, True])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_runahead_coulomb_stochastic(cuda_device, defer, recon):
+    """Coulomb gauge: the device decides on max_t theta_t; the Philox stream (seed, half-sweep counter) must be where the
+    waiting loop leaves it, also with deferred temporal links.  The oracle's fix loop gives the iteration count."""
+    dims = (6, 6, 6, 6)
+    U = gi.smooth_random_gauge(dims, 0.4, 1618)
+    kw = dict(gauge=gf.GF_COULOMB, algo=gf.GF_STOCHASTIC, omega=1.0, p=0.8, recon=recon, seed=2013, check_every=4, defer=defer, after=1)
+    a = run_fix(cuda_device, U, dims, 0, **kw)
+    b = run_fix(cuda_device, U, dims, 3, **kw)
+    assert a[0] == b[0] == gf.GF_OK and a[:4] == b[:4]
+    assert np.array_equal(a[5], b[5]) and np.array_equal(a[6], b[6])
+    if recon == 18 and not defer:
+        Uo = U.copy()
+        it, th, conv = oracle.fix_until(Uo, dims, gauge=oracle.COULOMB, algo=oracle.STOCHASTIC, p=0.8, seed=2013,
+                                        theta_target=1e-12, max_iter=3000, check_every=4)
+        assert conv and abs(it - b[1]) <= 4
+
+
+def test_runahead_target_met_at_the_first_evaluation(cuda_device):
+    """theta below the target at the first evaluation: every block enqueued behind it must be a no-op."""
+    dims = (4, 4, 4, 6)
+    U = gi.smooth_random_gauge(dims, 0.3, 99)
+    a = run_fix(cuda_device, U, dims, 0, target=10.0, check_every=3)
+    b = run_fix(cuda_device, U, dims, 8, target=10.0, check_every=3)
+    assert a[1] == b[1] == 3 and a[:4] == b[:4] and np.array_equal(a[5], b[5])
+    Uo = U.copy()
+    for _ in range(3):
+        for parity in (0, 1):
+            oracle.sweep(Uo, dims, parity, algo=oracle.OVERRELAX, omega=1.7)
+    assert np.abs(b[5] - Uo).max() < 1e-12                           # exactly three iterations were applied
+    assert b[4] == a[4] + 7 * (2 * 3 + 2)                            # seven more blocks of 6 half-sweeps + 2 reduction kernels
+
+
+def test_runahead_argument_errors(cuda_device):
+    fld = gf.GaugeField((4, 4, 4, 4), precisions=("f64",), device=cuda_device)
+    for bad in (-1, 9):
+        with pytest.raises(gf.GFError):
+            fld.set_fix_runahead(bad)
+    fld.close()
+
+
+def test_runahead_hides_the_round_trip(cuda_device):
+    """On a lattice whose block of iterations is shorter than a host round trip the run-ahead loop is faster
+    (8^4, theta every iteration: measured 2-3x)."""
+    dims = (8, 8, 8, 8)
+    U = torch.from_numpy(gi.smooth_random_gauge(dims, 0.5, 5)).to(cuda_device)
+    times = {}
+    for depth in (0, 4):
+        fld = gf.GaugeField(dims, precisions=("f64",), device=cuda_device)
+        fld.set_fix_runahead(depth)
+        best = 1e9
+        for _ in range(3):
+            fld.pack(U, gf.GF_F64)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64, 1e-12, 5000, 1)
+            b.record()
+            torch.cuda.synchronize()
+            best = min(best, a.elapsed_time(b))
+        times[depth] = (best, it)
+        fld.close()
+    assert times[0][1] == times[4][1]
+    assert times[4][0] < 0.8 * times[0][0], times
