@@ -308,11 +308,7 @@ def run_ours(args):
             "metric": METRIC, "value": main["value"], "unit": "site-updates/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": pkey, "data": "synthetic",
-            "config": {"workload": "BASELINE.json configs[2]: SU(3) Landau 32^4, overrelaxation omega=1.7, %s links "
-                                   "stored as %d reals, eps=0.6 smooth field + Haar gauge transform" % (pkey, recon),
-                       "lattice": list(DIMS), "iterations_per_step": args.iters, "theta_F_every": args.check,
-                       "l2": "field (%d MB) larger than L2, no flush" % (V * 4 * recon * VARIANTS[args.variant][2] // 2**20),
-                       "parallelism": "replicas only (one lattice per GPU)" if world > 1 else "single GPU"},
+            "config": workload_config(args, world),
             "gflops_nominal": main["value"] * FLOP_PER_SITE_UPDATE / 1e9,
             "gpu_launches": main["gpu_launches"], "clocks": main["clocks"], "e2e": main["e2e"],
             "roofline": main["roofline"], "cpu_baseline": cpu, "variants": variants, "fix_until_theta_1e-12": fixes,
@@ -448,6 +444,16 @@ def cpu_baseline(U, budget_s):
             "sample": "%d full overrelaxation iteration(s) of the same 32^4 field, fp64, %.1f s" % (n, dt)}
 
 
+def workload_config(args, world):
+    """The `config` object of the JSON line: the workload both arms (--impl ours / reference) measure."""
+    pkey, recon, nbytes = VARIANTS[args.variant]
+    return {"workload": "BASELINE.json configs[2]: SU(3) Landau 32^4, overrelaxation omega=1.7, %s links "
+                        "stored as %d reals, eps=0.6 smooth field + Haar gauge transform" % (pkey, recon),
+            "lattice": list(DIMS), "iterations_per_step": args.iters, "theta_F_every": args.check,
+            "l2": "field (%d MB) larger than L2, no flush" % (V * 4 * recon * nbytes // 2**20),
+            "parallelism": "replicas only (one lattice per GPU)" if world > 1 else "single GPU"}
+
+
 def run_reference(args):
     """The reference arm of this tier = the CPU oracle, timed as it stands on the host cores."""
     rank = int(os.environ.get("RANK", "0"))
@@ -478,10 +484,11 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": "site-updates/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "BASELINE.json configs[2]: SU(3) Landau 32^4, overrelaxation omega=1.7, CPU oracle fp64",
-                   "lattice": list(dims), "iterations_per_step": 1},
+        # the CUDA arm's config: the workload is the same, a step of this arm is a bounded sample of it (see `sample`)
+        "config": workload_config(args, int(os.environ.get("WORLD_SIZE", "1"))),
         "cpu_baseline": {"value": val, "unit": "site-updates/s", "cores": cores, "kind": "oracle",
-                         "sample": "each step = 1 full overrelaxation iteration of the 32^4 field (input generated in %.0f s)" % t_gen},
+                         "sample": "each step = ONE of the %d overrelaxation iterations of a step of the workload, on the same 32^4 field, "
+                                   "fp64 oracle (canonical 18-real layout), no F/theta reduction (input generated in %.0f s)" % (args.iters, t_gen)},
         "e2e": {"value": val, "unit": "site-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gflops_nominal": val * FLOP_PER_SITE_UPDATE / 1e9,
     }

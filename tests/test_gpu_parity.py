@@ -440,3 +440,44 @@ def test_measure_async_equals_measure(cuda_device):
         assert B.lib.gf_measure_async(b.ctx, gf.GF_F64, 16) == gf.GF_EINVAL
         a.close()
         b.close()
+
+
+# ------------------------------------------------------------------------------ extreme shapes
+
+@pytest.mark.parametrize("dims", [(4096, 2, 2, 2), (2, 1024, 2, 2), (2, 2, 1022, 2), (2, 2, 2, 1000), (2, 2, 2, 2)])
+@pytest.mark.parametrize("prec,recon", [("f64", 18), ("f32", 12)])
+def test_extreme_aspect_ratios(cuda_device, dims, prec, recon):
+    """The largest time extent the library accepts (4096 slices of 4 sites per parity: per-slice reductions with one
+    partial block each, a 4096-entry slice list) and lattices that are one long line in x, y or z (x rows of two sites:
+    every x neighbour wraps; strides that are not multiples of the tile): one overrelaxation iteration in Landau gauge and
+    one stochastic iteration in Coulomb gauge against the oracle, F / theta per slice, default launch configuration."""
+    U = gi.smooth_random_gauge(dims, 0.4, 77)
+    for gauge, og, algo, oalgo, omega, p in ((gf.GF_LANDAU, oracle.LANDAU, gf.GF_OVERRELAX, oracle.OVERRELAX, 1.7, 0.0),
+                                             (gf.GF_COULOMB, oracle.COULOMB, gf.GF_STOCHASTIC, oracle.STOCHASTIC, 1.0, 0.8)):
+        fld = make_field(dims, prec, cuda_device, gauge, recon, seed=11)
+        fld.pack(to_device(U, prec, cuda_device), PREC[prec])
+        Uo = oracle_input(U, prec)
+        if recon == 12:
+            Uo = get_links(fld, prec)                             # row 2 as the device rebuilds it
+        fld.iterate(1, algo, omega, p, PREC[prec])
+        for parity in (0, 1):
+            oracle.sweep(Uo, dims, parity, og, oalgo, omega, p, seed=11, half_sweep_counter=parity)
+        assert np.abs(get_links(fld, prec) - Uo).max() < 2 * LINK_TOL[prec]
+        F, th = fld.measure(PREC[prec])
+        Fo, tho = np.atleast_1d(oracle.functional(Uo, dims, og)), np.atleast_1d(oracle.theta(Uo, dims, og))
+        assert len(F) == (dims[0] if gauge == gf.GF_COULOMB else 1)
+        assert np.allclose(F, Fo, rtol=REL_TOL[prec], atol=0)
+        assert np.allclose(th, tho, rtol=20 * REL_TOL[prec], atol=1e-30)
+        assert abs(fld.plaquette(PREC[prec]) - oracle.plaquette(Uo, dims)) < (1e-12 if prec == "f64" else 1e-5)
+        if gauge == gf.GF_COULOMB and dims[0] > 2:               # slice freezing with the longest possible slice list
+            mask = np.ones(dims[0], dtype=np.uint8)
+            mask[1::3] = 0
+            fld.set_slice_mask(mask)
+            before = get_links(fld, prec)
+            c0 = gf.gf_get_counter(fld.ctx)
+            fld.iterate(1, algo, omega, p, PREC[prec])
+            Um = before.copy()
+            for parity in (0, 1):
+                oracle.sweep_masked(Um, dims, parity, mask, algo=oalgo, omega=omega, p=p, seed=11, half_sweep_counter=c0 + parity)
+            assert np.abs(get_links(fld, prec) - Um).max() < 2 * LINK_TOL[prec]
+        fld.close()
