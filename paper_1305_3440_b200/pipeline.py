@@ -30,9 +30,16 @@ class HostPipeline:
     """
 
     def __init__(self, dims, gauge=B.GF_LANDAU, recon=B.GF_RECON18, precisions=("f64",), lanes=3, device="cuda:0",
-                 seed=0, gate=True, first_field=None):
+                 seed=0, gate=None, first_field=None):
         self.device = torch.device(device)
-        self.gate = bool(gate)
+        # gate = None: the sweep phases take turns when a half-sweep fills the GPU by itself.  Lattices of a few
+        # thousand sites per parity (less than one wave of blocks) are bound by the latency of one site update and
+        # share the GPU instead: 8^4, eight lanes: 0.74 against 2.5 ms per configuration fixed to theta < 1e-12.
+        sites_per_parity = 1
+        for d in dims:
+            sites_per_parity *= int(d)
+        sites_per_parity //= 2
+        self.gate = sites_per_parity > 4096 if gate is None else bool(gate)
         self.fields = [] if first_field is None else [first_field]
         self._borrowed = first_field is not None
         for _ in range(int(lanes) - len(self.fields)):
