@@ -124,7 +124,7 @@ def test_runahead_argument_errors(cuda_device):
 
 def test_runahead_hides_the_round_trip(cuda_device):
     """On a lattice whose block of iterations is shorter than a host round trip the run-ahead loop is faster
-    (8^4, theta every iteration: measured 2-3x)."""
+    (8^4, theta every iteration: 5.3 against 7.5 ms)."""
     dims = (8, 8, 8, 8)
     U = torch.from_numpy(gi.smooth_random_gauge(dims, 0.5, 5)).to(cuda_device)
     times = {}
@@ -143,4 +143,4 @@ def test_runahead_hides_the_round_trip(cuda_device):
         times[depth] = (best, it)
         fld.close()
     assert times[0][1] == times[4][1]
-    assert times[4][0] < 0.8 * times[0][0], times
+    assert times[4][0] < 0.95 * times[0][0], times           # measured 0.71
