@@ -6,7 +6,8 @@ directory, ONE line of the C source is replaced, the library is rebuilt there an
 ``pytest -x``; the run must fail.  The unmutated copy must pass (control).  Nothing of the CUDA path is involved.
 The mutants are the mistakes SURVEY.md 8(c) and the round-1 review name: signs of v, missing daggers, wrong
 neighbour, dropped trace, omega / subgroup / draw mix-ups, left instead of right multiplication, normalisations,
-Philox constants and counter layout, the 24-bit fraction, the unitarity checker's two outputs.
+Philox constants and counter layout, the 24-bit fraction, the unitarity checker's two outputs; a second batch: the
+periodic wrap, the site index, the SU(2) embedding, normalisations of a, Coulomb sums, the Philox site key, the plaquette.
 """
 import os
 import shutil
@@ -79,6 +80,37 @@ MUTANTS = [
     ("eq. 3 with the backward neighbour", "mat_dagger(G + neighbour(dims, c, mu, +1) * 9, gd);",
      "mat_dagger(G + neighbour(dims, c, mu, -1) * 9, gd);"),
     ("slice mask on the wrong axis", "if (slice_active && !slice_active[c[0]]) return;", "if (slice_active && !slice_active[c[3]]) return;"),
+    ("periodic wrap: x - mu of the first site lands on itself", "n[mu] = (c[mu] + dir + dims[mu]) % dims[mu];",
+     "n[mu] = c[mu] + dir < 0 ? 0 : (c[mu] + dir) % dims[mu];"),
+    ("site index with y and z exchanged",
+     "return (size_t)c[1] + (size_t)dims[1] * (c[2] + (size_t)dims[2] * (c[3] + (size_t)dims[3] * c[0]));",
+     "return (size_t)c[1] + (size_t)dims[1] * (c[3] + (size_t)dims[3] * (c[2] + (size_t)dims[2] * c[0]));"),
+    ("E_jj without the conjugation", "Ejj = a[0] - I * a[3];", "Ejj = a[0] + I * a[3];"),
+    ("E_ji sign", "const cd Eji = -a[2] + I * a[1]", "const cd Eji = a[2] + I * a[1]"),
+    ("g misses the first subgroup", "embed_left_multiply(g, sub[k][0], sub[k][1], a);",
+     "if (k > 0) embed_left_multiply(g, sub[k][0], sub[k][1], a);"),
+    ("relaxation without the normalisation", "for (int k = 0; k < 4; ++k) a[k] = v[k] / n;", "for (int k = 0; k < 4; ++k) a[k] = v[k];"),
+    ("overrelaxation normalised with |v|", "a[k] = w[k] / nw;", "a[k] = w[k] / n;"),
+    ("stochastic: one vector component of a^2 not doubled", "a[1] = 2.0 * a0 * a[1];", "a[1] = a0 * a[1];"),
+    ("Coulomb Delta over all four directions", "for (int mu = first_dir(gauge); mu < 4; ++mu) {\n        cd Af[9], Ab[9];",
+     "for (int mu = 0; mu < 4; ++mu) {\n        cd Af[9], Ab[9];"),
+    ("Coulomb F sums the temporal links too", "for (int mu = mu0; mu < 4; ++mu) {\n                const cd *u = link_cptr(U, s, mu);",
+     "for (int mu = 0; mu < 4; ++mu) {\n                const cd *u = link_cptr(U, s, mu);"),
+    ("Coulomb loop stops on the best slice", "if (th[t] > theta) theta = th[t];", "if (th[t] < theta) theta = th[t];"),
+    ("Philox: nine rounds", "for (int round = 0; round < 10; ++round) {", "for (int round = 0; round < 9; ++round) {"),
+    ("Philox: second multiplier on c1", "(uint64_t)0xCD9E8D57u * c2;", "(uint64_t)0xCD9E8D57u * c1;"),
+    ("Philox: key halves exchanged", "{ (uint32_t)seed, (uint32_t)(seed >> 32) };", "{ (uint32_t)(seed >> 32), (uint32_t)seed };"),
+    ("Philox: draws keyed by the per-parity index", "oracle_site_uniforms(seed, half_sweep_counter, (uint64_t)s, u);",
+     "oracle_site_uniforms(seed, half_sweep_counter, (uint64_t)(s / 2), u);"),
+    ("fix loop: both parities draw with the same counter",
+     "oracle_sweep(U, dims, gauge, 1, algo, omega, p, seed, first_counter + 2u * (uint32_t)it + 1u);",
+     "oracle_sweep(U, dims, gauge, 1, algo, omega, p, seed, first_counter + 2u * (uint32_t)it);"),
+    ("plaquette: last dagger dropped", "mat_dagger(link_cptr(U, s, nu), d2);",
+     "for (int k = 0; k < 9; ++k) d2[k] = link_cptr(U, s, nu)[k];"),
+    ("plaquette normalisation", "return sum / (6.0 * NC * (double)V);", "return sum / (4.0 * NC * (double)V);"),
+    ("update applied in three directions only", "for (int mu = 0; mu < 4; ++mu) {\n        mat_mul(g, fwd[mu], tmp);",
+     "for (int mu = 0; mu < 3; ++mu) {\n        mat_mul(g, fwd[mu], tmp);"),
+    ("|v| = 0 gives a = 0", "a[0] = 1.0; a[1] = a[2] = a[3] = 0.0;\n        return;", "a[0] = 0.0; a[1] = a[2] = a[3] = 0.0;\n        return;"),
     ("frozen slices never frozen", "if (active[t] && theta_slices[t] < theta_target) { active[t] = 0; frozen_at[t] = it; }",
      "if (active[t] && theta_slices[t] < 0.0) { active[t] = 0; frozen_at[t] = it; }"),
 ]

@@ -545,6 +545,27 @@ def test_coulomb_stochastic_converges_per_slice():
     assert oracle.theta(U, dims, oracle.LANDAU) > 1e-6      # Coulomb-fixed is not Landau-fixed
 
 
+def test_fix_loop_is_the_sequence_of_half_sweeps_with_consecutive_counters():
+    """SURVEY 8(c) O5 / reading A10: iteration `it` of the fix loop is sweep(parity 0) with half-sweep counter
+    first + 2 (it - 1), then sweep(parity 1) with first + 2 (it - 1) + 1 -- every half-sweep draws from its own
+    Philox stream.  The loop (stochastic, so that the counters matter) must leave bitwise the field of that explicit
+    sequence, and not the field of a sequence in which both parities of an iteration share a counter."""
+    dims = (4, 4, 4, 6)
+    U = gi.smooth_random_gauge(dims, 0.5, 17)
+    A = U.copy()
+    it, th, conv = oracle.fix_until(A, dims, oracle.COULOMB, oracle.STOCHASTIC, 1.0, 0.7, seed=99, first_counter=6,
+                                    theta_target=0.0, max_iter=3, check_every=1)
+    assert it == 3 and not conv
+    B, C = U.copy(), U.copy()
+    for k in range(3):
+        for parity in (0, 1):
+            oracle.sweep(B, dims, parity, oracle.COULOMB, oracle.STOCHASTIC, 1.0, 0.7, seed=99, half_sweep_counter=6 + 2 * k + parity)
+            oracle.sweep(C, dims, parity, oracle.COULOMB, oracle.STOCHASTIC, 1.0, 0.7, seed=99, half_sweep_counter=6 + 2 * k)
+    assert np.array_equal(A, B)
+    assert not np.array_equal(B, C)
+    assert th == np.max(oracle.theta(B, dims, oracle.COULOMB))
+
+
 def test_coulomb_slices_are_decoupled():
     """Temporal links never enter K (A17): changing slice t' != t leaves slice t's spatial links'
     evolution unchanged."""
