@@ -190,6 +190,11 @@ def run_ours(args):
                          # consecutive launches without the flush: what crosses the DRAM interface inside a step
                          "traffic_in_run": traffic_warm,
                          "dram_frac_in_run": (traffic_warm / (kern_ms * 1e-3) / 1e9 / peak) if traffic_warm else None,
+                         # What bounds a streaming kernel on this part is the throughput of the L2 slices: every algorithmic
+                         # byte crosses them once between SM and L2, every DRAM byte once more (fill or write-back).  The
+                         # copy behind `peak` pushes 2 x peak through them.
+                         "l2_slice_GBs": ((bytes_per_launch + traffic_warm) / (kern_ms * 1e-3) / 1e9) if traffic_warm else None,
+                         "l2_slice_frac_of_copy": ((bytes_per_launch + traffic_warm) / (kern_ms * 1e-3) / 1e9 / (2 * peak)) if traffic_warm else None,
                          "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
                          "bytes_per_launch": bytes_per_launch, "avg_launch_ms": kern_ms, "peak_source": peak_src,
                          "frac_of_8TBs_nominal": achieved / 8000.0},
@@ -262,7 +267,8 @@ def run_ours(args):
             r = bench_variant(name, max(1, args.steps // 3), 3, False)
             variants[name] = {"site_updates_per_s": r["value"], "gflops_nominal": r["value"] * FLOP_PER_SITE_UPDATE / 1e9,
                               "roofline_GBs": r["roofline"]["achieved"], "roofline_frac": r["roofline"]["frac"],
-                              "dram_frac": r["roofline"]["dram_frac"], "avg_launch_ms": r["roofline"]["avg_launch_ms"],
+                              "dram_frac": r["roofline"]["dram_frac"], "dram_frac_in_run": r["roofline"]["dram_frac_in_run"],
+                              "l2_slice_GBs": r["roofline"]["l2_slice_GBs"], "avg_launch_ms": r["roofline"]["avg_launch_ms"],
                               "sm_mhz": r["clocks"]["sm_mhz"]}
 
     # Time to solution (BASELINE.json configs[2]: "fp32, mixed and fp64"): gf_fix_until to theta < 1e-12 on the
