@@ -80,7 +80,7 @@ def test_pipelined_lattices_do_not_disturb_each_other(cuda_device):
         f.close()
 
 
-@pytest.mark.parametrize("gate", [True, False])
+@pytest.mark.parametrize("gate", [True, False, None])
 def test_host_pipeline_ensemble_matches_lone_runs_and_the_oracle(cuda_device, gate):
     """HostPipeline (the form bench.py's e2e leg uses): seven configurations in host memory through three lanes;
     every fixed field is bitwise the one a lone GaugeField produces, the iteration counts are the same, and one
