@@ -188,3 +188,37 @@ def test_32_4_accumulated_transformation_full_field(cuda_device, prec, recon):
     # the links have been through both half-sweeps (fp32: see test_32_4_full_field_against_oracle on the ill-conditioned site)
     assert np.abs(held_by_device(fld, prec) - Uo).max() < (LINK_TOL[prec] if prec == "f64" else 3e-5)
     fld.close()
+
+
+def _max_abs_diff_by_slices(a, b):
+    """max |a - b| over two large host arrays without a full-size temporary (one time slice at a time)."""
+    return max(float(np.abs(a[t] - b[t]).max()) for t in range(a.shape[0]))
+
+
+@pytest.mark.parametrize("prec,recon", [("f64", 18), ("f64", 12)])
+def test_64_4_full_field_one_iteration_against_oracle(cuda_device, prec, recon):
+    """configs[3] at full size: 64^4 = 16.8 M sites (9.66 GB of fp64 links, byte offsets beyond 2^32 in every link block),
+    omega = 1.8, default launch configuration: all 67 million links after parity 0 and after parity 1 within 1e-12 of the
+    oracle (running on from its own field, all host cores), then F and theta of the swept field to 1e-10.  Host memory:
+    two canonical copies of the field (19 GB); the comparison goes slice by slice."""
+    dims = (64, 64, 64, 64)
+    U = gi.torch_smooth_random_gauge(dims, 0.6, 4, device=cuda_device)
+    fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
+    fld.pack(U, PREC[prec])
+    del U
+    torch.cuda.empty_cache()
+    Uo = fld.unpack(PREC[prec], torch.complex128).cpu().numpy()           # what the device holds (row 2 rebuilt for 12-real)
+    torch.cuda.empty_cache()
+    for parity in (0, 1):
+        fld.sweep(parity, gf.GF_OVERRELAX, 1.8, 0.0, PREC[prec])
+        oracle.sweep(Uo, dims, parity, oracle.LANDAU, oracle.OVERRELAX, 1.8)
+        got = fld.unpack(PREC[prec], torch.complex128).cpu().numpy()
+        torch.cuda.empty_cache()
+        err = _max_abs_diff_by_slices(got, Uo)
+        assert err < LINK_TOL[prec], (prec, recon, parity, err)
+        del got
+    F, th = fld.measure(PREC[prec])
+    Fo, tho = oracle.functional(Uo, dims), oracle.theta(Uo, dims)
+    assert abs(F[0] / Fo - 1) < REL_TOL[prec] and abs(th[0] / tho - 1) < REL_TOL[prec], (F[0], Fo, th[0], tho)
+    assert abs(fld.plaquette(PREC[prec]) - oracle.plaquette(Uo, dims)) < 1e-12
+    fld.close()
