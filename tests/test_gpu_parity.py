@@ -481,3 +481,27 @@ def test_extreme_aspect_ratios(cuda_device, dims, prec, recon):
                 oracle.sweep_masked(Um, dims, parity, mask, algo=oalgo, omega=omega, p=p, seed=11, half_sweep_counter=c0 + parity)
             assert np.abs(get_links(fld, prec) - Um).max() < 2 * LINK_TOL[prec]
         fld.close()
+
+
+def test_the_link_tolerance_detects_a_relative_error_of_1e_9(cuda_device):
+    """Sensitivity of the 1e-12 link comparison: the same half-sweep with omega off by one part in 10^9, or with one real
+    of one input link off by 1e-9, lands outside the tolerance -- a kernel mistake of that size cannot hide in it."""
+    dims = (4, 6, 4, 6)
+    U = gi.smooth_random_gauge(dims, 0.5, 5)
+    Uo = U.copy()
+    oracle.sweep(Uo, dims, 0, oracle.LANDAU, oracle.OVERRELAX, 1.7)
+    fld = make_field(dims, "f64", cuda_device)
+    fld.pack(to_device(U, "f64", cuda_device), gf.GF_F64)
+    fld.sweep(0, gf.GF_OVERRELAX, 1.7 * (1 + 1e-9), 0.0, gf.GF_F64)
+    err = np.abs(get_links(fld, "f64") - Uo).max()
+    assert 1e-11 < err < 1e-7, err
+    W = U.copy()
+    W[1, 2, 3, 0, 2, 1, 1] += 1e-9
+    fld.pack(to_device(W, "f64", cuda_device), gf.GF_F64)
+    fld.sweep(0, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+    err = np.abs(get_links(fld, "f64") - Uo).max()
+    assert 1e-11 < err < 1e-7, err
+    fld.pack(to_device(U, "f64", cuda_device), gf.GF_F64)            # control: the unperturbed run is inside
+    fld.sweep(0, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+    assert np.abs(get_links(fld, "f64") - Uo).max() < 1e-12
+    fld.close()
