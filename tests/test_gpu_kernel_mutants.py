@@ -1,0 +1,119 @@
+"""Mutation run of the GPU parity tests (opt-in: GF_KERNEL_MUTANTS=1 python -m pytest tests/test_gpu_kernel_mutants.py -m gpu -s).
+
+The counterpart of tests/test_oracle_mutants.py for the CUDA side: every plausible single-line mistake in the kernels
+must make the GPU parity tests fail.  For each mutant a private copy of the package, include/, oracle/, gf_inputs.py
+and the GPU test files is made in a temporary directory, ONE source line of csrc/ is replaced, the library is rebuilt
+THERE (nvcc, only the translation units that changed) and a subset of the parity tests is run against it with
+``pytest -x``; the run must fail.  The unmutated copy must pass (control).  All mutants keep every memory access inside
+the buffers (arithmetic, signs, which draw / which neighbour inside the lattice), so a mutant cannot fault the GPU.
+Off by default because it rebuilds the library a dozen times (about five minutes on the GPU box); the outcome of a run
+is recorded in profiles/r2_kernel_mutants.md.
+"""
+import os
+import shutil
+import subprocess
+import sys
+import tempfile
+from concurrent.futures import ThreadPoolExecutor
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+PKG = "paper_1305_3440_b200"
+TEST_FILES = ["conftest.py", "test_gpu_parity.py", "test_gpu_checkers.py", "test_gpu_coulomb.py", "test_gpu_transform.py",
+              "test_gpu_fix_runahead.py", "curand_philox_ref.cu"]
+# the subset that is run against every mutant (the whole of these files takes about a minute)
+SELECT = ("pack_unpack or unit_links or one_sweep or ten_sweeps or stochastic_counter or philox or config1_fix or random_small or "
+          "extreme or unitarity_matches or reunitarize or cast_f32 or deferred_temporal_links_one or slice_mask or "
+          "accumulated_transformation or apply_transform or runahead_equals or runahead_coulomb")
+
+# (name, file under csrc/, exact fragment (must occur exactly once), replacement)
+MUTANTS = [
+    ("v1 sign", "gf_device.cuh", "T v1 = -(GF_IM(K, I, J) + GF_IM(K, J, I));", "T v1 = (GF_IM(K, I, J) + GF_IM(K, J, I));"),
+    ("v3 from the wrong difference", "gf_device.cuh", "T v3 = GF_IM(K, J, J) - GF_IM(K, I, I);", "T v3 = GF_IM(K, I, I) - GF_IM(K, J, J);"),
+    ("overrelaxation without |v|", "gf_device.cuh", "v0 = omega * v0 + (T(1) - omega) * n;", "v0 = omega * v0 + (T(1) - omega);"),
+    ("a^2: scalar part", "gf_device.cuh", "a[0] = t * a[0] - T(1);", "a[0] = t * a[0];"),
+    ("K update: E_JI sign", "gf_device.cuh", "GF_RE(K, J, b) = -a[2] * ir - a[1] * ii + a[0] * jr + a[3] * ji;",
+     "GF_RE(K, J, b) = a[2] * ir - a[1] * ii + a[0] * jr + a[3] * ji;"),
+    ("g = E3 E2 E1: a sign in E2", "gf_device.cuh", "Rr = -b[2], Ri = b[1], Sr = b[0], Si = -b[3];", "Rr = b[2], Ri = b[1], Sr = b[0], Si = -b[3];"),
+    ("U g instead of U g^dagger (one term)", "gf_device.cuh", "im = gf_fma(-GF_RE(U, a, 0), GF_IM(g, b, 0), im);", "im = gf_fma(GF_RE(U, a, 0), GF_IM(g, b, 0), im);"),
+    ("third row without the conjugation", "gf_device.cuh", "        GF_RE(m, 2, b) = re;\n        GF_IM(m, 2, b) = -im;", "        GF_RE(m, 2, b) = re;\n        GF_IM(m, 2, b) = im;"),
+    ("x-backward neighbour of the wrong parity row", "gf_device.cuh", "        if (s.xodd) return s.h;                                   // x-1 = 2 xh: same xh",
+     "        if (!s.xodd) return s.h;                                   // x-1 = 2 xh: same xh"),
+    ("site parity ignores t", "gf_device.cuh", "s.xodd = (s.c[2] + s.c[3] + s.c[0] + parity) & 1u;", "s.xodd = (s.c[2] + s.c[3] + parity) & 1u;"),
+    ("Philox key schedule", "gf_device.cuh", "k1 += 0xBB67AE85u;", "k1 += 0x9E3779B9u;"),
+    ("K without the dagger on the backward link", "gf_sweep.cu", "GF_IM(K, a, b) += (TK)GF_IM(Uf[d], a, b) - (TK)GF_IM(Ub[d], b, a);",
+     "GF_IM(K, a, b) += (TK)GF_IM(Uf[d], a, b) + (TK)GF_IM(Ub[d], b, a);"),
+    ("second subgroup uses the first draw", "gf_sweep.cu", "sq1 = (double)(w[1] >> 8) * (1.0 / 16777216.0) < P.p;", "sq1 = (double)(w[0] >> 8) * (1.0 / 16777216.0) < P.p;"),
+    ("draws keyed by the half-index", "gf_sweep.cu", "philox4x32_10(P.site_offset + 2u * h + s.xodd, 0u, counter, 0u, P.key0, P.key1, w);",
+     "philox4x32_10(P.site_offset + 2u * h, 0u, counter, 0u, P.key0, P.key1, w);"),
+    ("reverse traversal skips a block", "gf_sweep.cu", "const uint32_t bid = P.reverse ? gridDim.x - 1u - blockIdx.x : blockIdx.x;",
+     "const uint32_t bid = P.reverse ? gridDim.x - blockIdx.x : blockIdx.x;"),
+    ("theta keeps the trace", "gf_aux.cu", "const double d = GF_IM(M, a, a) - tr3;", "const double d = GF_IM(M, a, a);"),
+    ("F from a wrong diagonal entry", "gf_aux.cu", "F += (double)Uf[0] + (double)Uf[8] + (double)Uf[16];", "F += (double)Uf[0] + (double)Uf[8] + (double)Uf[14];"),
+    ("unitarity checker returns zero", "gf_aux.cu", "    block_reduce2<OpMax>(dmax, detmax, partials + partial_slot(mg));", "    block_reduce2<OpMax>(0.0 * dmax, 0.0 * detmax, partials + partial_slot(mg));"),
+    ("device-side stop decision inverted", "gf_aux.cu", "if (tail.stop != nullptr && th < tail.target) *tail.stop = 1u;", "if (tail.stop != nullptr && th > tail.target) *tail.stop = 1u;"),
+    ("theta normalisation", "gf_api.cu", "t.scale1 = 1.0 / (3.0 * (double)ctx->V * ctx->slab_n);", "t.scale1 = 1.0 / ((double)ctx->V * ctx->slab_n);"),
+]
+
+
+def _prepare(tmp):
+    shutil.copytree(os.path.join(ROOT, PKG), os.path.join(tmp, PKG), ignore=shutil.ignore_patterns("__pycache__"))
+    shutil.copytree(os.path.join(ROOT, "include"), os.path.join(tmp, "include"))
+    shutil.copytree(os.path.join(ROOT, "oracle"), os.path.join(tmp, "oracle"), ignore=shutil.ignore_patterns("__pycache__"))
+    shutil.copy(os.path.join(ROOT, "gf_inputs.py"), tmp)
+    os.makedirs(os.path.join(tmp, "tests"))
+    for f in TEST_FILES:
+        shutil.copy(os.path.join(ROOT, "tests", f), os.path.join(tmp, "tests", f))
+    shutil.copytree(os.path.join(ROOT, "tests", "golden"), os.path.join(tmp, "tests", "golden"))
+
+
+def _build(name, fname, old, new):
+    """Returns (name, tmp dir) with the mutated library built, or (name, error text)."""
+    tmp = tempfile.mkdtemp(prefix="gf_kmut_")
+    _prepare(tmp)
+    if old is not None:
+        path = os.path.join(tmp, PKG, "csrc", fname)
+        text = open(path).read()
+        if text.count(old) != 1:
+            return name, "fragment occurs %d times in %s (the mutant list is stale)" % (text.count(old), fname)
+        open(path, "w").write(text.replace(old, new))
+    r = subprocess.run([sys.executable, os.path.join(tmp, PKG, "build.py")], capture_output=True, text=True)
+    if r.returncode != 0:
+        return name, "the mutated source does not compile: %s" % r.stderr[-300:]
+    return name, tmp
+
+
+def _run_tests(tmp):
+    env = dict(os.environ, PYTHONPATH=tmp)
+    env.pop("GF_KERNEL_MUTANTS", None)
+    r = subprocess.run([sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider", "-m", "gpu", "-k", SELECT, "tests"],
+                       cwd=tmp, env=env, capture_output=True, text=True, timeout=1200)
+    failed = [l for l in r.stdout.splitlines() if l.startswith("FAILED") or l.startswith("ERROR")]
+    return r.returncode, (failed[0] if failed else r.stdout.strip().splitlines()[-1] if r.stdout.strip() else r.stderr[-200:])
+
+
+def test_every_kernel_mutant_fails_a_gpu_parity_test():
+    if os.environ.get("GF_KERNEL_MUTANTS") != "1":
+        pytest.skip("opt-in (GF_KERNEL_MUTANTS=1): rebuilds the library once per mutant; last run: profiles/r2_kernel_mutants.md")
+    jobs = [("control (unmutated)", None, None, None)] + MUTANTS
+    with ThreadPoolExecutor(max_workers=max(1, min(5, (os.cpu_count() or 4) // 3))) as ex:
+        built = list(ex.map(lambda j: _build(*j), jobs))
+    report, survivors = [], []
+    try:
+        for name, tmp in built:
+            assert os.path.isdir(tmp), "%s: %s" % (name, tmp)
+            rc, first = _run_tests(tmp)
+            report.append("%-48s -> rc %d  %s" % (name, rc, first))
+            print(report[-1], flush=True)
+            if name.startswith("control"):
+                assert rc == 0, "the unmutated copy must pass: %s" % first
+            elif rc == 0:
+                survivors.append(name)
+    finally:
+        for _, tmp in built:
+            if os.path.isdir(tmp):
+                shutil.rmtree(tmp, ignore_errors=True)
+    assert not survivors, "kernel mutants that pass the GPU parity tests: %s" % survivors
