@@ -27,7 +27,8 @@ TEST_FILES = ["conftest.py", "test_gpu_parity.py", "test_gpu_checkers.py", "test
 # the subset that is run against every mutant (the whole of these files takes about a minute)
 SELECT = ("pack_unpack or unit_links or one_sweep or ten_sweeps or stochastic_counter or philox or config1_fix or random_small or "
           "extreme or unitarity_matches or reunitarize or cast_f32 or deferred_temporal_links_one or slice_mask or "
-          "accumulated_transformation or apply_transform or runahead_equals or runahead_coulomb")
+          "accumulated_transformation or apply_transform or transformation_reproduces or mixed_exact or runahead_equals or "
+          "runahead_coulomb")
 
 # (name, file under csrc/, exact fragment (must occur exactly once), replacement)
 MUTANTS = [
@@ -55,6 +56,18 @@ MUTANTS = [
     ("F from a wrong diagonal entry", "gf_aux.cu", "F += (double)Uf[0] + (double)Uf[8] + (double)Uf[16];", "F += (double)Uf[0] + (double)Uf[8] + (double)Uf[14];"),
     ("unitarity checker returns zero", "gf_aux.cu", "    block_reduce2<OpMax>(dmax, detmax, partials + partial_slot(mg));", "    block_reduce2<OpMax>(0.0 * dmax, 0.0 * detmax, partials + partial_slot(mg));"),
     ("device-side stop decision inverted", "gf_aux.cu", "if (tail.stop != nullptr && th < tail.target) *tail.stop = 1u;", "if (tail.stop != nullptr && th > tail.target) *tail.stop = 1u;"),
+    # path-specific: the lazy third rows of fp64 / 12-real, the recorded transformation, the fp32 / 18-real tail, deferred
+    # temporal links, eq. 3 applied to a field, the re-projection, the plaquette, the Coulomb sums
+    ("lazy third row of the forward link enters K with the wrong sign", "gf_sweep.cu",
+     "fi = a < 2 ? GF_IM(Uf[d], a, b) : rf[2 * b + 1];", "fi = a < 2 ? GF_IM(Uf[d], a, b) : -rf[2 * b + 1];"),
+    ("accumulated transformation: G g^dagger instead of g G", "gf_sweep.cu", "        mul_g_U<ROWS>(g, Gt, out);", "        mul_U_gdag<ROWS>(Gt, g, out);"),
+    ("fp32 / 18-real tail loaded with re and im exchanged", "gf_device.cuh", "        m[16] = v.x;\n        m[17] = v.y;", "        m[16] = v.y;\n        m[17] = v.x;"),
+    ("deferred temporal links: no lane carries G(x)", "gf_sweep.cu", "const bool gslot = MODE == MODE_DEFER && j == 0;", "const bool gslot = MODE == MODE_DEFER && j == 5;"),
+    ("eq. 3 on a field: G(x+mu) without the dagger", "gf_aux.cu", "        mul_full(tmp, Gf, out, true);", "        mul_full(tmp, Gf, out, false);"),
+    ("re-projection: row 1 not orthogonalised", "gf_aux.cu", "        GF_RE(m, 1, b) -= pr * GF_RE(m, 0, b) - pi * GF_IM(m, 0, b);", "        GF_RE(m, 1, b) -= pr * GF_RE(m, 0, b) + pi * GF_IM(m, 0, b);"),
+    ("plaquette: third link not daggered", "gf_aux.cu", "            mul_full(C, A, D, true);", "            mul_full(C, A, D, false);"),
+    ("Coulomb F and theta over all four directions", "gf_aux.cu", "        if (mu < mu0) continue;\n        T Uf[18], Ub[18];", "        T Uf[18], Ub[18];"),
+    ("Coulomb F normalisation", "gf_api.cu", "t.scale0 = 1.0 / (3.0 * 3.0 * Vs);", "t.scale0 = 1.0 / (3.0 * 4.0 * Vs);"),
     ("theta normalisation", "gf_api.cu", "t.scale1 = 1.0 / (3.0 * (double)ctx->V * ctx->slab_n);", "t.scale1 = 1.0 / ((double)ctx->V * ctx->slab_n);"),
 ]
 
