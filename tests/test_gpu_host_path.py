@@ -135,3 +135,32 @@ def test_host_pipeline_surfaces_errors(cuda_device):
     with pytest.raises(gf.GFError):
         pipe.process(bufs, lambda f: f.iterate(1, gf.GF_OVERRELAX, 2.5, 0.0, gf.GF_F64), gf.GF_F64)   # omega out of range
     pipe.close()
+
+
+@pytest.mark.parametrize("gauge,algo,precision,recon", [("landau", "overrelax", "f64", 18), ("landau", "overrelax", "mixed-exact", 12),
+                                                        ("coulomb", "stochastic", "f64", 18), ("landau", "overrelax", "mixed", 18)])
+def test_command_line_fixes_an_ensemble_of_files(cuda_device, tmp_path, gauge, algo, precision, recon):
+    """python -m paper_1305_3440_b200.fix: three configurations from .npy files through the pipeline; every result is
+    gauge fixed as judged by the ORACLE (theta, Coulomb: every theta_t), has the input's plaquette and lies in SU(3)."""
+    from paper_1305_3440_b200 import fix
+    dims = (6, 4, 4, 6)
+    paths = []
+    for i in range(3):
+        U = gi.smooth_random_gauge(dims, 0.4, 40 + i)
+        p = tmp_path / ("cfg%d.npy" % i)
+        np.save(p, U)
+        paths.append(str(p))
+    out_dir = tmp_path / "fixed"
+    rc = fix.main(paths + ["--out-dir", str(out_dir), "--gauge", gauge, "--algo", algo, "--precision", precision, "--recon", str(recon),
+                           "--target", "1e-12", "--check-every", "5", "--seed", "7", "--lanes", "2", "--device", str(cuda_device)])
+    assert rc == 0
+    og = oracle.COULOMB if gauge == "coulomb" else oracle.LANDAU
+    for p in paths:
+        U = np.load(p)
+        W = np.ascontiguousarray(np.load(out_dir / p.split("/")[-1]))
+        assert W.shape == U.shape and W.dtype == np.complex128
+        assert np.max(oracle.theta(W, dims, og)) < 1e-12
+        assert abs(oracle.plaquette(W, dims) - oracle.plaquette(U, dims)) < (1e-6 if precision == "mixed" else 1e-12)
+        du, dd = oracle.unitarity_defect(W, dims)
+        assert du < 1e-12 and dd < 1e-12
+        assert np.min(oracle.functional(W, dims, og)) > np.min(oracle.functional(np.ascontiguousarray(U), dims, og))
