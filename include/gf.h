@@ -280,6 +280,15 @@ int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff);
  * The links produced are bitwise the same (sites of one parity are independent). */
 int gf_set_traversal(gf_ctx* ctx, int zigzag);
 
+/* Re-projection onto SU(3) inside gf_fix_until.  The paper does not mention one (reading A16) and in fp64 none is
+ * needed (|U U^dagger - 1| = 6e-13 after 20 000 iterations of a hot 32^4 field), but fp32 links lose unitarity linearly
+ * with the number of site updates (8e-4 after 5 000 iterations of the same field, and F then starts to fall).
+ * iterations > 0: at every evaluation point of gf_fix_until at which at least that many iterations have passed since the
+ * last re-projection, the field being swept -- and the transformation recorded with it (GF_MIXED_EXACT, deferred temporal
+ * links) -- is re-projected (Gram-Schmidt on rows 0 and 1 in fp64, row 2 = conj(row0 x row1)) before theta is measured.
+ * 0 (default) = never: runs are then sweep by sweep those of the oracle.  Errors: GF_EINVAL. */
+int gf_set_reunitarize_every(gf_ctx* ctx, int iterations);
+
 /* How gf_fix_until follows theta ("iterated until the requested gauge precision theta has
  * been reached").  blocks = 0: after every evaluation the host waits for theta before it enqueues the
  * next check_every iterations.  blocks = 1..8 (default 4): up to that many blocks of {iterations;

@@ -56,6 +56,7 @@ struct gf_ctx {
     double* slice_tmp;          // workspace: 2 doubles per time slice (reduce_slices_kernel, whole-lattice sums)
     uint32_t* reduce_counter;   // workspace: blocks of the last reduction stage that have finished (zero between launches)
     uint32_t* stop_dev;         // workspace: zero except while a run-ahead fix loop has reached its target on the device
+    int reunit_every;           // gf_fix_until re-projects the swept field onto SU(3) every so many iterations (0 = never)
     int runahead;               // evaluation blocks gf_fix_until keeps in flight (0 = wait for every theta before going on)
     cudaEvent_t fix_events[8];  // one per block in flight
     double* slice_out;          // 2 doubles per time slice, written by the last reduction kernel: the DEVICE ADDRESS OF
@@ -709,6 +710,21 @@ extern "C" int gf_theta(gf_ctx* ctx, int precision, double* host_out)
     return gf_measure(ctx, precision, nullptr, host_out);
 }
 
+// Re-projection of the field being swept (and of the transformation recorded with it) onto SU(3) inside a fix loop
+// (gf_set_reunitarize_every): Gram-Schmidt on rows 0 and 1 in fp64, row 2 rebuilt.  Enqueued at an evaluation point, before
+// theta is measured; `stop`: the run-ahead loop's stop word (the re-projection too must leave a converged field alone).
+static int enqueue_reunitarize(gf_ctx* ctx, int precision, const uint32_t* stop)
+{
+    cudaError_t e = launch_cast(precision, precision, ctx->recon, ctx->links[precision], ctx->links[precision], ctx->G, 1, 8, ctx->stream, stop);
+    if (e == cudaSuccess && ctx->gtrans[precision]) {
+        e = launch_cast(precision, precision, ctx->recon, ctx->gtrans[precision], ctx->gtrans[precision], ctx->G, 1, 2, ctx->stream, stop);
+        ctx->launches += 1;
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "re-projection in the fix loop");
+    ctx->launches += 1;
+    return GF_OK;
+}
+
 // The fix loop without a host round trip per evaluation.  Blocks of {iterations up to the next evaluation; F / theta
 // reduction} are enqueued up to ctx->runahead ahead of the block whose result the host is waiting for.  The last
 // reduction kernel of a block compares theta with the target ON THE DEVICE (the same double, the same comparison the
@@ -723,7 +739,7 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
     const int depth = ctx->runahead < kRunAhead ? ctx->runahead : kRunAhead;
     const int mu0 = ctx->gauge == GF_COULOMB ? 1 : 0;
     const size_t slot_len = (size_t)2 * ctx->dims[0];
-    int it_enq = *it_io, rc = GF_NOT_CONVERGED, err = GF_OK;
+    int it_enq = *it_io, rc = GF_NOT_CONVERGED, err = GF_OK, since_reunit = 0;
     long head = 0, tail = 0;
     ReduceTail rt = measure_tail(ctx);
     rt.stop = ctx->stop_dev;
@@ -735,6 +751,12 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
             for (int k = 0; k < n && err == GF_OK; ++k) err = enqueue_iteration(ctx, algo, omega, p, precision);
             if (err != GF_OK) break;
             it_enq += n;
+            since_reunit += n;
+            if (ctx->reunit_every > 0 && since_reunit >= ctx->reunit_every) {
+                err = enqueue_reunitarize(ctx, precision, ctx->stop_dev);
+                if (err != GF_OK) break;
+                since_reunit = 0;
+            }
             const int s = (int)(head % depth);
             cudaError_t e = launch_measure(precision, ctx->recon, ctx->links[precision], ctx->prev_links[precision], ctx->G, mu0,
                                            ctx->mg, ctx->partials, rt, ctx->slots_dev + (size_t)(kAsyncSlots + s) * slot_len, ctx->stream);
@@ -771,7 +793,7 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
 static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
                      int check_every, int* it_io, double* theta_out)
 {
-    int it = *it_io;
+    int it = *it_io, since_reunit = 0;
     int rc = GF_NOT_CONVERGED;
     const bool freeze = ctx->freeze_slices && ctx->gauge == GF_COULOMB;
     // slice freezing changes the launch list between evaluations on the host: that loop waits for every theta
@@ -792,6 +814,12 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
             if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         }
         it += n;
+        since_reunit += n;
+        if (ctx->reunit_every > 0 && since_reunit >= ctx->reunit_every) {
+            int er = enqueue_reunitarize(ctx, precision, nullptr);
+            if (er != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return er; }
+            since_reunit = 0;
+        }
         int e = measure_to_host(ctx, precision, freeze);
         if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         *theta_out = finish_measure(ctx, nullptr, nullptr);
@@ -1193,6 +1221,14 @@ extern "C" int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff)
     if (!ctx) return GF_EINVAL;
     if (!(theta_handoff > 0.0)) return fail(ctx, GF_EINVAL, "the hand-off theta must be positive");
     ctx->handoff = theta_handoff;
+    return GF_OK;
+}
+
+extern "C" int gf_set_reunitarize_every(gf_ctx* ctx, int iterations)
+{
+    if (!ctx) return GF_EINVAL;
+    if (iterations < 0) return fail(ctx, GF_EINVAL, "negative re-projection interval");
+    ctx->reunit_every = iterations;
     return GF_OK;
 }
 

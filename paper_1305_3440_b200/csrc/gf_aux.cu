@@ -459,10 +459,11 @@ __device__ __forceinline__ void project_su3(double (&m)[18])
 
 // every (parity, mu, h) link: load as TS, optionally re-project in fp64, store as TD
 template <typename TS, typename TD, int RECON>
-__global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int reproject)   // src may alias dst
+__global__ void cast_kernel(const TS* src, TD* dst, const Geom G, const int reproject, const uint32_t* stop)   // src may alias dst
 {
     const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= G.Vh) return;
+    if (stop != nullptr && *stop != 0u) return;      // run-ahead fix loop: enqueued behind the evaluation that met the target
     const uint32_t pm = blockIdx.y;                  // parity*4 + mu
     TS u[18];
     load_link<RECON>(src + (size_t)pm * RECON * padded_vh<TS>(G), h, u);
@@ -527,27 +528,28 @@ cudaError_t launch_unpack(int precision, int recon, const void* links, const Geo
 }
 
 template <typename TS, typename TD>
-static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G, int reproject, int nblocks, cudaStream_t st)
+static cudaError_t cast_run(int recon, const void* src, void* dst, const Geom& G, int reproject, int nblocks, cudaStream_t st,
+                            const uint32_t* stop)
 {
     const uint32_t block = 128;
     const dim3 grid((G.Vh + block - 1) / block, (uint32_t)nblocks, 1);
     if (recon == 12) {
         uniform_carveout(cast_kernel<TS, TD, 12>);
-        cast_kernel<TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
+        cast_kernel<TS, TD, 12><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject, stop);
     } else {
         uniform_carveout(cast_kernel<TS, TD, 18>);
-        cast_kernel<TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject);
+        cast_kernel<TS, TD, 18><<<grid, block, 0, st>>>(static_cast<const TS*>(src), static_cast<TD*>(dst), G, reproject, stop);
     }
     return cudaGetLastError();
 }
 
 cudaError_t launch_cast(int from_precision, int to_precision, int recon, const void* src, void* dst,
-                        const Geom& G, int reproject, int nblocks, cudaStream_t st)
+                        const Geom& G, int reproject, int nblocks, cudaStream_t st, const uint32_t* stop)
 {
-    if (from_precision == PREC_F32 && to_precision == PREC_F64) return cast_run<float, double>(recon, src, dst, G, reproject, nblocks, st);
-    if (from_precision == PREC_F64 && to_precision == PREC_F32) return cast_run<double, float>(recon, src, dst, G, reproject, nblocks, st);
-    if (from_precision == PREC_F64) return cast_run<double, double>(recon, src, dst, G, reproject, nblocks, st);
-    return cast_run<float, float>(recon, src, dst, G, reproject, nblocks, st);
+    if (from_precision == PREC_F32 && to_precision == PREC_F64) return cast_run<float, double>(recon, src, dst, G, reproject, nblocks, st, stop);
+    if (from_precision == PREC_F64 && to_precision == PREC_F32) return cast_run<double, float>(recon, src, dst, G, reproject, nblocks, st, stop);
+    if (from_precision == PREC_F64) return cast_run<double, double>(recon, src, dst, G, reproject, nblocks, st, stop);
+    return cast_run<float, float>(recon, src, dst, G, reproject, nblocks, st, stop);
 }
 
 // ------------------------------------------------------- the accumulated transformation G(x)

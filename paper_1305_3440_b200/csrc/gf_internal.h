@@ -80,8 +80,9 @@ cudaError_t launch_pack(int precision, int recon, void* links, const Geom& G, co
 cudaError_t launch_unpack(int precision, int recon, const void* links, const Geom& G, void* canonical,
                           int canonical_is_f64, cudaStream_t st);
 // nblocks: 8 for a link field (parity x mu), 2 for a transformation field (parity)
+// stop: NULL, or the stop word of the run-ahead fix loop (the kernel then does nothing once it is set)
 cudaError_t launch_cast(int from_precision, int to_precision, int recon, const void* src, void* dst,
-                        const Geom& G, int reproject, int nblocks, cudaStream_t st);
+                        const Geom& G, int reproject, int nblocks, cudaStream_t st, const uint32_t* stop = nullptr);
 // transformation field G[parity][chunk][h] <-> canonical (V,3,3) complex; identity fill
 cudaError_t launch_transform_pack(int precision, int recon, void* gtrans, const Geom& G, const void* canonical,
                                   int canonical_is_f64, cudaStream_t st);

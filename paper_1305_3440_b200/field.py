@@ -171,3 +171,6 @@ class GaugeField:
 
     def set_fix_runahead(self, blocks):
         B.gf_set_fix_runahead(self.ctx, blocks)
+
+    def set_reunitarize_every(self, iterations):
+        B.gf_set_reunitarize_every(self.ctx, iterations)

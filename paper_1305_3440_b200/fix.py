@@ -3,6 +3,7 @@
     python -m paper_1305_3440_b200.fix IN.npy [IN2.npy ...] --out-dir DIR [--gauge landau|coulomb]
            [--algo overrelax|relax|stochastic] [--omega 1.7] [--p 0.8] [--precision f64|f32|mixed|mixed-exact]
            [--recon 18|12] [--target 1e-12] [--max-iter 100000] [--check-every 10] [--seed 0] [--lanes 3]
+           [--reunitarize-every 0]
 
 IN.npy holds the links in the canonical layout of include/gf.h: a complex128 array of shape (Nt, Nz, Ny, Nx, 4, 3, 3).
 The fixed configuration is written to DIR/<name>.npy and one line per file reports iterations, theta, F and the drift of
@@ -39,6 +40,8 @@ def main(argv=None):
     ap.add_argument("--max-iter", type=int, default=100000)
     ap.add_argument("--check-every", type=int, default=10)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--reunitarize-every", type=int, default=0,
+                    help="re-project the swept field onto SU(3) every so many iterations (fp32 runs of thousands of iterations)")
     ap.add_argument("--lanes", type=int, default=3)
     ap.add_argument("--device", default="cuda:0")
     args = ap.parse_args(argv)
@@ -63,6 +66,7 @@ def main(argv=None):
     for f in pipe.fields:
         if mode == gf.GF_MIXED_EXACT:
             f.attach_transform(("f64", "f32"))
+        f.set_reunitarize_every(args.reunitarize_every)
 
     def work(f):
         P0 = f.plaquette(io_prec)

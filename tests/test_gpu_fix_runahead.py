@@ -144,3 +144,64 @@ def test_runahead_hides_the_round_trip(cuda_device):
         fld.close()
     assert times[0][1] == times[4][1]
     assert times[4][0] < 0.95 * times[0][0], times           # measured 0.71
+
+
+# ------------------------------------------------------------------------------ re-projection inside the fix loop
+
+def _long_run(cuda_device, U, dims, prec_name, reunit, runahead=4, iters=1500, check=50):
+    prec = gf.GF_F32 if prec_name == "f32" else gf.GF_F64
+    cd = torch.complex64 if prec_name == "f32" else torch.complex128
+    fld = gf.GaugeField(dims, precisions=(prec_name,), device=cuda_device)
+    fld.pack(torch.from_numpy(U).to(cuda_device).to(cd), prec)
+    fld.set_reunitarize_every(reunit)
+    fld.set_fix_runahead(runahead)
+    rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, prec, 0.0, iters, check)       # target 0: runs all iterations
+    out = fld.unpack(prec, torch.complex128).cpu().numpy()
+    F, _ = fld.measure(prec)
+    fld.close()
+    return rc, it, th, out, F[0]
+
+
+def test_reprojection_keeps_a_long_fp32_run_in_SU3(cuda_device):
+    """fp32 links lose unitarity linearly with the number of site updates; with gf_set_reunitarize_every the defect stays
+    at the fp32 rounding level (both judged by the ORACLE's checker), the plaquette stays that of the input to fp32
+    accuracy, and the run-ahead loop takes bitwise the same path as the loop that waits."""
+    dims = (8, 8, 8, 8)
+    U = gi.hot_links(dims, 4)
+    P0 = oracle.plaquette(U, dims)
+    plain = _long_run(cuda_device, U, dims, "f32", 0)
+    kept = _long_run(cuda_device, U, dims, "f32", 100)
+    waits = _long_run(cuda_device, U, dims, "f32", 100, runahead=0)
+    assert plain[1] == kept[1] == 1500 and plain[0] == kept[0] == gf.GF_NOT_CONVERGED
+    d_plain = oracle.unitarity_defect(np.ascontiguousarray(plain[3]), dims)
+    d_kept = oracle.unitarity_defect(np.ascontiguousarray(kept[3]), dims)
+    assert d_plain[0] > 1e-4 and d_kept[0] < 2e-5 and d_kept[1] < 2e-5, (d_plain, d_kept)
+    assert abs(oracle.plaquette(np.ascontiguousarray(kept[3]), dims) - P0) < 2e-5
+    assert kept[4] >= plain[4] - 1e-6                          # the functional is not worse for it
+    assert np.array_equal(kept[3], waits[3]) and kept[2] == waits[2]
+
+
+def test_reprojection_in_fp64_is_invisible(cuda_device):
+    """In fp64 the re-projection moves the links by rounding errors only: same iteration count, links within 1e-12 of the
+    run without it, result fixed as judged by the oracle."""
+    dims = (4, 6, 6, 4)
+    U = gi.smooth_random_gauge(dims, 0.4, 8)
+    res = {}
+    for reunit in (0, 10):
+        fld = gf.GaugeField(dims, precisions=("f64",), device=cuda_device)
+        fld.pack(torch.from_numpy(U).to(cuda_device), gf.GF_F64)
+        fld.set_reunitarize_every(reunit)
+        n0 = gf.gf_launch_count(fld.ctx)
+        rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64, 1e-12, 3000, 5)
+        res[reunit] = (rc, it, fld.unpack(gf.GF_F64).cpu().numpy(), gf.gf_launch_count(fld.ctx) - n0)
+        fld.close()
+    assert res[0][0] == res[10][0] == gf.GF_OK and res[0][1] == res[10][1]
+    assert np.abs(res[0][2] - res[10][2]).max() < 1e-12
+    assert res[10][3] > res[0][3]                              # the re-projection kernels were launched
+    assert oracle.theta(np.ascontiguousarray(res[10][2]), dims) < 1e-12
+    with pytest.raises(gf.GFError):
+        f = gf.GaugeField(dims, precisions=("f64",), device=cuda_device)
+        try:
+            f.set_reunitarize_every(-1)
+        finally:
+            f.close()
