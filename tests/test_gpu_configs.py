@@ -266,9 +266,11 @@ def test_32_4_as_two_slabs_equals_the_undivided_lattice(cuda_device):
 # ------------------------------------------------------------------------------ the paper's own per-GPU lattices
 
 @pytest.mark.parametrize("dims,prec,recon", [((48, 48, 48, 48), "f64", 18), ((48, 48, 48, 48), "f32", 12),
-                                             ((32, 64, 64, 64), "f64", 12), ((32, 64, 64, 64), "f32", 18)])
+                                             ((32, 64, 64, 64), "f64", 12), ((32, 64, 64, 64), "f32", 18),
+                                             ((4, 128, 128, 128), "f64", 18), ((4, 128, 128, 128), "f32", 12)])
 def test_fig3_lattices_sampled_against_oracle(cuda_device, dims, prec, recon):
-    """48^4 and 64^3 x 32, the per-GPU lattices of the paper's weak-scaling figure: extents that are
+    """48^4 and 64^3 x 32, the per-GPU lattices of the paper's weak-scaling figure, and 128^3 x 4, the
+    largest time slice of its Tab. 1 (a temporal stride of a million sites): extents that are
     not powers of two at a size of several GB, default launch configuration.  One iteration with sampled sites
     recomputed by the oracle, then invariants after 20 more."""
     U = gi.torch_smooth_random_gauge(dims, 0.6, 48, device=cuda_device).to(CDTYPE[prec])
