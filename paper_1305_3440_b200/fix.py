@@ -7,8 +7,8 @@
 
 IN.npy holds the links in the canonical layout of include/gf.h: a complex128 array of shape (Nt, Nz, Ny, Nx, 4, 3, 3).
 The fixed configuration is written to DIR/<name>.npy and one line per file reports iterations, theta, F and the drift of
-the (gauge-invariant) plaquette.  Several files go through HostPipeline: copies of one configuration overlap the sweeps
-of another.  Argument marshalling and file I/O only; every step of the method runs in libgf_b200.so (the
+the (gauge-invariant) plaquette.  Several files go through HostPipeline, one pinned buffer per lane: reading, copying and
+writing one configuration overlap the sweeps of another, whatever the size of the ensemble.  Argument marshalling and file I/O only; every step of the method runs in libgf_b200.so (the
 sweeps are iterated until the requested gauge precision theta has been reached).
 """
 import argparse
@@ -77,17 +77,19 @@ def main(argv=None):
         F, _ = f.measure(io_prec)
         return rc, it, th, float(np.mean(F)), f.plaquette(io_prec) - P0
 
-    hosts = []
-    for path in args.inputs:
-        a = np.load(path)
+    def fill(i, buf):                               # runs in the lane's thread: file I/O overlaps the other lanes' sweeps
+        a = np.load(args.inputs[i])
         if tuple(a.shape) != tuple(first.shape):
-            raise SystemExit("%s: shape %r differs from %r" % (path, a.shape, first.shape))
-        hosts.append(torch.from_numpy(np.ascontiguousarray(a)).to(cdtype).pin_memory())
-    results = pipe.process(hosts, work, io_prec)
+            raise SystemExit("%s: shape %r differs from %r" % (args.inputs[i], a.shape, first.shape))
+        buf.copy_(torch.from_numpy(np.ascontiguousarray(a)).to(cdtype))
+
+    def drain(i, buf, result):
+        out = os.path.join(args.out_dir, os.path.basename(args.inputs[i]))
+        np.save(out, buf.numpy().astype(np.complex128))
+        return out, result
+
     status = 0
-    for path, host, (rc, it, th, F, dP) in zip(args.inputs, hosts, results):
-        out = os.path.join(args.out_dir, os.path.basename(path))
-        np.save(out, host.numpy())
+    for path, (out, (rc, it, th, F, dP)) in zip(args.inputs, pipe.process_stream(len(args.inputs), fill, work, drain, io_prec, cdtype)):
         print("%s -> %s: %s after %d iterations, theta = %.3e, F = %.9f, plaquette drift %.1e" % (
             path, out, "converged" if rc == gf.GF_OK else "NOT converged", it, th, F, dP), flush=True)
         status |= 0 if rc == gf.GF_OK else 1

@@ -99,6 +99,42 @@ class HostPipeline:
             raise errors[0]
         return results
 
+    def process_stream(self, n_items, fill, work, drain, precision=B.GF_F64, dtype=torch.complex128):
+        """An ensemble that does not fit host memory at once.  Every lane owns ONE pinned buffer of the canonical shape;
+        for item i (lane i % lanes, in order) `fill(i, buffer)` writes the configuration into it (e.g. from a file),
+        the buffer is loaded, `work(field)` runs in the lane's turn, the result is stored back into the buffer and
+        `drain(i, buffer, result)` consumes it (e.g. writes a file) before the lane goes on.  fill and drain run in the
+        lane's host thread: file I/O of one lane overlaps the copies and sweeps of the others.  Returns the list of
+        whatever drain returned."""
+        fields = self.fields
+        bufs = [torch.empty(f.shape, dtype=dtype).pin_memory() for f in fields]
+        out, errors = [None] * int(n_items), []
+        self.done_at = []
+
+        def lane(k):
+            try:
+                torch.cuda.set_device(self.device)
+                f, buf = fields[k], bufs[k]
+                for i in range(k, int(n_items), len(fields)):
+                    fill(i, buf)
+                    f.load_host(buf, precision)
+                    r = self._run_work(f, work)
+                    f.store_host(buf, precision)
+                    out[i] = drain(i, buf, r)
+                    self.done_at.append(time.perf_counter())
+            except Exception as e:
+                errors.append(e)
+
+        threads = [threading.Thread(target=lane, args=(k,)) for k in range(min(len(fields), int(n_items)))]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        torch.cuda.synchronize(self.device)
+        if errors:
+            raise errors[0]
+        return out
+
     def steady_seconds_per_item(self):
         """Between the first and the last completed item of the latest process() the pipeline is full: the time per
         item without the one copy before the first sweep and the one after the last that nothing overlaps."""

@@ -164,3 +164,31 @@ def test_command_line_fixes_an_ensemble_of_files(cuda_device, tmp_path, gauge, a
         du, dd = oracle.unitarity_defect(W, dims)
         assert du < 1e-12 and dd < 1e-12
         assert np.min(oracle.functional(W, dims, og)) > np.min(oracle.functional(np.ascontiguousarray(U), dims, og))
+
+
+def test_host_pipeline_streams_an_ensemble_through_one_buffer_per_lane(cuda_device):
+    """process_stream: nine items through two lanes with one pinned buffer each; fill / drain run per item in order on
+    their lane; results bitwise those of process() on the same inputs."""
+    from paper_1305_3440_b200.pipeline import HostPipeline
+    dims = (4, 4, 6, 4)
+    inputs = [torch.from_numpy(gi.smooth_random_gauge(dims, 0.4, 300 + i)) for i in range(9)]
+
+    def work(f):
+        f.iterate(7, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64)
+        return f.measure(gf.GF_F64)
+
+    pipe = HostPipeline(dims, precisions=("f64",), lanes=2, device=cuda_device)
+    want_bufs = [h.clone().pin_memory() for h in inputs]
+    want = pipe.process(want_bufs, work, gf.GF_F64)
+    seen = []
+    got = pipe.process_stream(9, lambda i, buf: buf.copy_(inputs[i]), work,
+                              lambda i, buf, r: (seen.append(i), buf.clone(), r)[1:], gf.GF_F64)
+    pipe.close()
+    assert sorted(seen) == list(range(9))
+    for i in range(9):
+        assert torch.equal(got[i][0], want_bufs[i]) and got[i][1] == want[i]
+    Uo = np.ascontiguousarray(inputs[4].numpy())
+    for _ in range(7):
+        for parity in (0, 1):
+            oracle.sweep(Uo, dims, parity, algo=oracle.OVERRELAX, omega=1.7)
+    assert np.abs(got[4][0].numpy() - Uo).max() < 1e-12
