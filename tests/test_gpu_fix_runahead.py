@@ -205,3 +205,28 @@ def test_reprojection_in_fp64_is_invisible(cuda_device):
             f.set_reunitarize_every(-1)
         finally:
             f.close()
+
+
+@pytest.mark.parametrize("runahead", [0, 4])
+def test_reprojection_with_the_recorded_transformation(cuda_device, runahead):
+    """GF_MIXED_EXACT with gf_set_reunitarize_every: the fp32 links AND the recorded fp32 G(x) are re-projected during the
+    fp32 phase; the result is still G U G^dagger of the untouched fp64 input -- plaquette kept to 1e-12, fixed to
+    theta < 1e-12 and in SU(3) as judged by the oracle -- and the returned G reproduces it through eq. 3."""
+    dims = (6, 4, 4, 6)
+    U = gi.smooth_random_gauge(dims, 0.5, 21)
+    fld = gf.GaugeField(dims, recon=12, precisions=("f64", "f32"), device=cuda_device)
+    fld.pack(torch.from_numpy(U).to(cuda_device), gf.GF_F64)
+    fld.attach_transform(("f64", "f32"))
+    fld.set_mixed_handoff(1e-9)
+    fld.set_reunitarize_every(10)
+    fld.set_fix_runahead(runahead)
+    rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_MIXED_EXACT, 1e-12, 5000, 5)
+    assert rc == gf.GF_OK and th < 1e-12
+    W = np.ascontiguousarray(fld.unpack(gf.GF_F64).cpu().numpy())
+    G = np.ascontiguousarray(fld.transform(gf.GF_F64).cpu().numpy())
+    fld.close()
+    assert oracle.theta(W, dims) < 1e-12
+    assert abs(oracle.plaquette(W, dims) - oracle.plaquette(U, dims)) < 1e-12
+    du, dd = oracle.unitarity_defect(W, dims)
+    assert du < 1e-12 and dd < 1e-12
+    assert np.abs(oracle.apply_transform(U, G, dims) - W).max() < 1e-11
