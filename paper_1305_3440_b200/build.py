@@ -25,12 +25,17 @@ NVCC_FLAGS += os.environ.get("GF_EXTRA_NVCC_FLAGS", "").split()
 
 
 def source_hash() -> str:
-    """sha256 over the kernel sources and headers: ties a profile under profiles/ to the code it was taken at."""
+    """sha256 over the CODE of the kernel sources and headers (comments and white space removed): ties a profile under
+    profiles/ to the code it was taken at; rewording a comment does not invalidate a capture."""
     import hashlib
+    import re
     h = hashlib.sha256()
     for f in [os.path.join(CSRC, s) for s in SOURCES] + HEADERS:
+        text = open(f, encoding="utf-8").read()
+        text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)          # block comments
+        text = re.sub(r"//[^\n]*", " ", text)                       # line comments (no string literal here holds "//")
         h.update(os.path.basename(f).encode())
-        h.update(open(f, "rb").read())
+        h.update(" ".join(text.split()).encode())
     return h.hexdigest()[:16]
 
 

@@ -104,9 +104,9 @@ __device__ __forceinline__ uint32_t forward_index(const Geom& G, const Site& s, 
 // A warp reading chunk c of 32 consecutive sites moves 512 contiguous bytes with one 128-bit load per lane, and a
 // neighbour shifted by one site stays 16-byte aligned, as with chunk planes over the whole lattice; but all the
 // chunks of a link for one tile now form ONE contiguous run of 32 * RECON * 8 = 4608 / 3072 bytes (the same in fp32
-// with its 64-site tiles), which is what the TMA bulk copies of the streamed kernel (gf_wave.cu) move per
-// request -- a bulk copy costs ~35 ns of TMA time whatever its size (profiles/r2_tma_request_size.txt) -- and the
-// chunks of one link share DRAM pages.  Registers hold a link as m[18] = row-major (re, im) pairs.
+// with its 64-site tiles): the chunks of one link share DRAM pages, gf_pack / gf_unpack get contiguous runs on this
+// side, and it is what a bulk copy moves per request (the streamed kernel of round 2, measured and removed:
+// profiles/r2_wavefront_attempt.md; a bulk copy costs ~35 ns of TMA time whatever its size, profiles/r2_tma_request_size.txt).  Registers hold a link as m[18] = row-major (re, im) pairs.
 
 template <typename T> struct Vec16;
 template <> struct Vec16<double> { using type = double2; };
