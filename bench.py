@@ -275,10 +275,12 @@ def run_ours(args):
     # same 32^4 input, theta every 10 iterations.  Context for the SP/MP/DP reading of the metric, not the headline.
     fixes = {}
     if not args.no_fix:
-        runs = [("f64", gf.GF_F64, None, 18), ("mixed_handoff_1e-6", gf.GF_MIXED, 1e-6, 18),
-                ("mixed_exact_handoff_1e-10", gf.GF_MIXED_EXACT, 1e-10, 18), ("f64_recon12", gf.GF_F64, None, 12),
-                ("mixed_exact_handoff_1e-10_recon12", gf.GF_MIXED_EXACT, 1e-10, 12)]
-        for name, mode, handoff, recon in runs:
+        # *_stall: hand-off when fp32 stops lowering theta (gf_set_mixed_stall(1.0), hand-off theta out of reach)
+        runs = [("f64", gf.GF_F64, None, 18, 0.0), ("mixed_handoff_1e-6", gf.GF_MIXED, 1e-6, 18, 0.0),
+                ("mixed_exact_handoff_1e-10", gf.GF_MIXED_EXACT, 1e-10, 18, 0.0), ("mixed_exact_stall", gf.GF_MIXED_EXACT, 1e-15, 18, 1.0),
+                ("f64_recon12", gf.GF_F64, None, 12, 0.0), ("mixed_exact_handoff_1e-10_recon12", gf.GF_MIXED_EXACT, 1e-10, 12, 0.0),
+                ("mixed_exact_stall_recon12", gf.GF_MIXED_EXACT, 1e-15, 12, 1.0)]
+        for name, mode, handoff, recon, stall in runs:
             fld = gf.GaugeField(DIMS, recon=recon, precisions=("f64",) if mode == gf.GF_F64 else ("f64", "f32"), device=dev)
             fld.pack(U64, gf.GF_F64)
             if mode == gf.GF_MIXED:
@@ -287,6 +289,7 @@ def run_ours(args):
                 fld.attach_transform(("f64", "f32"))
             if handoff:
                 fld.set_mixed_handoff(handoff)
+            fld.set_mixed_stall(stall)
             P0 = fld.plaquette(gf.GF_F64)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()

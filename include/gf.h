@@ -274,6 +274,14 @@ int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int block_thre
  * A hand-off below what fp32 can reach makes the fp32 phase run to max_iter. */
 int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff);
 
+/* Second hand-off criterion of the mixed-precision runs: how far fp32 sweeps can lower theta depends on the lattice
+ * and the field (about 3e-12 on the 32^4 bench field), so a fixed theta_handoff is either too cautious or never
+ * reached.  ratio in (0, 1]: the fp32 phase also ends at the first evaluation whose theta is above
+ * ratio x (theta of the previous evaluation), i.e. when fp32 has stopped lowering it at the rate asked for; with
+ * a small theta_handoff (e.g. 1e-15) the fp32 phase then runs exactly as long as it pays.  0 (default) = off.
+ * An early hand-off costs time only: the fp64 phase always finishes the run.  Errors: GF_EINVAL. */
+int gf_set_mixed_stall(gf_ctx* ctx, double ratio);
+
 /* Order in which the blocks of consecutive gf_sweep launches walk the lattice: 1 (default) =
  * zigzag, every other half-sweep runs from the last site to the first, so that a launch starts on
  * the links the previous one touched last and finds them in the L2 cache; 0 = always ascending.

@@ -72,6 +72,7 @@ def _load():
         "gf_set_solver_precision": (i32, [vp, i32]),
         "gf_set_traversal": (i32, [vp, i32]),
         "gf_set_fix_runahead": (i32, [vp, i32]),
+        "gf_set_mixed_stall": (i32, [vp, dbl]),
         "gf_set_reunitarize_every": (i32, [vp, i32]),
         "gf_set_mixed_handoff": (i32, [vp, dbl]),
         "gf_debug_philox": (i32, [vp, i32, vp, vp, vp]),
@@ -89,7 +90,7 @@ lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
            "gf_sweep gf_iterate gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
-           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_enable_peer gf_get_device gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_fix_runahead gf_set_reunitarize_every gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
+           "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_enable_peer gf_get_device gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_fix_runahead gf_set_mixed_stall gf_set_reunitarize_every gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
 
 
@@ -304,6 +305,10 @@ def gf_set_traversal(ctx, zigzag, check=True):
 
 def gf_set_reunitarize_every(ctx, iterations, check=True):
     return _rc(ctx, lib.gf_set_reunitarize_every(ctx, int(iterations)), check)
+
+
+def gf_set_mixed_stall(ctx, ratio, check=True):
+    return _rc(ctx, lib.gf_set_mixed_stall(ctx, float(ratio)), check)
 
 
 def gf_set_fix_runahead(ctx, blocks, check=True):

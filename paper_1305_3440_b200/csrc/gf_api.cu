@@ -42,6 +42,7 @@ struct gf_ctx {
     int n_active;               // entries of the list
     int mask_on;                // the sweeps cover the listed slices only
     double handoff;             // mixed precision: theta at which the fp32 phase hands over to fp64
+    double stall;               // mixed precision: the fp32 phase also ends when theta > stall * previous theta (0 = off)
     // slab decomposition along t (gf_set_slab): this context holds N_t local slices of a lattice nranks times as long
     int slab_rank, slab_n;
     void* prev_links[2];        // field of the slab below (per precision); NULL = own (one slab)
@@ -583,6 +584,8 @@ static ReduceTail measure_tail(const gf_ctx* ctx)
     t.counter = ctx->reduce_counter;
     t.stop = nullptr;
     t.target = 0.0;
+    t.stall = 0.0;
+    t.prev = nullptr;
     if (ctx->gauge == GF_COULOMB) {
         const double Vs = (double)(ctx->V / ctx->dims[0]);
         t.combine = 0;
@@ -605,6 +608,8 @@ static ReduceTail lattice_tail(const gf_ctx* ctx, double scale)
     t.scale0 = t.scale1 = scale;
     t.stop = nullptr;
     t.target = 0.0;
+    t.stall = 0.0;
+    t.prev = nullptr;
     return t;
 }
 
@@ -733,7 +738,7 @@ static int enqueue_reunitarize(gf_ctx* ctx, int precision, const uint32_t* stop)
 // and rewinds its half-sweep counter to that block: field, iteration count and Philox stream are those of the loop
 // that waits for every theta (fix_phase below with runahead = 0).
 static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
-                              int check_every, int* it_io, double* theta_out)
+                              int check_every, int* it_io, double* theta_out, double stall)
 {
     struct Block { int it_end; uint32_t counter_end; uint64_t sweeps_end; } meta[kRunAhead];
     const int depth = ctx->runahead < kRunAhead ? ctx->runahead : kRunAhead;
@@ -744,6 +749,13 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
     ReduceTail rt = measure_tail(ctx);
     rt.stop = ctx->stop_dev;
     rt.target = target;
+    rt.stall = stall;
+    rt.prev = reinterpret_cast<double*>(ctx->reduce_counter + 2);      // third and fourth word of the 16 bytes: 8-byte aligned
+    double prev_theta = 0.0;
+    if (stall > 0.0) {
+        cudaError_t e0 = cudaMemsetAsync(rt.prev, 0, sizeof(double), ctx->stream);
+        if (e0 != cudaSuccess) return cuda_fail(ctx, e0, "fix loop");
+    }
     while (true) {
         while (err == GF_OK && head - tail < depth && it_enq < max_iter) {
             int n = check_every - (it_enq % check_every);
@@ -775,11 +787,13 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
         *theta_out = finish_measure(ctx, nullptr, nullptr, ctx->host_slots + (size_t)(kAsyncSlots + s) * slot_len);
         *it_io = meta[s].it_end;
         ++tail;
-        if (*theta_out < target) {
+        const bool stalled = stall > 0.0 && prev_theta > 0.0 && *theta_out > stall * prev_theta;
+        prev_theta = *theta_out;
+        if (*theta_out < target || stalled) {
             // the device took the same decision after this block: what is enqueued behind it is a no-op there
             ctx->counter = meta[s].counter_end;
             ctx->sweeps = meta[s].sweeps_end;
-            rc = GF_OK;
+            rc = *theta_out < target ? GF_OK : GF_NOT_CONVERGED;
             break;
         }
     }
@@ -790,14 +804,17 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
 }
 
 // One phase of the fix loop in one precision.  Returns GF_OK when theta < target was seen.
+// stall > 0 (fp32 phase of the mixed-precision runs): the phase also ends, with GF_NOT_CONVERGED, at the first evaluation
+// whose theta is above stall * (theta of the previous evaluation).
 static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
-                     int check_every, int* it_io, double* theta_out)
+                     int check_every, int* it_io, double* theta_out, double stall = 0.0)
 {
     int it = *it_io, since_reunit = 0;
+    double prev_theta = 0.0;
     int rc = GF_NOT_CONVERGED;
     const bool freeze = ctx->freeze_slices && ctx->gauge == GF_COULOMB;
     // slice freezing changes the launch list between evaluations on the host: that loop waits for every theta
-    if (!freeze && ctx->runahead > 0) return fix_phase_runahead(ctx, algo, omega, p, precision, target, max_iter, check_every, it_io, theta_out);
+    if (!freeze && ctx->runahead > 0) return fix_phase_runahead(ctx, algo, omega, p, precision, target, max_iter, check_every, it_io, theta_out, stall);
     if (freeze) {                            // every slice starts active (the stream is idle or ordered: pinned copy is free)
         cudaError_t e = cudaStreamSynchronize(ctx->stream);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "fix loop");
@@ -824,6 +841,8 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
         if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         *theta_out = finish_measure(ctx, nullptr, nullptr);
         if (*theta_out < target) { rc = GF_OK; break; }
+        if (stall > 0.0 && prev_theta > 0.0 && *theta_out > stall * prev_theta) break;
+        prev_theta = *theta_out;
         if (freeze) {
             // reading A17b: a slice below the target stops being swept; nothing that enters its F_t and
             // theta_t changes afterwards, so max_t theta_t above remains the stopping criterion
@@ -884,7 +903,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
     double theta = -1.0;
     if (precision == GF_MIXED) {
         const double t32 = theta_target > ctx->handoff ? theta_target : ctx->handoff;
-        rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta);
+        rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta, ctx->stall);
         if (rc < 0) return rc;
         int e = gf_cast(ctx, GF_F32, GF_F64);
         if (e != GF_OK) return e;
@@ -897,7 +916,7 @@ extern "C" int gf_fix_until(gf_ctx* ctx, int algo, double omega, double p, int p
         if (e == GF_OK) e = gf_transform_identity(ctx, GF_F32);
         if (e != GF_OK) return e;
         const double t32 = theta_target > ctx->handoff ? theta_target : ctx->handoff;
-        rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta);
+        rc = fix_phase(ctx, algo, omega, p, GF_F32, t32, max_iter, check_every, &it, &theta, ctx->stall);
         if (rc < 0) return rc;
         e = gf_transform_cast(ctx, GF_F32, GF_F64);
         if (e == GF_OK) e = gf_apply_transform(ctx, GF_F64, GF_F64, GF_F64);
@@ -1212,6 +1231,14 @@ extern "C" int gf_set_tuning(gf_ctx* ctx, int precision, int lanes_per_site, int
         return fail(ctx, GF_EINVAL, "lanes must be 0,1,2,4 and block 0, 64, 128 or 256");
     ctx->lanes[precision] = lanes_per_site;
     ctx->block[precision] = block_threads;
+    return GF_OK;
+}
+
+extern "C" int gf_set_mixed_stall(gf_ctx* ctx, double ratio)
+{
+    if (!ctx) return GF_EINVAL;
+    if (!(ratio >= 0.0 && ratio <= 1.0)) return fail(ctx, GF_EINVAL, "the stall ratio must be in [0, 1]");
+    ctx->stall = ratio;
     return GF_OK;
 }
 

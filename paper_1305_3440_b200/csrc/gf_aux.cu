@@ -90,7 +90,14 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
         __syncthreads();
         block_reduce2<OpMax>(a, b, res);
         if (threadIdx.x == 0) {
-            if (res[0] < tail.target) *tail.stop = 1u;
+            const double th = res[0];
+            bool stop = th < tail.target;
+            if (tail.stall > 0.0) {
+                const double prev = *tail.prev;
+                if (prev > 0.0 && th > tail.stall * prev) stop = true;
+                *tail.prev = th;
+            }
+            if (stop) *tail.stop = 1u;
             *tail.counter = 0u;
         }
         return;
@@ -115,7 +122,15 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
         const double th = res[1] * tail.scale1;
         out[0] = res[0] * tail.scale0;
         out[1] = th;
-        if (tail.stop != nullptr && th < tail.target) *tail.stop = 1u;    // the value the host compares, same comparison
+        if (tail.stop != nullptr) {                                       // the value the host compares, same comparisons
+            bool stop = th < tail.target;
+            if (tail.stall > 0.0) {
+                const double prev = *tail.prev;
+                if (prev > 0.0 && th > tail.stall * prev) stop = true;
+                *tail.prev = th;
+            }
+            if (stop) *tail.stop = 1u;
+        }
         *tail.counter = 0u;
     }
 }

@@ -46,6 +46,10 @@ struct ReduceTail {
     double scale0, scale1;  // normalisations applied to the two sums on the device
     uint32_t* stop;         // run-ahead fix loop: set *stop = 1 when theta (Coulomb: every theta_t) < target; NULL = no decision
     double target;
+    // stall > 0 (fp32 phase of the mixed-precision runs): also stop when theta > stall * (theta of the previous
+    // evaluation), i.e. when fp32 no longer lowers it; *prev holds the previous value (0 = none yet)
+    double stall;
+    double* prev;
 };
 
 // All kernels of the library ask for the same shared-memory carveout (a hint).  The pack / unpack kernels need a few

@@ -174,3 +174,6 @@ class GaugeField:
 
     def set_reunitarize_every(self, iterations):
         B.gf_set_reunitarize_every(self.ctx, iterations)
+
+    def set_mixed_stall(self, ratio):
+        B.gf_set_mixed_stall(self.ctx, ratio)

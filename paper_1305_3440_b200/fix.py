@@ -3,7 +3,7 @@
     python -m paper_1305_3440_b200.fix IN.npy [IN2.npy ...] --out-dir DIR [--gauge landau|coulomb]
            [--algo overrelax|relax|stochastic] [--omega 1.7] [--p 0.8] [--precision f64|f32|mixed|mixed-exact]
            [--recon 18|12] [--target 1e-12] [--max-iter 100000] [--check-every 10] [--seed 0] [--lanes 3]
-           [--reunitarize-every 0]
+           [--reunitarize-every 0] [--handoff THETA]
 
 IN.npy holds the links in the canonical layout of include/gf.h: a complex128 array of shape (Nt, Nz, Ny, Nx, 4, 3, 3).
 The fixed configuration is written to DIR/<name>.npy and one line per file reports iterations, theta, F and the drift of
@@ -40,6 +40,9 @@ def main(argv=None):
     ap.add_argument("--max-iter", type=int, default=100000)
     ap.add_argument("--check-every", type=int, default=10)
     ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--handoff", type=float, default=None,
+                    help="theta at which the fp32 phase of the mixed modes hands over (default: 1e-6 for mixed; for mixed-exact "
+                         "out of reach, the fp32 phase then ends when it stops lowering theta)")
     ap.add_argument("--reunitarize-every", type=int, default=0,
                     help="re-project the swept field onto SU(3) every so many iterations (fp32 runs of thousands of iterations)")
     ap.add_argument("--lanes", type=int, default=3)
@@ -67,6 +70,11 @@ def main(argv=None):
         if mode == gf.GF_MIXED_EXACT:
             f.attach_transform(("f64", "f32"))
         f.set_reunitarize_every(args.reunitarize_every)
+        if args.handoff is not None:
+            f.set_mixed_handoff(args.handoff)
+        elif mode == gf.GF_MIXED_EXACT:             # the result does not inherit fp32 rounding: stay in fp32 as long as it pays
+            f.set_mixed_handoff(1e-15)
+            f.set_mixed_stall(1.0)
 
     def work(f):
         P0 = f.plaquette(io_prec)

@@ -230,3 +230,45 @@ def test_reprojection_with_the_recorded_transformation(cuda_device, runahead):
     du, dd = oracle.unitarity_defect(W, dims)
     assert du < 1e-12 and dd < 1e-12
     assert np.abs(oracle.apply_transform(U, G, dims) - W).max() < 1e-11
+
+
+# ------------------------------------------------------------------------------ hand-off when fp32 stalls
+
+@pytest.mark.parametrize("mode,recon", [(gf.GF_MIXED_EXACT, 18), (gf.GF_MIXED_EXACT, 12), (gf.GF_MIXED, 18)])
+def test_mixed_precision_hands_over_when_fp32_stops_lowering_theta(cuda_device, mode, recon):
+    """gf_set_mixed_stall: with a target (1e-20) and a hand-off theta (1e-15) that fp32 can never reach the fp32 phase ends at the first
+    evaluation at which theta has not fallen; the fp64 phase finishes.  The run-ahead loop (decision on the device) and
+    the loop that waits take bitwise the same path; the result is fixed, in SU(3) and -- for GF_MIXED_EXACT -- has the
+    input's plaquette to 1e-12, all as judged by the oracle."""
+    dims = (6, 6, 4, 6)
+    U = gi.smooth_random_gauge(dims, 0.5, 33)
+    out = {}
+    for runahead in (0, 4):
+        fld = gf.GaugeField(dims, recon=recon, precisions=("f64", "f32"), device=cuda_device)
+        Ud = torch.from_numpy(U).to(cuda_device)
+        if mode == gf.GF_MIXED_EXACT:
+            fld.pack(Ud, gf.GF_F64)
+            fld.attach_transform(("f64", "f32"))
+        else:
+            fld.pack(Ud.to(torch.complex64), gf.GF_F32)
+        fld.set_mixed_handoff(1e-15)
+        fld.set_mixed_stall(1.0)
+        fld.set_fix_runahead(runahead)
+        rc, it, th = fld.fix_until(gf.GF_OVERRELAX, 1.7, 0.0, mode, 1e-20, 3000, 5)
+        out[runahead] = (rc, it, th, gf.gf_get_counter(fld.ctx), fld.unpack(gf.GF_F64).cpu().numpy())
+        fld.close()
+    a, b = out[0], out[4]
+    assert a[0] == b[0] == gf.GF_OK and a[1:4] == b[1:4] and np.array_equal(a[4], b[4])
+    # theta < 1e-20 is far below what fp32 reaches: the run can only have converged through the stall hand-off
+    assert b[1] < 3000 and b[2] < 1e-20
+    W = np.ascontiguousarray(b[4])
+    assert oracle.theta(W, dims) < 2e-20
+    du, dd = oracle.unitarity_defect(W, dims)
+    assert du < 1e-12 and dd < 1e-12
+    assert abs(oracle.plaquette(W, dims) - oracle.plaquette(U, dims)) < (1e-12 if mode == gf.GF_MIXED_EXACT else 1e-6)
+    with pytest.raises(gf.GFError):
+        f = gf.GaugeField(dims, precisions=("f64",), device=cuda_device)
+        try:
+            f.set_mixed_stall(1.5)
+        finally:
+            f.close()
