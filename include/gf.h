@@ -124,6 +124,40 @@ int gf_measure(gf_ctx* ctx, int precision, double* host_functional, double* host
 int gf_measure_async(gf_ctx* ctx, int precision, int slot);
 int gf_measure_collect(gf_ctx* ctx, int slot, double* host_functional, double* host_theta);
 
+/* ---- F and theta for callers that cannot allocate.
+ * Every other call needs a gf_ctx, and gf_init_lattice allocates (the context on the heap, pinned host memory,
+ * events) and is handed a workspace the caller had to allocate.  Some callers can do neither at the point where they
+ * want theta: a monitor hooked into another program's update loop once that program's pool allocator owns all of the
+ * GPU's memory (cudaMalloc then fails and the pool is not yours to ask), a job whose memory budget is fixed and checked
+ * at start-up, a latency-bound loop that cannot afford the device-wide synchronisation that cudaMalloc,
+ * cudaMallocHost and cudaFree bring with them.  gf_measure_static is for them: it calls no cudaMalloc / cudaFree /
+ * cudaMallocHost and no library routine that allocates, creates no context, and takes only inputs and outputs.
+ *
+ * What it computes: exactly what gf_measure computes (PAPER.md:39 eq. 2, :50-52 eq. 4-5; same kernels, same summation
+ * order, bitwise the same numbers) for the lattice `dims`, `gauge`, and the INTERNAL link field dev_links of
+ * `precision` (GF_F32 | GF_F64) and `recon` -- the buffer gf_pack / gf_sweep of a context with the same dims,
+ * precision and recon wrote (gf_storage_bytes, 16-byte aligned), treated as periodic (no slabs).  dev_links is only read.
+ * dev_out (DEVICE pointer, 8-byte aligned; mapped pinned host memory works too) receives, for GF_LANDAU, 2 doubles
+ * {F, theta}; for GF_COULOMB 2 N_t doubles {F_t, theta_t} for t = 0 .. N_t-1, interleaved.  Asynchronous on
+ * cuda_stream (a cudaStream_t of the CURRENT device, which must be the one holding dev_links and dev_out; NULL = the
+ * legacy default stream); the values are there once the stream has reached this point.
+ *
+ * Scratch: the partial sums between the two reduction kernels live in an array that is part of the library's device
+ * image, 1 114 368 bytes on every GPU that loads the library, held until the process exits.  Hence
+ *   - the limit: N_t * 2 * ceil(N_x N_y N_z / 256) <= GF_STATIC_MAX_BLOCKS (up to 8.4 M sites: 32^4, 48^4, 64^3 x 32,
+ *     32^3 x 64 fit; 64^4 does not).  Larger lattices are refused with GF_EINVAL before anything is launched;
+ *   - every call on a device uses the same array and finds what the last call left; the call clears the one word that
+ *     has to start at zero itself.  Two calls that OVERLAP on the GPU (different streams without an ordering between
+ *     them, or several host threads) race on it and both results are then garbage: order them (same stream, or events);
+ *   - the first call on each device looks up the array's device address (cudaGetSymbolAddress) and checks the device's
+ *     architecture; later calls only launch.  Make that first call during set-up, before any stream capture begins.
+ * Errors: GF_EINVAL (dims, enums, NULL or misaligned pointers, lattice beyond the limit) and GF_ECUDA for a device
+ * that is not sm_100, both found before anything is launched; GF_ECUDA for a failed launch.  There is no context to keep
+ * an error text: host_err (HOST buffer of host_err_len bytes, may be NULL / 0) receives it, NUL-terminated, "" on success. */
+enum { GF_STATIC_MAX_BLOCKS = 65536 };
+int gf_measure_static(const int dims[4], int gauge, int precision, int recon, const void* dev_links,
+                      double* dev_out, void* cuda_stream, char* host_err, size_t host_err_len);
+
 /* Iterates {gf_sweep(parity 0); gf_sweep(parity 1)} (= 1 iteration); after every
  * iteration that is a multiple of check_every (and after the last) evaluates theta (Coulomb:
  * max over slices) and stops when it is below theta_target.  precision GF_MIXED: fp32

@@ -12,7 +12,7 @@ from .binding import (  # noqa: F401
     GFError, lib, lib_path,
     gf_storage_bytes, gf_workspace_bytes, gf_init_lattice, gf_destroy, gf_last_error,
     gf_pack, gf_unpack, gf_load_host, gf_store_host, gf_sweep, gf_iterate, gf_functional, gf_theta,
-    gf_measure, gf_measure_async, gf_measure_collect, gf_fix_until, gf_set_rng, gf_get_counter, gf_reunitarize, gf_cast,
+    gf_measure, gf_measure_async, gf_measure_collect, gf_measure_static, GF_STATIC_MAX_BLOCKS, gf_fix_until, gf_set_rng, gf_get_counter, gf_reunitarize, gf_cast,
     gf_transform_bytes, gf_set_transform, gf_transform_identity, gf_transform_pack, gf_transform_unpack,
     gf_transform_cast, gf_apply_transform, gf_set_coulomb_mode, gf_coulomb_finish, gf_set_slice_mask, gf_set_slab, gf_enable_peer, gf_get_device,
     gf_plaquette, gf_unitarity, gf_set_tuning, gf_set_solver_precision, gf_set_traversal, gf_set_fix_runahead, gf_set_mixed_stall, gf_set_reunitarize_every, gf_set_mixed_handoff, gf_debug_philox, gf_launch_count,

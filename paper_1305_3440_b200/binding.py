@@ -48,6 +48,7 @@ def _load():
         "gf_measure": (i32, [vp, i32, dp, dp]),
         "gf_measure_async": (i32, [vp, i32, i32]),
         "gf_measure_collect": (i32, [vp, i32, dp, dp]),
+        "gf_measure_static": (i32, [ip, i32, i32, i32, vp, vp, vp, C.c_char_p, C.c_size_t]),
         "gf_fix_until": (i32, [vp, i32, dbl, dbl, i32, dbl, i32, i32, ip, dp]),
         "gf_transform_bytes": (C.c_size_t, [ip, i32, i32]),
         "gf_set_transform": (i32, [vp, vp, vp]),
@@ -88,7 +89,7 @@ def _load():
 
 lib = _load()
 EXPORTS = ("gf_storage_bytes gf_workspace_bytes gf_init_lattice gf_pack gf_unpack gf_load_host gf_store_host "
-           "gf_sweep gf_iterate gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
+           "gf_sweep gf_iterate gf_functional gf_theta gf_measure gf_measure_async gf_measure_collect gf_measure_static gf_fix_until gf_set_rng gf_get_counter gf_reunitarize "
            "gf_cast gf_transform_bytes gf_set_transform gf_transform_identity gf_transform_pack gf_transform_unpack "
            "gf_transform_cast gf_apply_transform gf_set_coulomb_mode gf_coulomb_finish gf_set_slice_mask gf_set_slab gf_enable_peer gf_get_device gf_plaquette gf_unitarity gf_set_tuning gf_set_solver_precision gf_set_traversal gf_set_fix_runahead gf_set_mixed_stall gf_set_reunitarize_every gf_set_mixed_handoff gf_debug_philox gf_launch_count gf_last_error "
            "gf_destroy").split()
@@ -193,6 +194,23 @@ def gf_measure_collect(ctx, slot, n_out=1, check=True):
     t = (C.c_double * n_out)()
     _rc(ctx, lib.gf_measure_collect(ctx, int(slot), f, t), check)
     return list(f), list(t)
+
+
+GF_STATIC_MAX_BLOCKS = 65536
+
+
+def gf_measure_static(dims, gauge, precision, recon, dev_links, dev_out, cuda_stream, check=True):
+    """F and theta of an internal link field without a context and without any allocation (include/gf.h): for callers
+    that must not call cudaMalloc / cudaMallocHost where they need theta.  dev_links: the storage a context of the same
+    dims / precision / recon packs and sweeps; dev_out: device pointer to 2 doubles (Landau: F, theta) or 2 * Nt
+    (Coulomb: F_t, theta_t interleaved).  Asynchronous on cuda_stream; calls that overlap on the GPU race on the
+    library's static scratch.  Returns the C return code; a negative one raises GFError with the call's own text."""
+    err = C.create_string_buffer(512)
+    rc = lib.gf_measure_static(_dims(dims), gauge, precision, recon, dev_links or None, dev_out or None,
+                               cuda_stream or None, err, len(err))
+    if rc < 0 and check:
+        raise GFError(rc, err.value.decode())
+    return rc
 
 
 def gf_fix_until(ctx, algo, omega, p, precision, theta_target, max_iter, check_every, check=True):

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libgf_b200.so")
-SOURCES = ["gf_sweep.cu", "gf_aux.cu", "gf_api.cu"]
+SOURCES = ["gf_sweep.cu", "gf_aux.cu", "gf_api.cu", "gf_static.cu"]
 HEADERS = [os.path.join(CSRC, "gf_device.cuh"), os.path.join(CSRC, "gf_internal.h"),
            os.path.join(INCLUDE, "gf.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -67,6 +67,44 @@ inline void uniform_carveout(Kernel kernel)
     }
 }
 
+// Geometry and measurement grid of a lattice from its extents alone, for entry points that work without a context
+// (gf_static.cu).  Must describe the lattice exactly as gf_init_lattice does: tests/test_zz_no_alloc.py compares the two.
+constexpr uint32_t kMeasureBlockThreads = 128;
+
+inline Geom make_geom(const int dims[4])
+{
+    Geom G;
+    G.nt = (uint32_t)dims[0];
+    G.nxh = (uint32_t)dims[1] / 2u;
+    G.ny = (uint32_t)dims[2];
+    G.nz = (uint32_t)dims[3];
+    G.Vh = (uint32_t)((uint64_t)dims[0] * dims[1] * dims[2] * dims[3] / 2u);
+    G.Vp[PREC_F32] = (G.Vh + Tile<float>::W - 1u) / Tile<float>::W * Tile<float>::W;
+    G.Vp[PREC_F64] = (G.Vh + Tile<double>::W - 1u) / Tile<double>::W * Tile<double>::W;
+    for (int mu = 0; mu < 4; ++mu) G.extent[mu] = (uint32_t)dims[mu];
+    G.stride[1] = 1;
+    G.stride[2] = G.nxh;
+    G.stride[3] = G.nxh * G.ny;
+    G.stride[0] = G.nxh * G.ny * G.nz;
+    G.div_nxh = make_fastdiv(G.nxh);
+    G.div_ny = make_fastdiv(G.ny);
+    G.div_nz = make_fastdiv(G.nz);
+    G.sh = G.Vh / G.nt;
+    G.div_sh = make_fastdiv(G.sh);
+    return G;
+}
+
+inline MeasureGrid make_measure_grid(const int dims[4])
+{
+    MeasureGrid mg;
+    mg.Sh = (uint32_t)((uint64_t)dims[1] * dims[2] * dims[3] / 2u);
+    mg.block = kMeasureBlockThreads;
+    mg.bpp = (mg.Sh + mg.block - 1u) / mg.block;
+    mg.slice_list = nullptr;
+    mg.n_listed = 0;
+    return mg;
+}
+
 // every launcher returns cudaGetLastError() after the launch
 // solver_f64: with fp32 storage, accumulate K(x) and run the SU(2) solves in fp64 registers
 cudaError_t launch_sweep(int precision, int solver_f64, int recon, int lanes, int block, const SweepArgs& a, cudaStream_t st);

@@ -52,6 +52,11 @@ class GaugeField:
         except Exception:
             pass
 
+    def storage(self, precision):
+        """The uint8 tensor holding the internal link field of `precision` (what the context borrows): for calls that
+        take the field itself rather than the context, such as binding.gf_measure_static."""
+        return self._bufs[precision]
+
     # ---- layout conversion
     def _canon(self, t):
         if t.dtype not in (torch.complex128, torch.complex64) or tuple(t.shape) != self.shape \
