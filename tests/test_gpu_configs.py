@@ -9,6 +9,7 @@ import torch
 import gf_inputs as gi
 import oracle
 import paper_1305_3440_b200 as gf
+from gpu_helpers import assert_pack_round_trip
 
 pytestmark = pytest.mark.gpu
 
@@ -137,6 +138,7 @@ def test_config4_64_4(cuda_device, prec):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 4, device=cuda_device).to(CDTYPE[prec])
     fld = gf.GaugeField(dims, precisions=(prec,), device=cuda_device)
     fld.pack(U, PREC[prec])
+    assert_pack_round_trip(fld, PREC[prec], U)      # sampled_sweep_check reads the oracle's input back from the device
     del U
     torch.cuda.empty_cache()
     P0 = fld.plaquette(PREC[prec])
@@ -276,6 +278,7 @@ def test_fig3_lattices_sampled_against_oracle(cuda_device, dims, prec, recon):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 48, device=cuda_device).to(CDTYPE[prec])
     fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
     fld.pack(U, PREC[prec])
+    assert_pack_round_trip(fld, PREC[prec], U)      # sampled_sweep_check reads the oracle's input back from the device
     del U
     torch.cuda.empty_cache()
     P0 = fld.plaquette(PREC[prec])

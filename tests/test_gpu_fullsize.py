@@ -4,7 +4,8 @@ storage variants (fp64 / fp32 x 18- / 12-real, default tuning -- this covers the
 point and the one-lane-per-site, lazy-third-row fp64/12 path at full size); one full stochastic Coulomb iteration of 32^3 x 64;
 the mixed-precision runs at 32^4 judged by the oracle; the Coulomb fix loop's iteration count on a 16 x 16^3 replica.
 The oracle is fed the field the device holds (unpacked after gf_pack: the fp32-rounded input, row 2 rebuilt for
-12-real storage) and runs on all host cores.  Tolerances are north_star's."""
+12-real storage) only after that field has been compared with the independently generated input
+(assert_pack_round_trip), and runs on all host cores.  Tolerances are north_star's."""
 import numpy as np
 import pytest
 import torch
@@ -12,6 +13,7 @@ import torch
 import gf_inputs as gi
 import oracle
 import paper_1305_3440_b200 as gf
+from gpu_helpers import assert_pack_round_trip
 
 pytestmark = pytest.mark.gpu
 
@@ -49,6 +51,7 @@ def test_32_4_full_field_against_oracle(cuda_device, prec, recon):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device).to(CDTYPE[prec])
     fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)     # default tuning = what bench.py times
     fld.pack(U, PREC[prec])
+    assert_pack_round_trip(fld, PREC[prec], U)
     Uo = held_by_device(fld, prec)                # the oracle that runs on freely (F / theta after 10 iterations)
     Us = Uo.copy() if prec == "f32" else Uo       # fp32: re-synchronised before every half-sweep (links)
     for parity in (0, 1):
@@ -81,6 +84,7 @@ def test_32_4_full_field_against_oracle(cuda_device, prec, recon):
         # fp32 storage, solves in fp64 registers: one whole iteration, no re-synchronisation
         fld.set_solver_precision(gf.GF_F64)
         fld.pack(U, PREC[prec])
+        assert_pack_round_trip(fld, PREC[prec], U)
         Uo = held_by_device(fld, prec)
         for parity in (0, 1):
             fld.sweep(parity, gf.GF_OVERRELAX, 1.7, 0.0, PREC[prec])
@@ -99,6 +103,7 @@ def test_config5_full_field_stochastic_coulomb_iteration(cuda_device, recon):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device)
     fld = gf.GaugeField(dims, gauge=gf.GF_COULOMB, recon=recon, precisions=("f64",), seed=2013, device=cuda_device)
     fld.pack(U, gf.GF_F64)
+    assert_pack_round_trip(fld, gf.GF_F64, U)
     del U
     Uo = held_by_device(fld, "f64")
     for parity in (0, 1):
@@ -142,6 +147,7 @@ def test_32_4_mixed_precision_judged_by_the_oracle(cuda_device, mode):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device)
     fld = gf.GaugeField(dims, precisions=("f64", "f32"), device=cuda_device)
     fld.pack(U, gf.GF_F64)
+    assert_pack_round_trip(fld, gf.GF_F64, U)
     U0 = held_by_device(fld, "f64")
     P0 = oracle.plaquette(U0, dims)
     if mode == "mixed":
@@ -176,6 +182,7 @@ def test_32_4_accumulated_transformation_full_field(cuda_device, prec, recon):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 1, device=cuda_device).to(CDTYPE[prec])
     fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
     fld.pack(U, PREC[prec])
+    assert_pack_round_trip(fld, PREC[prec], U)
     del U
     fld.attach_transform((prec,))
     Uo = held_by_device(fld, prec)
@@ -205,6 +212,7 @@ def test_64_4_full_field_one_iteration_against_oracle(cuda_device, prec, recon):
     U = gi.torch_smooth_random_gauge(dims, 0.6, 4, device=cuda_device)
     fld = gf.GaugeField(dims, recon=recon, precisions=(prec,), device=cuda_device)
     fld.pack(U, PREC[prec])
+    assert_pack_round_trip(fld, PREC[prec], U)                            # all 67 M links, byte offsets beyond 2^32 included
     del U
     torch.cuda.empty_cache()
     Uo = fld.unpack(PREC[prec], torch.complex128).cpu().numpy()           # what the device holds (row 2 rebuilt for 12-real)

@@ -458,7 +458,10 @@ def test_extreme_aspect_ratios(cuda_device, dims, prec, recon):
         fld.pack(to_device(U, prec, cuda_device), PREC[prec])
         Uo = oracle_input(U, prec)
         if recon == 12:
-            Uo = get_links(fld, prec)                             # row 2 as the device rebuilds it
+            Uin = Uo
+            Uo = get_links(fld, prec)                             # row 2 as the device rebuilds it ...
+            assert np.array_equal(Uo[..., :2, :], Uin[..., :2, :])              # ... from rows it holds bit for bit
+            assert np.abs(Uo[..., 2, :] - Uin[..., 2, :]).max() < (1e-14 if prec == "f64" else 1e-6)
         fld.iterate(1, algo, omega, p, PREC[prec])
         for parity in (0, 1):
             oracle.sweep(Uo, dims, parity, og, oalgo, omega, p, seed=11, half_sweep_counter=parity)
