@@ -73,7 +73,9 @@ int gf_init_lattice(gf_ctx** out, const int dims[4], int gauge, int recon, void*
                     void* dev_links_f32, void* dev_workspace, void* cuda_stream, uint64_t seed);
 
 /* canonical (device) -> internal field of `precision` (GF_F32 | GF_F64); converts the real type
- * if canonical_is_f64 differs.  Asynchronous on the context's stream. */
+ * if canonical_is_f64 differs.  Asynchronous on the context's stream.  The canonical buffer (here and in gf_unpack,
+ * gf_transform_pack / _unpack; the staging buffer of gf_load_host / gf_store_host) is moved as 16-byte vectors:
+ * a pointer that is not 16-byte aligned is refused with GF_EINVAL. */
 int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_f64, int precision);
 
 /* internal field of `precision` -> canonical (device); GF_RECON12 rebuilds row 2.  Asynchronous. */
@@ -310,8 +312,9 @@ int gf_set_mixed_handoff(gf_ctx* ctx, double theta_handoff);
 
 /* Second hand-off criterion of the mixed-precision runs: how far fp32 sweeps can lower theta depends on the lattice
  * and the field (about 3e-12 on the 32^4 bench field), so a fixed theta_handoff is either too cautious or never
- * reached.  ratio in (0, 1]: the fp32 phase also ends at the first evaluation whose theta is above
- * ratio x (theta of the previous evaluation), i.e. when fp32 has stopped lowering it at the rate asked for; with
+ * reached.  ratio in (0, 1]: the fp32 phase also ends at the first evaluation whose theta is not below
+ * ratio x (theta of the previous evaluation), i.e. when fp32 has stopped lowering it at the rate asked for (a theta
+ * that repeats bit for bit, the fixed point a deterministic run can reach at the rounding floor, counts as stalled); with
  * a small theta_handoff (e.g. 1e-15) the fp32 phase then runs exactly as long as it pays.  0 (default) = off.
  * An early hand-off costs time only: the fp64 phase always finishes the run.  Errors: GF_EINVAL. */
 int gf_set_mixed_stall(gf_ctx* ctx, double ratio);

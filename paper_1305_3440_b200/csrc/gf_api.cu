@@ -399,6 +399,7 @@ extern "C" int gf_pack(gf_ctx* ctx, const void* dev_canonical, int canonical_is_
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    if ((uintptr_t)dev_canonical & 15u) return fail(ctx, GF_EINVAL, "the canonical buffer must be 16-byte aligned (it is read and written as 16-byte vectors)");
     ctx->pending[precision] = 0;      // the field is overwritten: nothing left to apply
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_pack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
@@ -416,6 +417,7 @@ extern "C" int gf_unpack(gf_ctx* ctx, void* dev_canonical, int canonical_is_f64,
     rc = gf_coulomb_finish(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    if ((uintptr_t)dev_canonical & 15u) return fail(ctx, GF_EINVAL, "the canonical buffer must be 16-byte aligned (it is read and written as 16-byte vectors)");
     GF_SLAB_BEGIN(ctx);
     cudaError_t e = launch_unpack(precision, ctx->recon, ctx->links[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_unpack");
@@ -432,6 +434,7 @@ extern "C" int gf_load_host(gf_ctx* ctx, const void* host_canonical, int canonic
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (!host_canonical || !dev_staging) return fail(ctx, GF_EINVAL, "null host or staging pointer");
+    if ((uintptr_t)dev_staging & 15u) return fail(ctx, GF_EINVAL, "the staging buffer must be 16-byte aligned (it is read and written as 16-byte vectors)");
     cudaError_t e = cudaMemcpyAsync(dev_staging, host_canonical, canonical_bytes(ctx, canonical_is_f64), cudaMemcpyHostToDevice, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_load_host copy");
     return gf_pack(ctx, dev_staging, canonical_is_f64, precision);
@@ -443,6 +446,7 @@ extern "C" int gf_store_host(gf_ctx* ctx, void* host_canonical, int canonical_is
     int rc = check_prec(ctx, precision);
     if (rc) return rc;
     if (!host_canonical || !dev_staging) return fail(ctx, GF_EINVAL, "null host or staging pointer");
+    if ((uintptr_t)dev_staging & 15u) return fail(ctx, GF_EINVAL, "the staging buffer must be 16-byte aligned (it is read and written as 16-byte vectors)");
     rc = gf_unpack(ctx, dev_staging, canonical_is_f64, precision);
     if (rc) return rc;
     cudaError_t e = cudaMemcpyAsync(host_canonical, dev_staging, canonical_bytes(ctx, canonical_is_f64), cudaMemcpyDeviceToHost, ctx->stream);
@@ -787,7 +791,7 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
         *theta_out = finish_measure(ctx, nullptr, nullptr, ctx->host_slots + (size_t)(kAsyncSlots + s) * slot_len);
         *it_io = meta[s].it_end;
         ++tail;
-        const bool stalled = stall > 0.0 && prev_theta > 0.0 && *theta_out > stall * prev_theta;
+        const bool stalled = stall > 0.0 && prev_theta > 0.0 && *theta_out >= stall * prev_theta;
         prev_theta = *theta_out;
         if (*theta_out < target || stalled) {
             // the device took the same decision after this block: what is enqueued behind it is a no-op there
@@ -805,7 +809,7 @@ static int fix_phase_runahead(gf_ctx* ctx, int algo, double omega, double p, int
 
 // One phase of the fix loop in one precision.  Returns GF_OK when theta < target was seen.
 // stall > 0 (fp32 phase of the mixed-precision runs): the phase also ends, with GF_NOT_CONVERGED, at the first evaluation
-// whose theta is above stall * (theta of the previous evaluation).
+// whose theta is not below stall * (theta of the previous evaluation).
 static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precision, double target, int max_iter,
                      int check_every, int* it_io, double* theta_out, double stall = 0.0)
 {
@@ -841,7 +845,7 @@ static int fix_phase(gf_ctx* ctx, int algo, double omega, double p, int precisio
         if (e != GF_OK) { *it_io = it; if (freeze) ctx->mask_on = 0; return e; }
         *theta_out = finish_measure(ctx, nullptr, nullptr);
         if (*theta_out < target) { rc = GF_OK; break; }
-        if (stall > 0.0 && prev_theta > 0.0 && *theta_out > stall * prev_theta) break;
+        if (stall > 0.0 && prev_theta > 0.0 && *theta_out >= stall * prev_theta) break;
         prev_theta = *theta_out;
         if (freeze) {
             // reading A17b: a slice below the target stops being swept; nothing that enters its F_t and
@@ -1050,6 +1054,7 @@ extern "C" int gf_transform_pack(gf_ctx* ctx, const void* dev_canonical, int can
     int rc = check_transform_writable(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    if ((uintptr_t)dev_canonical & 15u) return fail(ctx, GF_EINVAL, "the canonical buffer must be 16-byte aligned (it is read and written as 16-byte vectors)");
     cudaError_t e = launch_transform_pack(precision, ctx->recon, ctx->gtrans[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_pack");
     ctx->launches += 1;
@@ -1062,6 +1067,7 @@ extern "C" int gf_transform_unpack(gf_ctx* ctx, void* dev_canonical, int canonic
     int rc = check_transform(ctx, precision);
     if (rc) return rc;
     if (!dev_canonical) return fail(ctx, GF_EINVAL, "null canonical pointer");
+    if ((uintptr_t)dev_canonical & 15u) return fail(ctx, GF_EINVAL, "the canonical buffer must be 16-byte aligned (it is read and written as 16-byte vectors)");
     cudaError_t e = launch_transform_unpack(precision, ctx->recon, ctx->gtrans[precision], ctx->G, dev_canonical, canonical_is_f64, ctx->stream);
     if (e != cudaSuccess) return cuda_fail(ctx, e, "gf_transform_unpack");
     ctx->launches += 1;

@@ -55,6 +55,21 @@ __device__ __forceinline__ void block_reduce2(double a, double b, double* out)
 // them, again in a fixed order, into out[0], out[1].  `out` may be mapped pinned host memory: the host
 // reads finished results and does no arithmetic of the method.
 
+// The stopping decision of the run-ahead fix loop, taken by the last thread of the last reduction stage on the value
+// the host will read from pinned memory, with the comparisons the host makes (gf_api.cu, fix_phase_runahead):
+// theta below the target, or -- fp32 phase of the mixed-precision runs, tail.stall > 0 -- theta not below stall x the
+// previous evaluation's (>=: a bit-identical plateau at the rounding floor counts as stalled).
+__device__ __forceinline__ void decide_stop(const ReduceTail& tail, double th)
+{
+    bool stop = th < tail.target;
+    if (tail.stall > 0.0) {
+        const double prev = *tail.prev;
+        if (prev > 0.0 && th >= tail.stall * prev) stop = true;
+        *tail.prev = th;
+    }
+    if (stop) *tail.stop = 1u;
+}
+
 template <typename Op>
 __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32_t per_slice, const ReduceTail tail,
                                      double* __restrict__ out, const uint16_t* __restrict__ slice_list)
@@ -90,14 +105,7 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
         __syncthreads();
         block_reduce2<OpMax>(a, b, res);
         if (threadIdx.x == 0) {
-            const double th = res[0];
-            bool stop = th < tail.target;
-            if (tail.stall > 0.0) {
-                const double prev = *tail.prev;
-                if (prev > 0.0 && th > tail.stall * prev) stop = true;
-                *tail.prev = th;
-            }
-            if (stop) *tail.stop = 1u;
+            decide_stop(tail, res[0]);
             *tail.counter = 0u;
         }
         return;
@@ -122,15 +130,7 @@ __global__ void reduce_slices_kernel(const double* __restrict__ partials, uint32
         const double th = res[1] * tail.scale1;
         out[0] = res[0] * tail.scale0;
         out[1] = th;
-        if (tail.stop != nullptr) {                                       // the value the host compares, same comparisons
-            bool stop = th < tail.target;
-            if (tail.stall > 0.0) {
-                const double prev = *tail.prev;
-                if (prev > 0.0 && th > tail.stall * prev) stop = true;
-                *tail.prev = th;
-            }
-            if (stop) *tail.stop = 1u;
-        }
+        if (tail.stop != nullptr) decide_stop(tail, th);
         *tail.counter = 0u;
     }
 }

@@ -46,7 +46,7 @@ struct ReduceTail {
     double scale0, scale1;  // normalisations applied to the two sums on the device
     uint32_t* stop;         // run-ahead fix loop: set *stop = 1 when theta (Coulomb: every theta_t) < target; NULL = no decision
     double target;
-    // stall > 0 (fp32 phase of the mixed-precision runs): also stop when theta > stall * (theta of the previous
+    // stall > 0 (fp32 phase of the mixed-precision runs): also stop when theta >= stall * (theta of the previous
     // evaluation), i.e. when fp32 no longer lowers it; *prev holds the previous value (0 = none yet)
     double stall;
     double* prev;
@@ -60,10 +60,16 @@ constexpr int kCarveoutPercent = 25;
 template <typename Kernel>
 inline void uniform_carveout(Kernel kernel)
 {
-    static bool done = false;          // per kernel instantiation; a benign race at worst sets it twice
-    if (!done) {
+    // cudaFuncSetAttribute acts on the CURRENT device only: one bit per device ordinal and kernel instantiation, so that
+    // every GPU of a multi-device process (slabs.SlabSet) gets the hint, not just the first one used.  A benign race at
+    // worst sets an attribute twice.
+    static uint64_t done = 0;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return;
+    const uint64_t bit = uint64_t(1) << (dev & 63);
+    if (!(done & bit)) {
         cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, kCarveoutPercent);
-        done = true;
+        done |= bit;
     }
 }
 

@@ -87,8 +87,8 @@ def main(argv=None):
 
     def fill(i, buf):                               # runs in the lane's thread: file I/O overlaps the other lanes' sweeps
         a = np.load(args.inputs[i])
-        if tuple(a.shape) != tuple(first.shape):
-            raise SystemExit("%s: shape %r differs from %r" % (args.inputs[i], a.shape, first.shape))
+        if tuple(a.shape) != tuple(first.shape):         # an ordinary exception: the pipeline hands it to the caller's thread
+            raise ValueError("%s: shape %r differs from %r" % (args.inputs[i], a.shape, first.shape))
         buf.copy_(torch.from_numpy(np.ascontiguousarray(a)).to(cdtype))
 
     def drain(i, buf, result):
@@ -97,7 +97,12 @@ def main(argv=None):
         return out, result
 
     status = 0
-    for path, (out, (rc, it, th, F, dP)) in zip(args.inputs, pipe.process_stream(len(args.inputs), fill, work, drain, io_prec, cdtype)):
+    try:
+        done = pipe.process_stream(len(args.inputs), fill, work, drain, io_prec, cdtype)
+    except ValueError as e:                         # a bad input file: stop with its message (results already drained stay on disk)
+        pipe.close()
+        raise SystemExit(str(e))
+    for path, (out, (rc, it, th, F, dP)) in zip(args.inputs, done):
         print("%s -> %s: %s after %d iterations, theta = %.3e, F = %.9f, plaquette drift %.1e" % (
             path, out, "converged" if rc == gf.GF_OK else "NOT converged", it, th, F, dP), flush=True)
         status |= 0 if rc == gf.GF_OK else 1

@@ -86,8 +86,8 @@ class HostPipeline:
                     f.store_host(hosts[i], precision)       # synchronises the lane's stream
                     results[i] = r
                     self.done_at.append(time.perf_counter())
-            except Exception as e:                          # re-raised in the caller's thread
-                errors.append(e)
+            except BaseException as e:                      # re-raised in the caller's thread (SystemExit from a callback too:
+                errors.append(e)                            # threading would swallow it and the item would just be missing)
 
         threads = [threading.Thread(target=lane, args=(k,)) for k in range(min(len(fields), len(hosts)))]
         for t in threads:
@@ -122,7 +122,7 @@ class HostPipeline:
                     f.store_host(buf, precision)
                     out[i] = drain(i, buf, r)
                     self.done_at.append(time.perf_counter())
-            except Exception as e:
+            except BaseException as e:
                 errors.append(e)
 
         threads = [threading.Thread(target=lane, args=(k,)) for k in range(min(len(fields), int(n_items)))]

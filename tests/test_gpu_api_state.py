@@ -79,3 +79,28 @@ def test_a_context_belongs_to_its_device(cuda_device):
     assert B.lib.gf_enable_peer(fld.ctx, 4096) == gf.GF_EINVAL
     assert B.lib.gf_enable_peer(fld.ctx, -1) == gf.GF_EINVAL
     fld.close()
+
+
+def test_misaligned_canonical_buffers_are_refused_before_any_launch(cuda_device):
+    """pack / unpack move the canonical side as 16-byte vectors: a canonical or staging pointer at an odd offset (a tensor
+    view, say) is answered with GF_EINVAL on the host instead of a misaligned-address fault that would poison the CUDA
+    context; the field is untouched and the context keeps working."""
+    dims = (4, 4, 4, 4)
+    U = torch.from_numpy(gi.smooth_random_gauge(dims, 0.4, 9)).to(cuda_device)
+    fld = gf.GaugeField(dims, precisions=("f64",), device=cuda_device, staging=True)
+    fld.attach_transform(("f64",))
+    fld.pack(U, gf.GF_F64)
+    n = U.numel() * 16
+    raw = torch.zeros(n + 64, dtype=torch.uint8, device=cuda_device)
+    odd = raw.data_ptr() + 8                                               # 8-byte aligned only
+    host = torch.zeros(U.shape, dtype=torch.complex128).pin_memory()
+    for rc in (B.lib.gf_pack(fld.ctx, odd, 1, gf.GF_F64), B.lib.gf_unpack(fld.ctx, odd, 1, gf.GF_F64),
+               B.lib.gf_load_host(fld.ctx, host.data_ptr(), 1, gf.GF_F64, odd),
+               B.lib.gf_store_host(fld.ctx, host.data_ptr(), 1, gf.GF_F64, odd),
+               B.lib.gf_transform_pack(fld.ctx, odd, 1, gf.GF_F64), B.lib.gf_transform_unpack(fld.ctx, odd, 1, gf.GF_F64)):
+        assert rc == gf.GF_EINVAL
+        assert "16-byte aligned" in gf.gf_last_error(fld.ctx)
+    torch.cuda.synchronize(cuda_device)                                    # nothing faulted
+    assert torch.equal(fld.unpack(gf.GF_F64), U)                           # and nothing was written
+    assert float(host.abs().max()) == 0.0
+    fld.close()

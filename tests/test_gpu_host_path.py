@@ -137,6 +137,32 @@ def test_host_pipeline_surfaces_errors(cuda_device):
     pipe.close()
 
 
+def test_errors_raised_in_a_lane_thread_reach_the_caller(cuda_device, tmp_path):
+    """A callback that fails inside a lane's thread -- with an ordinary exception or with SystemExit, which threading
+    would swallow -- is re-raised by the pipeline; the command line turns a file of the wrong shape into an exit message
+    naming the file instead of tripping over the missing result."""
+    from paper_1305_3440_b200 import fix
+    from paper_1305_3440_b200.pipeline import HostPipeline
+    dims = (4, 4, 4, 4)
+    pipe = HostPipeline(dims, precisions=("f64",), lanes=2, device=cuda_device)
+
+    def fill(i, buf):
+        if i == 1:
+            raise SystemExit("item 1 cannot be read")
+        buf.copy_(torch.from_numpy(gi.smooth_random_gauge(dims, 0.4, 5)))
+
+    with pytest.raises(SystemExit, match="item 1"):
+        pipe.process_stream(3, fill, lambda f: f.iterate(1, gf.GF_OVERRELAX, 1.7, 0.0, gf.GF_F64), lambda i, buf, r: i)
+    pipe.close()
+    paths = []
+    for i, d in enumerate(((4, 4, 4, 4), (4, 4, 4, 6))):
+        p = tmp_path / ("cfg%d.npy" % i)
+        np.save(p, gi.smooth_random_gauge(d, 0.4, 50 + i))
+        paths.append(str(p))
+    with pytest.raises(SystemExit, match="cfg1.npy.*differs"):
+        fix.main(paths + ["--out-dir", str(tmp_path / "fixed"), "--target", "1e-10", "--lanes", "2", "--device", str(cuda_device)])
+
+
 @pytest.mark.parametrize("gauge,algo,precision,recon", [("landau", "overrelax", "f64", 18), ("landau", "overrelax", "mixed-exact", 12),
                                                         ("coulomb", "stochastic", "f64", 18), ("landau", "overrelax", "mixed", 18)])
 def test_command_line_fixes_an_ensemble_of_files(cuda_device, tmp_path, gauge, algo, precision, recon):

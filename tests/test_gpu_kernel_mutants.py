@@ -7,7 +7,8 @@ THERE (nvcc, only the translation units that changed) and a subset of the parity
 ``pytest -x``; the run must fail.  The unmutated copy must pass (control).  All mutants keep every memory access inside
 the buffers (arithmetic, signs, which draw / which neighbour inside the lattice), so a mutant cannot fault the GPU.
 Off by default because it rebuilds the library a dozen times (about five minutes on the GPU box); the outcome of a run
-is recorded in profiles/r2_kernel_mutants.md.
+is recorded in profiles/r3_kernel_mutants.md.  What needs no rebuild is checked on every run, without a GPU: every
+fragment of the list occurs exactly once in the current sources (a list that has gone stale fails at once).
 """
 import os
 import shutil
@@ -18,17 +19,15 @@ from concurrent.futures import ThreadPoolExecutor
 
 import pytest
 
-pytestmark = pytest.mark.gpu
-
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 PKG = "paper_1305_3440_b200"
 TEST_FILES = ["conftest.py", "test_gpu_parity.py", "test_gpu_checkers.py", "test_gpu_coulomb.py", "test_gpu_transform.py",
-              "test_gpu_fix_runahead.py", "curand_philox_ref.cu"]
+              "test_gpu_fix_runahead.py", "curand_philox_ref.cu", "gpu_helpers.py"]
 # the subset that is run against every mutant (the whole of these files takes about a minute)
 SELECT = ("pack_unpack or unit_links or one_sweep or ten_sweeps or stochastic_counter or philox or config1_fix or random_small or "
           "extreme or unitarity_matches or reunitarize or cast_f32 or deferred_temporal_links_one or slice_mask or "
           "accumulated_transformation or apply_transform or transformation_reproduces or mixed_exact or runahead_equals or "
-          "runahead_coulomb")
+          "runahead_coulomb or hands_over or reprojection_keeps")
 
 # (name, file under csrc/, exact fragment (must occur exactly once), replacement)
 MUTANTS = [
@@ -55,7 +54,17 @@ MUTANTS = [
     ("theta keeps the trace", "gf_aux.cu", "const double d = GF_IM(M, a, a) - tr3;", "const double d = GF_IM(M, a, a);"),
     ("F from a wrong diagonal entry", "gf_aux.cu", "F += (double)Uf[0] + (double)Uf[8] + (double)Uf[16];", "F += (double)Uf[0] + (double)Uf[8] + (double)Uf[14];"),
     ("unitarity checker returns zero", "gf_aux.cu", "    block_reduce2<OpMax>(dmax, detmax, partials + partial_slot(mg));", "    block_reduce2<OpMax>(0.0 * dmax, 0.0 * detmax, partials + partial_slot(mg));"),
-    ("device-side stop decision inverted", "gf_aux.cu", "if (tail.stop != nullptr && th < tail.target) *tail.stop = 1u;", "if (tail.stop != nullptr && th > tail.target) *tail.stop = 1u;"),
+    ("device-side stop decision inverted", "gf_aux.cu", "    bool stop = th < tail.target;", "    bool stop = th > tail.target;"),
+    # hand-off when fp32 stalls (gf_set_mixed_stall): the device's decision must be the host's
+    ("stall ratio compared the wrong way on the device", "gf_aux.cu", "if (prev > 0.0 && th >= tail.stall * prev) stop = true;", "if (prev > 0.0 && th <= tail.stall * prev) stop = true;"),
+    ("stall: previous theta never recorded on the device", "gf_aux.cu", "        *tail.prev = th;\n", "\n"),
+    ("stall tested at the first evaluation (no previous theta)", "gf_aux.cu", "if (prev > 0.0 && th >= tail.stall * prev) stop = true;", "if (th >= tail.stall * prev) stop = true;"),
+    ("stall ratio compared the wrong way on the host (run-ahead loop)", "gf_api.cu", "prev_theta > 0.0 && *theta_out >= stall * prev_theta;", "prev_theta > 0.0 && *theta_out <= stall * prev_theta;"),
+    # re-projection inside the fix loop (gf_set_reunitarize_every)
+    ("re-projection skipped by the run-ahead loop", "gf_api.cu", "err = enqueue_reunitarize(ctx, precision, ctx->stop_dev);", "err = GF_OK;"),
+    ("re-projection skipped by the waiting loop", "gf_api.cu", "int er = enqueue_reunitarize(ctx, precision, nullptr);", "int er = GF_OK;"),
+    ("re-projection in the fix loop copies without projecting", "gf_api.cu", "ctx->links[precision], ctx->links[precision], ctx->G, 1, 8, ctx->stream, stop);",
+     "ctx->links[precision], ctx->links[precision], ctx->G, 0, 8, ctx->stream, stop);"),
     # path-specific: the lazy third rows of fp64 / 12-real, the recorded transformation, the fp32 / 18-real tail, deferred
     # temporal links, eq. 3 applied to a field, the re-projection, the plaquette, the Coulomb sums
     ("lazy third row of the forward link enters K with the wrong sign", "gf_sweep.cu",
@@ -108,9 +117,21 @@ def _run_tests(tmp):
     return r.returncode, (failed[0] if failed else r.stdout.strip().splitlines()[-1] if r.stdout.strip() else r.stderr[-200:])
 
 
+def test_the_mutant_list_is_current():
+    """No GPU, no rebuild: every fragment occurs exactly once in today's sources, and its replacement differs."""
+    stale = []
+    for name, fname, old, new in MUTANTS:
+        n = open(os.path.join(ROOT, PKG, "csrc", fname)).read().count(old)
+        if n != 1 or old == new:
+            stale.append("%s: fragment occurs %d times in %s" % (name, n, fname))
+    assert not stale, stale
+    assert len({m[0] for m in MUTANTS}) == len(MUTANTS)
+
+
+@pytest.mark.gpu
 def test_every_kernel_mutant_fails_a_gpu_parity_test():
     if os.environ.get("GF_KERNEL_MUTANTS") != "1":
-        pytest.skip("opt-in (GF_KERNEL_MUTANTS=1): rebuilds the library once per mutant; last run: profiles/r2_kernel_mutants.md")
+        pytest.skip("opt-in (GF_KERNEL_MUTANTS=1): rebuilds the library once per mutant; last run: profiles/r3_kernel_mutants.md")
     jobs = [("control (unmutated)", None, None, None)] + MUTANTS
     with ThreadPoolExecutor(max_workers=max(1, min(5, (os.cpu_count() or 4) // 3))) as ex:
         built = list(ex.map(lambda j: _build(*j), jobs))
