@@ -220,6 +220,8 @@ def fix_until_freeze(U, dims, algo=OVERRELAX, omega=1.0, p=0.0, seed=0, first_co
     conv = C.c_int()
     it = load().oracle_fix_until_freeze(_field(U, dims), _dims(dims), algo, omega, p, int(seed), int(first_counter),
                                         theta_target, max_iter, check_every, _dbl(th), fr, C.byref(conv))
+    if it < 0:
+        raise ValueError("oracle fix loops hold per-slice state for at most 4096 time slices, got %d" % dims[0])
     return it, th, np.array(list(fr)), bool(conv.value)
 
 
@@ -231,6 +233,8 @@ def fix_until(U, dims, gauge=LANDAU, algo=OVERRELAX, omega=1.0, p=0.0, seed=0, f
     it = load().oracle_fix_until(_field(U, dims), _dims(dims), gauge, algo, omega, p, int(seed),
                                  int(first_counter), theta_target, max_iter, check_every,
                                  C.byref(th), C.byref(conv))
+    if it < 0:
+        raise ValueError("oracle fix loops hold per-slice state for at most 4096 time slices, got %d" % dims[0])
     return it, th.value, bool(conv.value)
 
 

@@ -495,6 +495,8 @@ int oracle_fix_until(cd *U, const int dims[4], int gauge, int algo, double omega
     const int nslice = gauge == ORACLE_COULOMB ? dims[0] : 1;
     double theta = INFINITY;
     *converged = 0;
+    *theta_out = INFINITY;
+    if (nslice > 4096) return -1;              /* th[] holds one theta_t per time slice: refuse, do not overrun */
     int it = 0;
     if (check_every < 1) check_every = 1;
     while (it < max_iter) {
@@ -524,8 +526,9 @@ int oracle_fix_until_freeze(cd *U, const int dims[4], int algo, double omega, do
 {
     int active[4096];
     const int nt = dims[0];
-    for (int t = 0; t < nt; ++t) { active[t] = 1; frozen_at[t] = 0; }
     *converged = 0;
+    if (nt > 4096) return -1;                  /* active[] holds one flag per time slice: refuse, do not overrun */
+    for (int t = 0; t < nt; ++t) { active[t] = 1; frozen_at[t] = 0; }
     int it = 0;
     if (check_every < 1) check_every = 1;
     while (it < max_iter) {

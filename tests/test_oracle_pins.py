@@ -676,3 +676,19 @@ def test_fix_until_freeze_fixes_every_slice_as_the_unfrozen_run_does():
     it_plain, _, conv_plain = oracle.fix_until(U0.copy(), dims, gauge=oracle.COULOMB, theta_target=1e-12, max_iter=3000,
                                                check_every=1, **kw)
     assert conv_plain and it == it_plain
+
+
+def test_fix_loops_refuse_more_time_slices_than_their_per_slice_state_holds():
+    """oracle_fix_until / oracle_fix_until_freeze keep theta_t / the active flags in arrays of 4096 entries (the
+    library's own limit on N_t): a longer lattice is refused instead of overrunning them; 4096 itself still runs."""
+    long = (4098, 2, 2, 2)
+    U = gi.unit_links(long)
+    with pytest.raises(ValueError):
+        oracle.fix_until(U, long, oracle.COULOMB, max_iter=1)
+    with pytest.raises(ValueError):
+        oracle.fix_until_freeze(U, long, max_iter=1)
+    ok = (4096, 2, 2, 2)
+    it, th, conv = oracle.fix_until(gi.unit_links(ok), ok, oracle.COULOMB, max_iter=3)
+    assert it == 1 and th == 0.0 and conv                  # unit links are fixed: the first evaluation stops
+    it, th_t, frozen_at, conv = oracle.fix_until_freeze(gi.unit_links(ok), ok, max_iter=3)
+    assert it == 1 and conv and (frozen_at == 1).all() and (th_t == 0.0).all()
