@@ -37,25 +37,35 @@ METRIC = "overrelaxation site-updates/s at 32^4"
 VARIANTS = {            # name: (precision key, recon, bytes per real)
     "f64-18": ("f64", 18, 8), "f64-12": ("f64", 12, 8),
     "f32-18": ("f32", 18, 4), "f32-12": ("f32", 12, 4),
+    # fp32 storage with the opt-in all-fp32 solver (gf_set_solver_precision(GF_F32)): faster, but one iteration at 32^4
+    # ends 1.08e-5 from the oracle, above north_star's 1e-5; the plain f32-* rows are the library default (K(x) and the
+    # SU(2) solves in fp64 registers), which meets it
+    "f32-18/solver-f32": ("f32", 18, 4), "f32-12/solver-f32": ("f32", 12, 4),
 }
 
 
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.json")
+def solver_of(name):
+    """Arithmetic of K(x) and the SU(2) solves for a variant: the storage precision for fp64, fp64 registers for fp32
+    storage by default, fp32 for the */solver-f32 rows."""
+    return "f32" if name.endswith("/solver-f32") else "f64"
+
+
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r3_traffic.json")
 
 
 def ncu_traffic(variant):
     """dram__bytes_read.sum + dram__bytes_write.sum per sweep launch at 32^4 from the committed `ncu --set full`
-    summary (written by paper_1305_3440_b200/profile_traffic.py; command in profiles/r2_sweep_variants_ncu.md).
+    summary (averages of the ncu metrics over the captured sweep launches; commands in profiles/r3_sweep_variants_ncu.md).
     Valid only for the kernel sources it was captured at: returns (None, why, None) when they have changed since.
     Third value: the same sum from the single-pass capture of consecutive launches without ncu's L2 flush, if on record."""
     try:
         from paper_1305_3440_b200.build import source_hash
         doc = json.load(open(TRAFFIC_FILE))
         if doc.get("source_hash") != source_hash():
-            return None, "profiles/r2_traffic.json was captured at sources %s, the library is at %s" % (doc.get("source_hash"), source_hash()), None
+            return None, "profiles/r3_traffic.json was captured at sources %s, the library is at %s" % (doc.get("source_hash"), source_hash()), None
         v = doc["variants"][variant]
         warm = v.get("in_run", {}).get("traffic_bytes")
-        return float(v["traffic_bytes"]), "profiles/r2_traffic.json (ncu --set full, sources %s)" % doc["source_hash"], warm
+        return float(v["traffic_bytes"]), "profiles/r3_traffic.json (ncu --set full, sources %s)" % doc["source_hash"], warm
     except Exception as e:                                      # missing file or variant: no claim
         return None, "no ncu capture on record (%s)" % type(e).__name__, None
 
@@ -132,6 +142,8 @@ def run_ours(args):
         prec = gf.GF_F64 if pkey == "f64" else gf.GF_F32
         cdtype = torch.complex128 if pkey == "f64" else torch.complex64
         fld = gf.GaugeField(DIMS, recon=recon, precisions=(pkey,), device=dev, staging=with_e2e)
+        if name.endswith("/solver-f32"):
+            fld.set_solver_precision(gf.GF_F32)
         Uc = U64.to(cdtype).contiguous()
         fld.pack(Uc, prec)
         n_blocks = args.iters // args.check
@@ -174,6 +186,7 @@ def run_ours(args):
         bytes_per_launch = (V // 2) * 16 * recon * B
         achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
         traffic, traffic_src, traffic_warm = ncu_traffic(name)
+        solver = solver_of(name)
         out = {
             "value": world * V * args.iters * steps / (ms_total * 1e-3),
             "ms_per_step": ms_total / steps,
@@ -195,7 +208,7 @@ def run_ours(args):
                          # copy behind `peak` pushes 2 x peak through them.
                          "l2_slice_GBs": ((bytes_per_launch + traffic_warm) / (kern_ms * 1e-3) / 1e9) if traffic_warm else None,
                          "l2_slice_frac_of_copy": ((bytes_per_launch + traffic_warm) / (kern_ms * 1e-3) / 1e9 / (2 * peak)) if traffic_warm else None,
-                         "kernel": "gf::sweep_kernel<%s,recon%d>" % (pkey, recon),
+                         "kernel": "gf::sweep_kernel<storage %s, solver %s, recon%d>" % (pkey, solver, recon),
                          "bytes_per_launch": bytes_per_launch, "avg_launch_ms": kern_ms, "peak_source": peak_src,
                          "frac_of_8TBs_nominal": achieved / 8000.0},
             "final_F": F[0], "final_theta": th[0],
@@ -264,12 +277,14 @@ def run_ours(args):
         for name in VARIANTS:
             if name == args.variant:
                 continue
-            r = bench_variant(name, max(1, args.steps // 3), 3, False)
+            # the same steps, warm-up, timing and clock sampling as the headline variant (no end-to-end leg)
+            r = bench_variant(name, args.steps, args.warmup, False)
             variants[name] = {"site_updates_per_s": r["value"], "gflops_nominal": r["value"] * FLOP_PER_SITE_UPDATE / 1e9,
-                              "roofline_GBs": r["roofline"]["achieved"], "roofline_frac": r["roofline"]["frac"],
-                              "dram_frac": r["roofline"]["dram_frac"], "dram_frac_in_run": r["roofline"]["dram_frac_in_run"],
-                              "l2_slice_GBs": r["roofline"]["l2_slice_GBs"], "avg_launch_ms": r["roofline"]["avg_launch_ms"],
-                              "sm_mhz": r["clocks"]["sm_mhz"]}
+                              "storage": name.split("/")[0], "solver": solver_of(name),
+                              "meets_north_star_link_tolerance_at_32^4": not name.endswith("/solver-f32"),
+                              "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"],
+                              "gpu_launches": r["gpu_launches"], "clocks": r["clocks"], "roofline": r["roofline"],
+                              "final_F": r["final_F"], "final_theta": r["final_theta"]}
 
     # Time to solution (BASELINE.json configs[2]: "fp32, mixed and fp64"): gf_fix_until to theta < 1e-12 on the
     # same 32^4 input, theta every 10 iterations.  Context for the SP/MP/DP reading of the metric, not the headline.
@@ -299,6 +314,21 @@ def run_ours(args):
             ms = e0.elapsed_time(e1)
             fixes[name] = {"converged": rc == gf.GF_OK, "iterations": it, "theta": th, "seconds": ms * 1e-3,
                            "site_updates_per_s": V * it / (ms * 1e-3), "plaquette_drift": fld.plaquette(gf.GF_F64) - P0}
+            if name == "mixed_handoff_1e-6":
+                # MP of the metric (BASELINE.json configs[2], "fp32 sweeps to theta < 1e-6, then fp64"): how the iterations
+                # split.  The fp32 phase IS gf_fix_until(GF_F32, 1e-6) on the same input (same kernels, deterministic), so
+                # its length is measured by running exactly that, outside the timed run above.
+                fld.pack(U64.to(torch.complex64), gf.GF_F32)
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a0.record()
+                rc32, it32, th32 = fld.fix_until(gf.GF_OVERRELAX, OMEGA, 0.0, gf.GF_F32, 1e-6, 50000, 10)
+                a1.record()
+                torch.cuda.synchronize()
+                ms32 = a0.elapsed_time(a1)
+                fixes[name].update({"fp32_phase_iterations": it32, "fp64_phase_iterations": it - it32,
+                                    "fp32_phase_seconds": ms32 * 1e-3, "fp32_phase_theta": th32,
+                                    "fp32_phase_site_updates_per_s": V * it32 / (ms32 * 1e-3),
+                                    "fp64_phase_site_updates_per_s": V * (it - it32) / max(1e-9, (ms - ms32) * 1e-3)})
             fld.close()
             del fld
             torch.cuda.empty_cache()

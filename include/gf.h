@@ -346,10 +346,12 @@ int gf_set_reunitarize_every(gf_ctx* ctx, int iterations);
 int gf_set_fix_runahead(gf_ctx* ctx, int blocks);
 
 /* Arithmetic of the per-site solver when the STORAGE is fp32 (gf_sweep with GF_F32): K(x) is
- * accumulated and the three SU(2) solves run in solver_precision: GF_F32 (everything in fp32),
- * GF_F64 (fp64 registers: no extra memory traffic, ~15 % more time, removes the amplification of
- * fp32 rounding at sites whose SU(2) projection |v| is small), or GF_SOLVER_AUTO (the default:
- * GF_F64 for GF_STOCHASTIC, whose g -> g^2 step doubles that amplification, GF_F32 otherwise).
+ * accumulated and the three SU(2) solves run in solver_precision: GF_F64 (fp64 registers: no extra memory traffic;
+ * the links stay within 1e-5 of an fp64 computation on the same input over a whole iteration at 32^4, measured
+ * 2.2e-6), GF_F32 (everything in fp32: 10 % (18-real) to 20 % (12-real) faster at 32^4, but the fp32 rounding of K is
+ * amplified by |K| / |v| at sites whose SU(2) projection |v| is small -- one site in 5 x 10^5 of a 32^4 field ends
+ * 1.08e-5 away after one iteration, 1.4e-5 with GF_STOCHASTIC, whose g -> g^2 step doubles the amplification), or
+ * GF_SOLVER_AUTO (the default) = GF_F64.  Callers that only precondition with fp32 sweeps may prefer GF_F32.
  * The 3x3 products g U and U g^dagger are always formed in the storage precision.  No effect on
  * GF_F64 sweeps. */
 enum { GF_SOLVER_AUTO = -1 };

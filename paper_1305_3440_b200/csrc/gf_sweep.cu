@@ -270,12 +270,14 @@ __global__ void __launch_bounds__(256, 2) sweep_kernel_r128(const SweepConsts<T,
     sweep_body<T, TK, RECON, L, MODE>(P);
 }
 
-template <typename T, int RECON, int L> struct UseR128 {
-    static constexpr bool value = sizeof(T) == 4 && RECON == 18 && L == 2;
+// Only with the fp32 solver: K(x) and the SU(2) solves in fp64 registers do not fit 128 registers (the capped entry
+// spilled 10 loads + 10 stores per thread), that variant takes the uncapped entry like every other.
+template <typename T, typename TK, int RECON, int L> struct UseR128 {
+    static constexpr bool value = sizeof(T) == 4 && sizeof(TK) == 4 && RECON == 18 && L == 2;
 };
 
 template <typename Kernel, typename Consts>
-static void launch_pdl(Kernel kernel, uint32_t grid, int block, cudaStream_t st, const Consts& P)
+static cudaError_t launch_pdl(Kernel kernel, uint32_t grid, int block, cudaStream_t st, const Consts& P)
 {
     uniform_carveout(kernel);
     cudaLaunchConfig_t cfg = {};
@@ -288,16 +290,16 @@ static void launch_pdl(Kernel kernel, uint32_t grid, int block, cudaStream_t st,
     attr[0].val.programmaticStreamSerializationAllowed = GF_PDL;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kernel, P);
+    return cudaLaunchKernelEx(&cfg, kernel, P);
 }
 
 template <typename T, typename TK, int RECON, int L, int MODE>
-static void launch_kernel(uint32_t grid, int block, cudaStream_t st, const SweepConsts<T, TK>& P)
+static cudaError_t launch_kernel(uint32_t grid, int block, cudaStream_t st, const SweepConsts<T, TK>& P)
 {
-    if constexpr (UseR128<T, RECON, L>::value) {
-        launch_pdl(sweep_kernel_r128<T, TK, RECON, L, MODE>, grid, block, st, P);
+    if constexpr (UseR128<T, TK, RECON, L>::value) {
+        return launch_pdl(sweep_kernel_r128<T, TK, RECON, L, MODE>, grid, block, st, P);
     } else {
-        launch_pdl(sweep_kernel<T, TK, RECON, L, MODE>, grid, block, st, P);
+        return launch_pdl(sweep_kernel<T, TK, RECON, L, MODE>, grid, block, st, P);
     }
 }
 
@@ -325,13 +327,15 @@ static cudaError_t launch_one(int block, const SweepArgs& a, cudaStream_t st)
     if (P.n_sites == 0) return cudaSuccess;             // every slice frozen: nothing to launch
     const uint64_t threads = (uint64_t)P.n_sites * L;
     const uint32_t grid = (uint32_t)((threads + block - 1) / block);
+    cudaError_t e;
     if (a.gtrans && a.defer_temporal)
-        launch_kernel<T, TK, RECON, L, MODE_DEFER>(grid, block, st, P);
+        e = launch_kernel<T, TK, RECON, L, MODE_DEFER>(grid, block, st, P);
     else if (a.gtrans)
-        launch_kernel<T, TK, RECON, L, MODE_ACC>(grid, block, st, P);
+        e = launch_kernel<T, TK, RECON, L, MODE_ACC>(grid, block, st, P);
     else
-        launch_kernel<T, TK, RECON, L, MODE_PLAIN>(grid, block, st, P);
-    return cudaGetLastError();
+        e = launch_kernel<T, TK, RECON, L, MODE_PLAIN>(grid, block, st, P);
+    const cudaError_t sticky = cudaGetLastError();        // clears it; the launch's own code names the cause more precisely
+    return e != cudaSuccess ? e : sticky;
 }
 
 bool sweep_config_valid(int lanes, int block)

@@ -175,7 +175,9 @@ def test_reprojection_keeps_a_long_fp32_run_in_SU3(cuda_device):
     assert plain[1] == kept[1] == 1500 and plain[0] == kept[0] == gf.GF_NOT_CONVERGED
     d_plain = oracle.unitarity_defect(np.ascontiguousarray(plain[3]), dims)
     d_kept = oracle.unitarity_defect(np.ascontiguousarray(kept[3]), dims)
-    assert d_plain[0] > 1e-4 and d_kept[0] < 2e-5 and d_kept[1] < 2e-5, (d_plain, d_kept)
+    # measured with the default solver (K and the SU(2) solves in fp64 registers, products g U in fp32): 7.9e-5 without
+    # re-projection, 9e-8 with it (the all-fp32 solver of round 2 lost unitarity faster: 1e-4 .. 8e-4)
+    assert d_plain[0] > 3e-5 and d_kept[0] < 2e-6 and d_kept[1] < 2e-6, (d_plain, d_kept)
     assert abs(oracle.plaquette(np.ascontiguousarray(kept[3]), dims) - P0) < 2e-5
     assert kept[4] >= plain[4] - 1e-6                          # the functional is not worse for it
     assert np.array_equal(kept[3], waits[3]) and kept[2] == waits[2]
