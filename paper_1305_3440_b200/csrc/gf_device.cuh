@@ -106,7 +106,7 @@ __device__ __forceinline__ uint32_t forward_index(const Geom& G, const Site& s, 
 // chunks of a link for one tile now form ONE contiguous run of 32 * RECON * 8 = 4608 / 3072 bytes (the same in fp32
 // with its 64-site tiles): the chunks of one link share DRAM pages, gf_pack / gf_unpack get contiguous runs on this
 // side, and it is what a bulk copy moves per request (the streamed kernel of round 2, measured and removed:
-// profiles/r2_wavefront_attempt.md; a bulk copy costs ~35 ns of TMA time whatever its size, profiles/r2_tma_request_size.txt).  Registers hold a link as m[18] = row-major (re, im) pairs.
+// DESIGN.md section 13; a bulk copy costs ~35 ns of TMA time whatever its size).  Registers hold a link as m[18] = row-major (re, im) pairs.
 
 template <typename T> struct Vec16;
 template <> struct Vec16<double> { using type = double2; };
